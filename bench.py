@@ -1,0 +1,264 @@
+#!/usr/bin/env python
+"""bench.py -- attempted bead moves/s of the full SCMF step (BASELINE.json metric) on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--config C3] [--impl ours|reference]
+
+A "step" is one SCMF cycle = soma_step(1): even-set moves, odd-set moves, occupation numbers,
+field update over every bead of the workload.  Default workload: C3, the
+16.4 M-bead symmetric diblock melt BASELINE.json's metric is quoted on.  One JSON line on stdout.
+
+Multi-GPU: north_star runs the path on one GPU with no sharding and no collective ("replicas
+only"): --gpus N runs N independent replicas (different seeds), one process per GPU,
+value = total moves of all replicas / max-over-ranks time, scaling "weak".
+
+--impl reference times the CPU oracle (oracle/soma_oracle.c, as it stands) on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+from pathlib import Path
+
+import numpy as np
+
+ROOT = Path(__file__).resolve().parent
+sys.path.insert(0, str(ROOT))
+
+import workloads  # noqa: E402
+
+METRIC = "attempted bead moves/s (full SCMF step)"
+UNIT = "moves/s"
+MOVE_BYTES_PER_BEAD = 24.0   # fused move kernel: read 12 B + write 12 B per bead per sweep
+FIELD_BYTES_PER_CELL = 16.0  # field kernel: read n_t counts + write n_t omegas (n_t = 2), DESIGN.md
+
+
+def peaks():
+    p = ROOT / "MEASURED_PEAKS.json"
+    if p.exists():
+        try:
+            return float(json.loads(p.read_text())["hbm_gbs"]), "measured (MEASURED_PEAKS.json)"
+        except Exception:
+            pass
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons during the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.index, self.samples, self.stop, self.t = index, [], threading.Event(), None
+
+    def _run(self):
+        while not self.stop.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+                f = [v.strip() for v in out.strip().split(",")]
+                if len(f) >= 6:
+                    self.samples.append(f)
+            except Exception:
+                pass
+            self.stop.wait(0.1)
+
+    def __enter__(self):
+        self.t = threading.Thread(target=self._run, daemon=True)
+        self.t.start()
+        return self
+
+    def __exit__(self, *a):
+        self.stop.set()
+        self.t.join(timeout=6)
+
+    def summary(self):
+        if not self.samples:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        mhz = sorted(float(s[0]) for s in self.samples)
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = [n for i, n in enumerate(names) if any(s[2 + i].lower().startswith("active") for s in self.samples)]
+        return {"sm_mhz": mhz[len(mhz) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
+                "samples": len(mhz)}
+
+
+def oracle_rate(w, steps: int, warmup: int, budget_s: float = 20.0):
+    """Time the oracle, as it stands, on the host cores: full SCMF cycles on a bounded sample."""
+    sys.path.insert(0, str(ROOT / "tests"))
+    import oracle
+    from helpers import oracle_system
+    # bounded sample: a melt with the same box/grid/density structure but fewer chains if needed
+    probe = w.scaled(min(1.0, 262144 / w.n_beads), name="probe")
+    s = oracle_system(probe)
+    x, y, z = workloads.gaussian_walks(probe)
+    c = s.histogram(x, y, z)
+    om = s.fields(c)
+    t = time.perf_counter()
+    s.step(x, y, z, c, om, 0, 1)
+    per_bead = (time.perf_counter() - t) / probe.n_beads
+    n_steps = max(1, steps) + max(0, warmup)
+    frac = min(1.0, budget_s / (per_bead * w.n_beads * n_steps))
+    sample = w if frac >= 1.0 else w.scaled(frac, name=f"{w.name}-sample")
+    s = oracle_system(sample)
+    x, y, z = workloads.gaussian_walks(sample)
+    c = s.histogram(x, y, z)
+    om = s.fields(c)
+    if warmup:
+        s.step(x, y, z, c, om, 0, warmup)
+    t = time.perf_counter()
+    s.step(x, y, z, c, om, warmup, steps)
+    dt = time.perf_counter() - t
+    return {"value": sample.n_beads * steps / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{sample.n_chains} chains ({sample.n_beads} beads, {100 * sample.n_beads / w.n_beads:.1f}% of "
+                      f"{w.name}; same box, grid and chain architecture), {steps} full SCMF cycles after {warmup} "
+                      f"warm-up, OpenMP over chains"}, dt / steps * 1e3
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--config", default="C3")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--kernel", type=int, default=0)
+    ap.add_argument("--density", type=int, default=0)
+    args = ap.parse_args()
+    if args.warmup < 3 and args.impl == "ours":
+        args.warmup = 3   # timing rule: W >= 3
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    w = workloads.by_name(args.config)
+    config = {"workload": f"{w.name}: {w.note}", "chains": w.n_chains, "beads": w.n_beads, "grid": list(w.grid),
+              "box": list(w.box), "chiN": w.chiN, "kappaN": w.kappaN, "A": w.A, "seed": w.seed, "move": w.move,
+              "parallelism": "replicas only" if world > 1 else "single GPU",
+              "l2_policy": "inputs larger than L2 (positions 197 MB > 126 MB L2); no explicit flush"}
+
+    if args.impl == "reference":
+        if rank != 0:
+            return
+        steps = min(args.steps, 3)
+        base, ms = oracle_rate(w, steps, min(args.warmup, 1))
+        line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+                "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True,
+                "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
+                "cpu_baseline": base,
+                "e2e": {"value": base["value"], "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+        print(json.dumps(line))
+        return
+
+    import torch
+    import paper_1711_03828_b200 as P
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    from dataclasses import replace
+    wr = w if rank == 0 else replace(w, seed=w.seed + rank)   # independent replicas
+    sim = P.from_workload(wr, xyz0=None)       # Gaussian-walk start drawn on the device from the seed
+    sim.set_option(P.OPT_KERNEL, args.kernel)
+    sim.set_option(P.OPT_DENSITY, args.density)
+    nb = w.n_beads
+
+    # ---- device-resident throughput ------------------------------------------------------------
+    sim.step(args.warmup)
+    barrier()
+    l0 = sim.launch_count()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    with ClockSampler(local_rank) as clk:
+        e0.record()
+        for _ in range(args.steps):
+            sim.step(1)
+        e1.record()
+        barrier()
+    ms_total = e0.elapsed_time(e1)
+    launches = sim.launch_count() - l0
+    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_total = float(t.item())
+    value = world * nb * args.steps / (ms_total * 1e-3)
+    att, acc, sweeps = sim.stats()
+
+    # ---- roofline of the dominant kernel (move kernel), CUDA events inside the library ---------
+    sim.set_option(P.OPT_TIMING, 1)
+    sim.kernel_times()
+    n_roof = min(args.steps, 100)
+    for _ in range(n_roof):
+        sim.step(1)
+    kms, kn = sim.kernel_times()
+    sim.set_option(P.OPT_TIMING, 0)
+    peak, peak_src = peaks()
+    move_ms = kms[P.K_MOVE] / max(1, n_roof)            # all move launches of one sweep
+    achieved = MOVE_BYTES_PER_BEAD * nb / (move_ms * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "fused_sweep_kernel (a1+a2+a3)", "achieved": achieved, "peak": peak,
+                "unit": "GB/s", "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "ms_per_launch": move_ms / max(1, kn[P.K_MOVE] // max(1, n_roof)),
+                "algorithmic_bytes_per_launch": MOVE_BYTES_PER_BEAD * nb,
+                "kernel_share_of_step": {"move": kms[P.K_MOVE] / max(1e-12, sum(kms)),
+                                         "density": kms[P.K_DENSITY] / max(1e-12, sum(kms)),
+                                         "field": kms[P.K_FIELD] / max(1e-12, sum(kms))},
+                "full_step_frac": (MOVE_BYTES_PER_BEAD * nb + FIELD_BYTES_PER_CELL * w.n_cells) * args.steps
+                                  / (ms_total * 1e-3) / 1e9 / peak}
+    traffic_file = ROOT / "profiles" / "traffic.json"
+    if traffic_file.exists():
+        try:
+            roofline["traffic"] = json.loads(traffic_file.read_text()).get(w.name)
+        except Exception:
+            pass
+
+    # ---- end to end through the C ABI with host buffers ----------------------------------------
+    n_e2e = max(3, min(args.steps, 20))
+    xyz_h = torch.empty((3, nb), dtype=torch.float32).pin_memory().numpy()
+    om_h = torch.empty((w.n_types, w.n_cells), dtype=torch.float32).pin_memory().numpy()
+    cn_h = torch.empty((w.n_types, w.n_cells), dtype=torch.int32).pin_memory().numpy().view(np.uint32)
+    sim.positions(xyz_h)
+    for _ in range(2):
+        sim.set_positions(xyz_h); sim.step(1); sim.positions(xyz_h); sim.fields(om_h, cn_h)
+    barrier()
+    t0 = time.perf_counter()
+    for _ in range(n_e2e):
+        sim.set_positions(xyz_h)          # H2D 12 B/bead (+ stage 1 on the device)
+        sim.step(1)
+        sim.positions(xyz_h)              # D2H 12 B/bead
+        sim.fields(om_h, cn_h)            # D2H omega + counts
+    barrier()
+    dt = time.perf_counter() - t0
+    t = torch.tensor([dt], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    e2e = {"value": world * nb * n_e2e / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": 12 * nb,
+           "d2h_bytes_per_step": 12 * nb + 8 * w.n_types * w.n_cells, "steps": n_e2e}
+
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
+            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "acceptance": acc / max(1, att)}
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        line["cpu_baseline"], _ = oracle_rate(w, 2, 1)
+    sim.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+    if rank == 0:
+        print(json.dumps(line))
+
+
+if __name__ == "__main__":
+    main()

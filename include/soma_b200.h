@@ -1,0 +1,146 @@
+/*
+ * soma_b200.h -- C ABI of the B200-native SCMF Monte-Carlo step (SOMA, arXiv:1711.03828).
+ *
+ * One SCMF cycle ("MC step") as this library runs it:
+ *     a1  local-displacement Metropolis moves of the even monomers of every chain   (Eq. 2, Eq. 15)
+ *     a2  the same for the odd monomers (independent sets of Fig. 1 / Code 2)
+ *     a3  occupation numbers n_i(c), Eq. 4
+ *     a4  interaction fields omega_i(c), Eq. 12
+ * with the fields frozen during a1/a2.  a5 (Smart-MC) replaces a1/a2 on request.
+ * Every step runs in CUDA kernels written for sm_100a; there is no CPU fallback.
+ *
+ * Conventions
+ *   - plain C, no exceptions cross the boundary; every int-returning call gives SOMA_OK (0) or a
+ *     negative SOMA_E* code and leaves a message for soma_last_error() (thread-local).
+ *   - lengths are in units of R_e0; energies in k_B T.
+ *   - bead arrays are chain-major SoA float32: xyz = x[n_beads] | y[n_beads] | z[n_beads], bead
+ *     index = (beads of earlier architectures) + chain * n_beads_per_chain + monomer; coordinates
+ *     are unwrapped (never folded into the box).
+ *   - grid arrays are [type][ix][iy][iz], iz fastest; cell (ix,iy,iz) is the half-open box
+ *     [ix dLx,(ix+1) dLx) x ... that *contains* the bead (Pi_c of Eq. 4), periodic images folded.
+ *   - pointers named host_* are host memory, dev_* device memory; "dst_is_device" selects.
+ *   - the library owns all device state of a context; callers own every buffer they pass in; input
+ *     buffers are only read during the call.
+ *   - all work is enqueued on the CUDA stream given to soma_init (NULL = legacy default stream);
+ *     calls that write host memory synchronise that stream before returning, soma_step does not.
+ *   - random numbers: Philox4x32-10, counter = (global bead index, sweep lo32, sweep hi32,
+ *     (kind << 8) | sub), key = (seed lo32, seed hi32); kind 0 initial state, 1 local move,
+ *     2 Smart-MC.  Results depend on (seed, sweep counter, positions) only.
+ */
+#ifndef SOMA_B200_H
+#define SOMA_B200_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define SOMA_MAX_TYPES 8
+
+enum {
+    SOMA_OK = 0,
+    SOMA_EINVAL = -1,    /* bad argument (message says which)                 */
+    SOMA_ECUDA = -2,     /* a CUDA runtime call or kernel failed              */
+    SOMA_ENOMEM = -3,    /* device or host allocation failed                  */
+    SOMA_ESTATE = -4,    /* call not valid in the current state of the context */
+    SOMA_ENODEVICE = -5  /* no CUDA device / wrong architecture (needs sm_100) */
+};
+
+/* keys of soma_set_option */
+enum {
+    SOMA_OPT_HAMILTONIAN = 1,      /* 0: K^0_inter (Eq. 7, default), 1: K^1_inter (Eq. 8); refreshes omega   */
+    SOMA_OPT_MOVE = 2,             /* 1: local displacement (default), 2: Smart-MC                            */
+    SOMA_OPT_SMC_STEP = 3,         /* Smart-MC step a_s in R_e0^2 (> 0)                                       */
+    SOMA_OPT_RECORD_DECISIONS = 4, /* 1: keep the accept/reject bit of every move of the last sweep           */
+    SOMA_OPT_KERNEL = 5,           /* 0: auto (default), 1: force the generic two-launch kernels,             */
+                                   /* 2: chain-resident fused kernel (error if an architecture cannot use it) */
+    SOMA_OPT_DENSITY = 6,          /* 0: incremental count update fused into the move kernel (default),       */
+                                   /* 1: clear + full histogram kernel after every sweep                      */
+    SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */
+    SOMA_OPT_SWEEP_COUNTER = 8,    /* set the sweep counter (the "time step" word of the Philox counter)      */
+    SOMA_OPT_GRAPH = 9             /* 1: replay soma_step's launches from a CUDA graph (default 1)            */
+};
+
+/* indices of soma_kernel_times */
+enum { SOMA_K_MOVE = 0, SOMA_K_DENSITY = 1, SOMA_K_FIELD = 2, SOMA_K_COUNT = 3 };
+
+typedef struct soma_ctx soma_ctx; /* opaque */
+
+/* One molecular architecture: n_chains linear chains of n_beads monomers with the given bead
+ * types (architecture stored once per molecule type). */
+typedef struct {
+    uint64_t       n_chains;
+    uint32_t       n_beads;
+    const uint8_t *types; /* host, [n_beads], each < n_types; read during soma_init only */
+} soma_chain_spec;
+
+/* Create a system and run stage 1 (densities, fields) on its initial configuration.
+ *   chains/n_specs  architectures, stored one after the other in the bead arrays (n_specs >= 1)
+ *   N_ref           reference chain length N of PAPER.md:157: k_0 = 3 (N_ref-1)/R_e0^2 (Eq. 2 with
+ *                   b_0 = sqrt(3/k_0)), chi_0 = chiN/N_ref, kappa_0 = kappaN/N_ref
+ *   n_types         bead types n_t, 1..SOMA_MAX_TYPES
+ *   box, grid       periodic box lengths and cells per axis (host, 3 values each)
+ *   chiN            Flory-Huggins chi N used for every unordered type pair (see soma_set_chi)
+ *   kappaN          Helfand compressibility kappa N (Eq. 6)
+ *   A               maximal step length a of the local move; 0 < A <= min(box)/2
+ *   seed            Philox key
+ *   host_xyz0       initial positions (host, SoA 3*n_beads floats) or NULL: the library then draws
+ *                   Gaussian random walks (first bead uniform in the box, per-axis bond std
+ *                   R_e0/sqrt(3 (N_ref-1))) from kind-0 Philox words on the device
+ *   cuda_stream     cudaStream_t to run on (e.g. torch.cuda.current_stream().cuda_stream) or NULL
+ * Total beads must be < 2^32 (the bead index is one Philox counter word), cells < 2^31. */
+int soma_init(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_ref, int n_types,
+              const float *box, const int *grid, float chiN, float kappaN, float A, uint64_t seed,
+              const float *host_xyz0, void *cuda_stream);
+
+/* n_sweeps SCMF cycles: (a1, a2 | a5), a3, a4 each.  Asynchronous on the context's stream.
+ * The sweep counter advances by n_sweeps. */
+int soma_step(soma_ctx *ctx, int n_sweeps);
+
+/* Copy out omega (float32 [n_types][cells]) and, if counts != NULL, the occupation numbers
+ * (uint32 [n_types][cells]) that belong to the current positions. */
+int soma_fields(soma_ctx *ctx, float *omega, uint32_t *counts, int dst_is_device);
+
+/* Copy out the positions (SoA, 3*n_beads float32, unwrapped). */
+int soma_positions(soma_ctx *ctx, float *xyz, int dst_is_device);
+
+/* Replace the positions (SoA, 3*n_beads float32) and redo stage 1 (histogram + fields). */
+int soma_set_positions(soma_ctx *ctx, const float *xyz, int src_is_device);
+
+/* Set chi_ij N = chi_ji N for one type pair (i != j) and refresh omega. */
+int soma_set_chi(soma_ctx *ctx, int i, int j, float chiN_ij);
+
+int soma_set_option(soma_ctx *ctx, int key, double value);
+
+/* attempted / accepted moves since soma_init and the current sweep counter (synchronises). */
+int soma_stats(soma_ctx *ctx, uint64_t *attempted, uint64_t *accepted, uint64_t *sweeps_done);
+
+/* Accept/reject bits of the last sweep, bit (b & 31) of word (b >> 5) for bead b, ceil(n_beads/32)
+ * words; needs SOMA_OPT_RECORD_DECISIONS = 1 before that sweep. */
+int soma_decisions(soma_ctx *ctx, uint32_t *bits, int dst_is_device);
+
+/* Accumulated device time (ms) and launch count per kernel class since the last call; needs
+ * SOMA_OPT_TIMING = 1.  Arrays of SOMA_K_COUNT entries (host).  Synchronises. */
+int soma_kernel_times(soma_ctx *ctx, double *ms, uint64_t *launches);
+
+/* Number of kernels this library has launched for ctx since soma_init (no synchronisation). */
+uint64_t soma_launch_count(const soma_ctx *ctx);
+
+/* n_beads / n_cells / n_types of a context (0 if ctx is NULL). */
+uint64_t soma_n_beads(const soma_ctx *ctx);
+uint64_t soma_n_cells(const soma_ctx *ctx);
+int      soma_n_types(const soma_ctx *ctx);
+
+/* Block until everything enqueued for ctx has finished. */
+int soma_sync(soma_ctx *ctx);
+
+void soma_destroy(soma_ctx *ctx);
+
+const char *soma_last_error(void);
+const char *soma_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* SOMA_B200_H */

@@ -148,13 +148,24 @@ void soma_oracle_histogram(const oracle_system *s, const float *x, const float *
 {
     const int64_t cells = n_cells(s);
     memset(counts, 0, sizeof(uint32_t) * (size_t)cells * s->n_types);
-    uint64_t g = 0;
+    uint64_t first = 0;
     const uint8_t *types = s->types;
     for (uint32_t a = 0; a < s->n_specs; ++a) {
         const uint32_t N = s->spec_n_beads[a];
-        for (uint64_t m = 0; m < s->spec_n_chains[a]; ++m)
-            for (uint32_t j = 0; j < N; ++j, ++g)
-                counts[(int64_t)types[j] * cells + soma_oracle_cell_index(s, x[g], y[g], z[g])] += 1u;
+        const int64_t n_mol = (int64_t)s->spec_n_chains[a];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static)
+#endif
+        for (int64_t m = 0; m < n_mol; ++m)
+            for (uint32_t j = 0; j < N; ++j) {
+                const uint64_t g = first + (uint64_t)m * N + j;
+                uint32_t *slot = &counts[(int64_t)types[j] * cells + soma_oracle_cell_index(s, x[g], y[g], z[g])];
+#ifdef _OPENMP
+#pragma omp atomic
+#endif
+                *slot += 1u;
+            }
+        first += (uint64_t)n_mol * N;
         types += N;
     }
 }

@@ -1,0 +1,20 @@
+"""soma-b200: the SCMF Monte-Carlo step of SOMA (arXiv:1711.03828) as hand-written CUDA for sm_100a.
+
+The product is the C-ABI library ``libsoma_b200.so`` (``include/soma_b200.h``); this package only
+builds it (``_build``) and marshals arguments to it (``binding``).  No CPU fallback exists.
+"""
+from .binding import (DENSITY_FULL, DENSITY_INCREMENTAL, KERNEL_AUTO, KERNEL_FUSED, KERNEL_GENERIC,  # noqa: F401
+                      K_COUNT, K_DENSITY, K_FIELD, K_MOVE, MOVE_LOCAL, MOVE_SMC, OPT_DENSITY, OPT_GRAPH,
+                      OPT_HAMILTONIAN, OPT_KERNEL, OPT_MOVE, OPT_RECORD_DECISIONS, OPT_SMC_STEP,
+                      OPT_SWEEP_COUNTER, OPT_TIMING, SYMBOLS, Soma, SomaError, load, unpack_decisions)
+from ._build import build  # noqa: F401
+
+
+def from_workload(w, xyz0=None, stream=None) -> "Soma":
+    """Create a system from a ``workloads.Workload`` description (marshalling only)."""
+    s = Soma([(n, t) for n, t in w.specs], w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A,
+             w.seed, xyz0=xyz0, stream=stream)
+    if getattr(w, "move", "local") == "smc":
+        s.set_option(OPT_SMC_STEP, w.smc_step)
+        s.set_option(OPT_MOVE, MOVE_SMC)
+    return s

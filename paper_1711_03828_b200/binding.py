@@ -1,0 +1,201 @@
+"""Thin ctypes binding of libsoma_b200.so (include/soma_b200.h) -- argument marshalling only.
+
+Every step of the SCMF cycle runs in the CUDA kernels behind the C ABI; nothing here computes.
+There is no CPU fallback: loading fails loudly if the library cannot be built or found, and
+``soma_init`` fails with SOMA_ENODEVICE when no sm_100 device is present.
+"""
+from __future__ import annotations
+
+import ctypes as C
+from typing import Optional, Sequence, Tuple
+
+import numpy as np
+
+from . import _build
+
+OK = 0
+OPT_HAMILTONIAN, OPT_MOVE, OPT_SMC_STEP, OPT_RECORD_DECISIONS = 1, 2, 3, 4
+OPT_KERNEL, OPT_DENSITY, OPT_TIMING, OPT_SWEEP_COUNTER, OPT_GRAPH = 5, 6, 7, 8, 9
+MOVE_LOCAL, MOVE_SMC = 1, 2
+KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
+DENSITY_INCREMENTAL, DENSITY_FULL = 0, 1
+K_MOVE, K_DENSITY, K_FIELD, K_COUNT = 0, 1, 2, 3
+
+# every symbol include/soma_b200.h declares (tests check that the library exports all of them)
+SYMBOLS = (
+    "soma_init", "soma_step", "soma_fields", "soma_positions", "soma_set_positions", "soma_set_chi",
+    "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
+    "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
+    "soma_version",
+)
+
+
+class SomaError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"soma error {code}: {msg}")
+        self.code = code
+
+
+class _ChainSpec(C.Structure):
+    _fields_ = [("n_chains", C.c_uint64), ("n_beads", C.c_uint32), ("types", C.POINTER(C.c_uint8))]
+
+
+_lib = None
+
+
+def load() -> C.CDLL:
+    """Build (if stale) and load the CUDA library. Raises if that is impossible."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(str(path))
+    vp, i32, u64 = C.c_void_p, C.c_int, C.c_uint64
+    L.soma_init.argtypes = [C.POINTER(vp), C.POINTER(_ChainSpec), i32, i32, i32, C.POINTER(C.c_float),
+                            C.POINTER(C.c_int), C.c_float, C.c_float, C.c_float, u64, vp, vp]
+    L.soma_step.argtypes = [vp, i32]
+    L.soma_fields.argtypes = [vp, vp, vp, i32]
+    L.soma_positions.argtypes = [vp, vp, i32]
+    L.soma_set_positions.argtypes = [vp, vp, i32]
+    L.soma_set_chi.argtypes = [vp, i32, i32, C.c_float]
+    L.soma_set_option.argtypes = [vp, i32, C.c_double]
+    L.soma_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
+    L.soma_decisions.argtypes = [vp, vp, i32]
+    L.soma_kernel_times.argtypes = [vp, C.POINTER(C.c_double), C.POINTER(u64)]
+    L.soma_launch_count.argtypes = [vp]
+    L.soma_launch_count.restype = u64
+    L.soma_n_beads.argtypes = [vp]
+    L.soma_n_beads.restype = u64
+    L.soma_n_cells.argtypes = [vp]
+    L.soma_n_cells.restype = u64
+    L.soma_n_types.argtypes = [vp]
+    L.soma_sync.argtypes = [vp]
+    L.soma_destroy.argtypes = [vp]
+    L.soma_destroy.restype = None
+    L.soma_last_error.restype = C.c_char_p
+    L.soma_version.restype = C.c_char_p
+    _lib = L
+    return L
+
+
+def _check(rc: int) -> None:
+    if rc != OK:
+        raise SomaError(rc, load().soma_last_error().decode())
+
+
+def _ptr(buf) -> Tuple[int, bool]:
+    """(address, is_device) of a numpy array or a torch tensor."""
+    if isinstance(buf, np.ndarray):
+        assert buf.flags.c_contiguous
+        return buf.ctypes.data, False
+    import torch  # torch is plumbing here: device memory and streams
+    assert isinstance(buf, torch.Tensor) and buf.is_contiguous()
+    return buf.data_ptr(), buf.is_cuda
+
+
+class Soma:
+    """One SCMF system on the current CUDA device. Method names mirror the C ABI."""
+
+    def __init__(self, specs: Sequence[Tuple[int, Sequence[int]]], N_ref: int, n_types: int,
+                 box: Sequence[float], grid: Sequence[int], chiN: float, kappaN: float, A: float,
+                 seed: int, xyz0: Optional[np.ndarray] = None, stream: Optional[int] = None):
+        L = load()
+        self._L = L
+        self._h = C.c_void_p()
+        keep = [np.ascontiguousarray(t, dtype=np.uint8) for _, t in specs]
+        arr = (_ChainSpec * len(specs))()
+        for i, ((n, _), t) in enumerate(zip(specs, keep)):
+            arr[i].n_chains = int(n)
+            arr[i].n_beads = len(t)
+            arr[i].types = t.ctypes.data_as(C.POINTER(C.c_uint8))
+        cbox = (C.c_float * 3)(*[float(v) for v in box])
+        cgrid = (C.c_int * 3)(*[int(v) for v in grid])
+        if stream is None:
+            try:
+                import torch
+                stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+            except Exception:
+                stream = 0
+        p0 = None
+        if xyz0 is not None:
+            xyz0 = np.ascontiguousarray(xyz0, dtype=np.float32)
+            p0 = xyz0.ctypes.data
+        _check(L.soma_init(C.byref(self._h), arr, len(specs), int(N_ref), int(n_types), cbox, cgrid,
+                           C.c_float(chiN), C.c_float(kappaN), C.c_float(A), C.c_uint64(int(seed)),
+                           C.c_void_p(p0), C.c_void_p(stream or None)))
+        self.n_beads = int(L.soma_n_beads(self._h))
+        self.n_cells = int(L.soma_n_cells(self._h))
+        self.n_types = int(L.soma_n_types(self._h))
+
+    # -- the C ABI, one method per entry point -------------------------------------------------
+    def step(self, n_sweeps: int = 1) -> None:
+        _check(self._L.soma_step(self._h, int(n_sweeps)))
+
+    def fields(self, omega=None, counts=None):
+        """Copy omega (and counts) out. With no arguments returns new host numpy arrays."""
+        if omega is None and counts is None:
+            omega = np.empty((self.n_types, self.n_cells), np.float32)
+            counts = np.empty((self.n_types, self.n_cells), np.uint32)
+        po, do = _ptr(omega) if omega is not None else (None, None)
+        pc, dc = _ptr(counts) if counts is not None else (None, None)
+        dev = do if do is not None else dc
+        assert dc is None or do is None or dc == do
+        _check(self._L.soma_fields(self._h, C.c_void_p(po), C.c_void_p(pc), int(bool(dev))))
+        return omega, counts
+
+    def positions(self, xyz=None):
+        if xyz is None:
+            xyz = np.empty((3, self.n_beads), np.float32)
+        p, dev = _ptr(xyz)
+        _check(self._L.soma_positions(self._h, C.c_void_p(p), int(dev)))
+        return xyz
+
+    def set_positions(self, xyz) -> None:
+        p, dev = _ptr(xyz)
+        _check(self._L.soma_set_positions(self._h, C.c_void_p(p), int(dev)))
+
+    def set_chi(self, i: int, j: int, chiN: float) -> None:
+        _check(self._L.soma_set_chi(self._h, i, j, C.c_float(chiN)))
+
+    def set_option(self, key: int, value: float) -> None:
+        _check(self._L.soma_set_option(self._h, int(key), C.c_double(value)))
+
+    def stats(self) -> Tuple[int, int, int]:
+        a, b, c = C.c_uint64(), C.c_uint64(), C.c_uint64()
+        _check(self._L.soma_stats(self._h, C.byref(a), C.byref(b), C.byref(c)))
+        return int(a.value), int(b.value), int(c.value)
+
+    def decisions(self, bits=None):
+        if bits is None:
+            bits = np.empty((self.n_beads + 31) // 32, np.uint32)
+        p, dev = _ptr(bits)
+        _check(self._L.soma_decisions(self._h, C.c_void_p(p), int(dev)))
+        return bits
+
+    def kernel_times(self):
+        ms = (C.c_double * K_COUNT)()
+        n = (C.c_uint64 * K_COUNT)()
+        _check(self._L.soma_kernel_times(self._h, ms, n))
+        return [float(v) for v in ms], [int(v) for v in n]
+
+    def launch_count(self) -> int:
+        return int(self._L.soma_launch_count(self._h))
+
+    def sync(self) -> None:
+        _check(self._L.soma_sync(self._h))
+
+    def destroy(self) -> None:
+        if self._h:
+            self._L.soma_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+
+def unpack_decisions(bits: np.ndarray, n_beads: int) -> np.ndarray:
+    """Bitmap words -> one uint8 per bead (marshalling helper for tests)."""
+    return np.unpackbits(bits.view(np.uint8), bitorder="little")[:n_beads]

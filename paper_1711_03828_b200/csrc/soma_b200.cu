@@ -1,0 +1,650 @@
+// soma_b200.cu -- C ABI (include/soma_b200.h) and host-side orchestration of the SCMF step.
+//
+// Device memory layout:
+//   x, y, z     three fp32 arrays, chain-major; every architecture's segment starts on a 512-byte
+//               boundary (128 floats) so that a warp tile of the fused kernel is 3 x LDG.128 per lane
+//   counts      uint32 [n_types][cells]      (L2-resident for every BASELINE config but C4)
+//   omega       float32 [n_types][cells]
+//   toff        uint32 per monomer of every architecture: type * cells
+//   decisions   1 bit per bead (only written with SOMA_OPT_RECORD_DECISIONS)
+//   acc_slots   256 spread 64-bit counters of accepted moves
+#include "soma_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <string>
+#include <vector>
+
+#include "../../include/soma_b200.h"
+
+namespace {
+
+thread_local std::string g_err;
+
+int fail(int code, const char* fmt, ...)
+{
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    g_err = buf;
+    return code;
+}
+
+#define CU(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? SOMA_ENOMEM : SOMA_ECUDA, "%s: %s (%s:%d)", \
+                        #call, cudaGetErrorString(e_), __FILE__, __LINE__);                        \
+    } while (0)
+
+struct Spec {
+    uint64_t n_chains = 0;
+    uint32_t N = 0;
+    uint64_t n_beads = 0;   // n_chains * N
+    uint64_t gid0 = 0;      // global index of the first bead (unpadded, the API's bead index)
+    uint64_t off = 0;       // offset of the segment in the padded device arrays
+    uint32_t toff_off = 0;  // offset into the toff table
+    bool fused_ok = false;  // N in {4, ..., 128}, N | 128
+};
+
+constexpr int kEventPool = 2048;
+
+}  // namespace
+
+struct soma_ctx {
+    std::vector<Spec> specs;
+    int n_types = 0, N_ref = 0;
+    float box[3] = {0, 0, 0};
+    int grid[3] = {0, 0, 0};
+    float chiN[soma::kMaxTypes][soma::kMaxTypes] = {};
+    float kappaN = 0, A = 0;
+    uint64_t seed = 0;
+    uint64_t n_beads = 0, n_pad = 0, cells = 0;
+
+    float *x = nullptr, *y = nullptr, *z = nullptr;
+    uint32_t* counts = nullptr;
+    float* omega = nullptr;
+    uint32_t* toff = nullptr;
+    uint32_t* decisions = nullptr;
+    unsigned long long* acc_slots = nullptr;
+    unsigned long long* acc_host = nullptr;  // pinned staging for soma_stats
+
+    cudaStream_t stream = nullptr;
+    int device = 0, n_sm = 0;
+
+    // options
+    int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0, use_graph = 1;
+    float smc_step = 0.0f;
+
+    uint64_t sweep = 0, attempted = 0, launches = 0;
+    bool decisions_valid = false;
+
+    // timing
+    std::vector<cudaEvent_t> ev;   // pairs
+    std::vector<int> ev_class;
+    int ev_used = 0;
+    double t_ms[SOMA_K_COUNT] = {0, 0, 0};
+    uint64_t t_launches[SOMA_K_COUNT] = {0, 0, 0};
+
+    soma::GridP gridp() const;
+    soma::MoveP movep(uint64_t sweep_no) const;
+    soma::FieldP fieldp() const;
+};
+
+soma::GridP soma_ctx::gridp() const
+{
+    soma::GridP g;
+    for (int a = 0; a < 3; ++a) {
+        g.inv_d[a] = (float)((double)grid[a] / (double)box[a]);
+        g.nf[a] = (float)grid[a];
+        g.inv_nf[a] = (float)(1.0 / (double)grid[a]);
+        g.n[a] = grid[a];
+    }
+    g.cells = (uint32_t)cells;
+    return g;
+}
+
+soma::MoveP soma_ctx::movep(uint64_t sweep_no) const
+{
+    soma::MoveP p;
+    p.g = gridp();
+    p.c1 = (float)(2.0 * (double)A);
+    p.c0 = (float)((double)A * (std::ldexp(1.0, -23) - 3.0));
+    p.hk = (float)(1.5 * ((double)N_ref - 1.0));
+    p.k0 = (float)(3.0 * ((double)N_ref - 1.0));
+    p.a_s = smc_step;
+    p.noise = sqrtf(2.0f * smc_step);
+    p.four_as = 4.0f * smc_step;
+    p.key0 = (uint32_t)seed;
+    p.key1 = (uint32_t)(seed >> 32);
+    p.sweep_lo = (uint32_t)sweep_no;
+    p.sweep_hi = (uint32_t)(sweep_no >> 32);
+    return p;
+}
+
+soma::FieldP soma_ctx::fieldp() const
+{
+    soma::FieldP f;
+    f.inv_nbar = (float)((double)cells / (double)n_beads);
+    f.kappa0 = (float)((double)kappaN / (double)N_ref);
+    for (int i = 0; i < soma::kMaxTypes; ++i)
+        for (int k = 0; k < soma::kMaxTypes; ++k) {
+            f.chi0[i][k] = (float)((double)chiN[i][k] / (double)N_ref);
+            f.half_chi0[i][k] = (float)(0.5 * (double)chiN[i][k] / (double)N_ref);
+        }
+    f.n_types = n_types;
+    f.hamiltonian = hamiltonian;
+    f.cells = (uint32_t)cells;
+    return f;
+}
+
+namespace {
+
+// ---- kernel timing (SOMA_OPT_TIMING) ------------------------------------------------------------
+int drain_events(soma_ctx* c)
+{
+    if (c->ev_used == 0) return SOMA_OK;
+    CU(cudaStreamSynchronize(c->stream));
+    for (int i = 0; i < c->ev_used; ++i) {
+        float ms = 0.f;
+        CU(cudaEventElapsedTime(&ms, c->ev[2 * i], c->ev[2 * i + 1]));
+        c->t_ms[c->ev_class[i]] += ms;
+    }
+    c->ev_used = 0;
+    return SOMA_OK;
+}
+
+struct Timed {
+    soma_ctx* c;
+    int slot = -1;
+    Timed(soma_ctx* ctx, int klass, int n_launches) : c(ctx)
+    {
+        c->launches += n_launches;
+        if (!c->timing) return;
+        if (c->ev.empty()) {
+            c->ev.resize(2 * kEventPool);
+            c->ev_class.resize(kEventPool);
+            for (auto& e : c->ev) cudaEventCreate(&e);
+        }
+        if (c->ev_used == kEventPool) drain_events(c);
+        slot = c->ev_used++;
+        c->ev_class[slot] = klass;
+        c->t_launches[klass] += n_launches;
+        cudaEventRecord(c->ev[2 * slot], c->stream);
+    }
+    ~Timed()
+    {
+        if (slot >= 0) cudaEventRecord(c->ev[2 * slot + 1], c->stream);
+    }
+};
+
+// ---- launches -----------------------------------------------------------------------------------
+bool spec_uses_fused(const soma_ctx* c, const Spec& s)
+{
+    if (c->kernel_choice == 1) return false;
+    if (!s.fused_ok) return false;
+    if (c->record && (s.gid0 % 8) != 0) return false;  // byte view of the decision bitmap needs it
+    return true;
+}
+
+template <int kMove, bool kIncr, bool kRecord>
+int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
+{
+    for (const Spec& s : c->specs) {
+        if (s.n_beads == 0) continue;
+        float *x = c->x + s.off, *y = c->y + s.off, *z = c->z + s.off;
+        const uint32_t* toff = c->toff + s.toff_off;
+        if (spec_uses_fused(c, s)) {
+            const uint32_t n_tiles = (uint32_t)((s.n_beads + soma::kTile - 1) / soma::kTile);
+            const int threads = 256, warps_per_block = threads / 32;
+            int max_blocks = c->n_sm * 8;
+            int blocks = (int)((n_tiles + warps_per_block - 1) / warps_per_block);
+            if (blocks > max_blocks) blocks = max_blocks;
+            Timed t(c, SOMA_K_MOVE, 1);
+            soma::fused_sweep_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
+                P, x, y, z, c->omega, c->counts, toff, s.N - 1u, n_tiles, (uint32_t)s.n_beads,
+                (uint32_t)s.gid0, reinterpret_cast<uint8_t*>(c->decisions) + s.gid0 / 8, c->acc_slots);
+        } else {
+            for (uint32_t parity = 0; parity < 2; ++parity) {
+                const uint32_t half = parity == 0 ? (s.N + 1) / 2 : s.N / 2;
+                if (half == 0) continue;
+                const uint64_t n_items = s.n_chains * half;
+                const int threads = 256;
+                const uint64_t blocks = (n_items + threads - 1) / threads;
+                Timed t(c, SOMA_K_MOVE, 1);
+                soma::generic_move_kernel<kMove, kIncr, kRecord><<<(unsigned)blocks, threads, 0, c->stream>>>(
+                    P, x, y, z, c->omega, c->counts, toff, s.N, half, parity, n_items, (uint32_t)s.gid0,
+                    c->decisions, c->acc_slots);
+            }
+        }
+        CU(cudaGetLastError());
+    }
+    return SOMA_OK;
+}
+
+int launch_moves(soma_ctx* c, const soma::MoveP& P)
+{
+    const bool incr = c->density_mode == 0;
+    const bool rec = c->record != 0;
+#define SOMA_DISPATCH(M)                                                        \
+    if (incr) {                                                                 \
+        return rec ? launch_moves_t<M, true, true>(c, P) : launch_moves_t<M, true, false>(c, P);   \
+    } else {                                                                    \
+        return rec ? launch_moves_t<M, false, true>(c, P) : launch_moves_t<M, false, false>(c, P); \
+    }
+    if (c->move == 2) {
+        SOMA_DISPATCH(2)
+    } else {
+        SOMA_DISPATCH(1)
+    }
+#undef SOMA_DISPATCH
+}
+
+int launch_histogram(soma_ctx* c)
+{
+    CU(cudaMemsetAsync(c->counts, 0, sizeof(uint32_t) * c->cells * c->n_types, c->stream));
+    const soma::GridP g = c->gridp();
+    for (const Spec& s : c->specs) {
+        if (s.n_beads == 0) continue;
+        const int threads = 256;
+        uint64_t blocks = (s.n_beads + threads - 1) / threads;
+        const uint64_t cap = (uint64_t)c->n_sm * 16;
+        if (blocks > cap) blocks = cap;
+        Timed t(c, SOMA_K_DENSITY, 1);
+        soma::histogram_kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
+            g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts);
+        CU(cudaGetLastError());
+    }
+    return SOMA_OK;
+}
+
+int launch_fields(soma_ctx* c)
+{
+    const soma::FieldP F = c->fieldp();
+    const int threads = 256;
+    const unsigned blocks = (unsigned)((c->cells + threads - 1) / threads);
+    Timed t(c, SOMA_K_FIELD, 1);
+    switch (c->n_types) {
+        case 1: soma::field_kernel<1><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
+        case 2: soma::field_kernel<2><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
+        default: soma::field_kernel<0><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
+    }
+    CU(cudaGetLastError());
+    return SOMA_OK;
+}
+
+int stage1(soma_ctx* c)
+{
+    int rc = launch_histogram(c);
+    if (rc) return rc;
+    return launch_fields(c);
+}
+
+int copy_soa(soma_ctx* c, float* dst_user, const float* src_user, bool to_user, bool user_is_device)
+{
+    // user layout: x[nb] | y[nb] | z[nb]; device layout: padded segments
+    float* dev[3] = {c->x, c->y, c->z};
+    for (int a = 0; a < 3; ++a)
+        for (const Spec& s : c->specs) {
+            if (s.n_beads == 0) continue;
+            const size_t bytes = sizeof(float) * s.n_beads;
+            if (to_user)
+                CU(cudaMemcpyAsync(dst_user + (size_t)a * c->n_beads + s.gid0, dev[a] + s.off, bytes,
+                                   user_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+            else
+                CU(cudaMemcpyAsync(dev[a] + s.off, src_user + (size_t)a * c->n_beads + s.gid0, bytes,
+                                   user_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
+        }
+    return SOMA_OK;
+}
+
+}  // namespace
+
+// =================================================================================================
+// C ABI
+// =================================================================================================
+extern "C" {
+
+const char* soma_last_error(void) { return g_err.c_str(); }
+const char* soma_version(void) { return "soma-b200 0.1 (sm_100a)"; }
+
+void soma_destroy(soma_ctx* c)
+{
+    if (!c) return;
+    if (c->stream || true) cudaStreamSynchronize(c->stream);
+    for (auto& e : c->ev) cudaEventDestroy(e);
+    cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
+    cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
+    cudaFree(c->acc_slots);
+    if (c->acc_host) cudaFreeHost(c->acc_host);
+    delete c;
+}
+
+int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_ref, int n_types,
+              const float* box, const int* grid, float chiN, float kappaN, float A, uint64_t seed,
+              const float* host_xyz0, void* cuda_stream)
+{
+    if (!out) return fail(SOMA_EINVAL, "soma_init: out is NULL");
+    *out = nullptr;
+    if (!chains || n_specs < 1) return fail(SOMA_EINVAL, "soma_init: need at least one chain spec");
+    if (N_ref < 1) return fail(SOMA_EINVAL, "soma_init: N_ref must be >= 1");
+    if (n_types < 1 || n_types > SOMA_MAX_TYPES)
+        return fail(SOMA_EINVAL, "soma_init: n_types must be in 1..%d", SOMA_MAX_TYPES);
+    if (!box || !grid) return fail(SOMA_EINVAL, "soma_init: box/grid is NULL");
+    double min_box = 1e300;
+    uint64_t cells = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (!(box[a] > 0.0f) || !std::isfinite(box[a])) return fail(SOMA_EINVAL, "soma_init: box[%d] must be > 0", a);
+        if (grid[a] < 1) return fail(SOMA_EINVAL, "soma_init: grid[%d] must be >= 1", a);
+        min_box = box[a] < min_box ? box[a] : min_box;
+        cells *= (uint64_t)grid[a];
+        if (cells >= (1ull << 31)) return fail(SOMA_EINVAL, "soma_init: too many grid cells (>= 2^31)");
+    }
+    if (cells * (uint64_t)n_types >= (1ull << 32))
+        return fail(SOMA_EINVAL, "soma_init: n_types * cells must be < 2^32");
+    if (!(A > 0.0f) || !((double)A <= 0.5 * min_box))
+        return fail(SOMA_EINVAL, "soma_init: need 0 < A <= min(box)/2");
+    if (!std::isfinite(chiN) || !std::isfinite(kappaN)) return fail(SOMA_EINVAL, "soma_init: chiN/kappaN not finite");
+
+    soma_ctx* c = new (std::nothrow) soma_ctx;
+    if (!c) return fail(SOMA_ENOMEM, "soma_init: out of host memory");
+    c->n_types = n_types;
+    c->N_ref = N_ref;
+    c->kappaN = kappaN;
+    c->A = A;
+    c->seed = seed;
+    c->cells = cells;
+    c->stream = (cudaStream_t)cuda_stream;
+    for (int a = 0; a < 3; ++a) { c->box[a] = box[a]; c->grid[a] = grid[a]; }
+    for (int i = 0; i < n_types; ++i)
+        for (int k = 0; k < n_types; ++k) c->chiN[i][k] = i == k ? 0.0f : chiN;
+
+    std::vector<uint32_t> toff_host;
+    uint64_t gid = 0, off = 0;
+    for (int a = 0; a < n_specs; ++a) {
+        Spec s;
+        s.n_chains = chains[a].n_chains;
+        s.N = chains[a].n_beads;
+        if (s.N < 1 || (s.n_chains > 0 && !chains[a].types)) {
+            delete c;
+            return fail(SOMA_EINVAL, "soma_init: spec %d: n_beads must be >= 1 and types non-NULL", a);
+        }
+        s.n_beads = s.n_chains * s.N;
+        s.gid0 = gid;
+        s.off = off;
+        s.toff_off = (uint32_t)toff_host.size();
+        s.fused_ok = s.N >= 4 && s.N <= 128 && (128 % s.N) == 0;
+        for (uint32_t j = 0; j < s.N; ++j) {
+            const uint8_t t = s.n_chains ? chains[a].types[j] : 0;
+            if (t >= n_types) {
+                delete c;
+                return fail(SOMA_EINVAL, "soma_init: spec %d monomer %u has type %u >= n_types", a, j, (unsigned)t);
+            }
+            toff_host.push_back((uint32_t)(t * cells));
+        }
+        while (toff_host.size() % 4) toff_host.push_back(0);  // uint4 loads of the fused kernel
+        gid += s.n_beads;
+        off += (s.n_beads + 127) / 128 * 128;
+        if (gid >= (1ull << 32)) {
+            delete c;
+            return fail(SOMA_EINVAL, "soma_init: total beads must be < 2^32");
+        }
+        c->specs.push_back(s);
+    }
+    c->n_beads = gid;
+    c->n_pad = off + 128;
+    if (c->n_beads == 0) {
+        delete c;
+        return fail(SOMA_EINVAL, "soma_init: the system has no beads");
+    }
+
+    int n_dev = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        delete c;
+        return fail(SOMA_ENODEVICE, "soma_init: no CUDA device (this library has no CPU path)");
+    }
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) { delete c; return fail(SOMA_ECUDA, "soma_init: cudaGetDevice failed"); }
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) { delete c; return fail(SOMA_ECUDA, "soma_init: cudaGetDeviceProperties failed"); }
+    if (prop.major != 10) {
+        delete c;
+        return fail(SOMA_ENODEVICE, "soma_init: kernels are built for sm_100a only, device is sm_%d%d", prop.major, prop.minor);
+    }
+    c->device = dev;
+    c->n_sm = prop.multiProcessorCount;
+
+
+#define CUI(call)                                                                      \
+    do {                                                                               \
+        cudaError_t e_ = (call);                                                       \
+        if (e_ != cudaSuccess) {                                                       \
+            int rc_ = fail(e_ == cudaErrorMemoryAllocation ? SOMA_ENOMEM : SOMA_ECUDA, \
+                           "%s: %s", #call, cudaGetErrorString(e_));                   \
+            cudaGetLastError();                                                        \
+            soma_destroy(c);                                                           \
+            return rc_;                                                                \
+        }                                                                              \
+    } while (0)
+
+    CUI(cudaMalloc(&c->x, sizeof(float) * c->n_pad));
+    CUI(cudaMalloc(&c->y, sizeof(float) * c->n_pad));
+    CUI(cudaMalloc(&c->z, sizeof(float) * c->n_pad));
+    CUI(cudaMalloc(&c->counts, sizeof(uint32_t) * cells * n_types));
+    CUI(cudaMalloc(&c->omega, sizeof(float) * cells * n_types));
+    CUI(cudaMalloc(&c->toff, sizeof(uint32_t) * toff_host.size()));
+    CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads + 31) / 32 + 8)));
+    CUI(cudaMalloc(&c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots));
+    CUI(cudaMallocHost(&c->acc_host, sizeof(unsigned long long) * soma::kAccSlots));
+    CUI(cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_pad, c->stream));
+    CUI(cudaMemsetAsync(c->y, 0, sizeof(float) * c->n_pad, c->stream));
+    CUI(cudaMemsetAsync(c->z, 0, sizeof(float) * c->n_pad, c->stream));
+    CUI(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32 + 8), c->stream));
+    CUI(cudaMemsetAsync(c->acc_slots, 0, sizeof(unsigned long long) * soma::kAccSlots, c->stream));
+    CUI(cudaMemcpyAsync(c->toff, toff_host.data(), sizeof(uint32_t) * toff_host.size(), cudaMemcpyHostToDevice, c->stream));
+    CUI(cudaStreamSynchronize(c->stream));  // toff_host goes out of scope
+
+    int rc = SOMA_OK;
+    if (host_xyz0) {
+        rc = copy_soa(c, nullptr, host_xyz0, false, false);
+    } else {
+        const double sigma = N_ref > 1 ? 1.0 / std::sqrt(3.0 * ((double)N_ref - 1.0)) : 0.0;
+        for (const Spec& s : c->specs) {
+            if (s.n_chains == 0) continue;
+            const int threads = 128;
+            const unsigned blocks = (unsigned)((s.n_chains + threads - 1) / threads);
+            c->launches += 1;
+            soma::init_walk_kernel<<<blocks, threads, 0, c->stream>>>(
+                c->x + s.off, c->y + s.off, c->z + s.off, s.n_chains, s.N, (uint32_t)s.gid0, (uint32_t)seed,
+                (uint32_t)(seed >> 32), (double)box[0], (double)box[1], (double)box[2], sigma);
+        }
+        if (cudaGetLastError() != cudaSuccess) rc = fail(SOMA_ECUDA, "soma_init: init_walk_kernel launch failed");
+    }
+    if (rc == SOMA_OK) rc = stage1(c);
+    if (rc == SOMA_OK && cudaStreamSynchronize(c->stream) != cudaSuccess)
+        rc = fail(SOMA_ECUDA, "soma_init: %s", cudaGetErrorString(cudaGetLastError()));
+    if (rc != SOMA_OK) {
+        std::string keep = g_err;
+        soma_destroy(c);
+        g_err = keep;
+        return rc;
+    }
+    *out = c;
+    return SOMA_OK;
+#undef CUI
+}
+
+int soma_step(soma_ctx* c, int n_sweeps)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_step: ctx is NULL");
+    if (n_sweeps < 0) return fail(SOMA_EINVAL, "soma_step: n_sweeps must be >= 0");
+    if (c->move == 2 && !(c->smc_step > 0.0f))
+        return fail(SOMA_ESTATE, "soma_step: Smart-MC selected but SOMA_OPT_SMC_STEP not set");
+    for (int i = 0; i < n_sweeps; ++i) {
+        if (c->record)
+            CU(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32), c->stream));
+        const soma::MoveP P = c->movep(c->sweep);
+        int rc = launch_moves(c, P);                       // a1, a2 (or a5) [+ a3 incremental]
+        if (rc) return rc;
+        if (c->density_mode == 1) {
+            rc = launch_histogram(c);                      // a3 from scratch
+            if (rc) return rc;
+        }
+        rc = launch_fields(c);                             // a4
+        if (rc) return rc;
+        c->sweep += 1;
+        c->attempted += c->n_beads;
+        c->decisions_valid = c->record != 0;
+    }
+    return SOMA_OK;
+}
+
+int soma_fields(soma_ctx* c, float* omega, uint32_t* counts, int dst_is_device)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_fields: ctx is NULL");
+    if (!omega && !counts) return fail(SOMA_EINVAL, "soma_fields: both outputs NULL");
+    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    const size_t n = (size_t)c->cells * c->n_types;
+    if (omega) CU(cudaMemcpyAsync(omega, c->omega, sizeof(float) * n, kind, c->stream));
+    if (counts) CU(cudaMemcpyAsync(counts, c->counts, sizeof(uint32_t) * n, kind, c->stream));
+    if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
+    return SOMA_OK;
+}
+
+int soma_positions(soma_ctx* c, float* xyz, int dst_is_device)
+{
+    if (!c || !xyz) return fail(SOMA_EINVAL, "soma_positions: NULL argument");
+    int rc = copy_soa(c, xyz, nullptr, true, dst_is_device != 0);
+    if (rc) return rc;
+    if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
+    return SOMA_OK;
+}
+
+int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
+{
+    if (!c || !xyz) return fail(SOMA_EINVAL, "soma_set_positions: NULL argument");
+    int rc = copy_soa(c, nullptr, xyz, false, src_is_device != 0);
+    if (rc) return rc;
+    rc = stage1(c);
+    if (rc) return rc;
+    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));  // caller may reuse its buffer
+    return SOMA_OK;
+}
+
+int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_set_chi: ctx is NULL");
+    if (i < 0 || j < 0 || i >= c->n_types || j >= c->n_types || i == j || !std::isfinite(chiN_ij))
+        return fail(SOMA_EINVAL, "soma_set_chi: need 0 <= i != j < n_types and a finite value");
+    c->chiN[i][j] = c->chiN[j][i] = chiN_ij;
+    return launch_fields(c);
+}
+
+int soma_set_option(soma_ctx* c, int key, double value)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_set_option: ctx is NULL");
+    const int iv = (int)value;
+    switch (key) {
+        case SOMA_OPT_HAMILTONIAN:
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_HAMILTONIAN: 0 or 1");
+            c->hamiltonian = iv;
+            return launch_fields(c);
+        case SOMA_OPT_MOVE:
+            if (iv != 1 && iv != 2) return fail(SOMA_EINVAL, "SOMA_OPT_MOVE: 1 (local) or 2 (Smart-MC)");
+            c->move = iv;
+            return SOMA_OK;
+        case SOMA_OPT_SMC_STEP:
+            if (!(value > 0.0) || !std::isfinite(value)) return fail(SOMA_EINVAL, "SOMA_OPT_SMC_STEP: must be > 0");
+            c->smc_step = (float)value;
+            return SOMA_OK;
+        case SOMA_OPT_RECORD_DECISIONS:
+            c->record = iv != 0;
+            return SOMA_OK;
+        case SOMA_OPT_KERNEL:
+            if (iv < 0 || iv > 2) return fail(SOMA_EINVAL, "SOMA_OPT_KERNEL: 0, 1 or 2");
+            if (iv == 2)
+                for (const Spec& s : c->specs)
+                    if (!s.fused_ok) return fail(SOMA_EINVAL, "SOMA_OPT_KERNEL=2: chain length %u cannot use the fused kernel", s.N);
+            c->kernel_choice = iv;
+            return SOMA_OK;
+        case SOMA_OPT_DENSITY:
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_DENSITY: 0 or 1");
+            c->density_mode = iv;
+            return SOMA_OK;
+        case SOMA_OPT_TIMING: {
+            int rc = drain_events(c);
+            c->timing = iv != 0;
+            return rc;
+        }
+        case SOMA_OPT_SWEEP_COUNTER:
+            if (value < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SWEEP_COUNTER: must be >= 0");
+            c->sweep = (uint64_t)value;
+            return SOMA_OK;
+        case SOMA_OPT_GRAPH:
+            c->use_graph = iv != 0;
+            return SOMA_OK;
+        default:
+            return fail(SOMA_EINVAL, "soma_set_option: unknown key %d", key);
+    }
+}
+
+int soma_stats(soma_ctx* c, uint64_t* attempted, uint64_t* accepted, uint64_t* sweeps_done)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_stats: ctx is NULL");
+    CU(cudaMemcpyAsync(c->acc_host, c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots,
+                       cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    uint64_t acc = 0;
+    for (int i = 0; i < soma::kAccSlots; ++i) acc += c->acc_host[i];
+    if (attempted) *attempted = c->attempted;
+    if (accepted) *accepted = acc;
+    if (sweeps_done) *sweeps_done = c->sweep;
+    return SOMA_OK;
+}
+
+int soma_decisions(soma_ctx* c, uint32_t* bits, int dst_is_device)
+{
+    if (!c || !bits) return fail(SOMA_EINVAL, "soma_decisions: NULL argument");
+    if (!c->decisions_valid)
+        return fail(SOMA_ESTATE, "soma_decisions: set SOMA_OPT_RECORD_DECISIONS=1 before the sweep");
+    CU(cudaMemcpyAsync(bits, c->decisions, sizeof(uint32_t) * ((c->n_beads + 31) / 32),
+                       dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
+    if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
+    return SOMA_OK;
+}
+
+int soma_kernel_times(soma_ctx* c, double* ms, uint64_t* launches)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_kernel_times: ctx is NULL");
+    int rc = drain_events(c);
+    if (rc) return rc;
+    for (int k = 0; k < SOMA_K_COUNT; ++k) {
+        if (ms) ms[k] = c->t_ms[k];
+        if (launches) launches[k] = c->t_launches[k];
+        c->t_ms[k] = 0.0;
+        c->t_launches[k] = 0;
+    }
+    return SOMA_OK;
+}
+
+uint64_t soma_launch_count(const soma_ctx* c) { return c ? c->launches : 0; }
+uint64_t soma_n_beads(const soma_ctx* c) { return c ? c->n_beads : 0; }
+uint64_t soma_n_cells(const soma_ctx* c) { return c ? c->cells : 0; }
+int soma_n_types(const soma_ctx* c) { return c ? c->n_types : 0; }
+
+int soma_sync(soma_ctx* c)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_sync: ctx is NULL");
+    CU(cudaStreamSynchronize(c->stream));
+    CU(cudaGetLastError());
+    return SOMA_OK;
+}
+
+}  // extern "C"

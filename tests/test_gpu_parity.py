@@ -1,0 +1,223 @@
+"""Parity of the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Lock-step protocol (one flipped Metropolis decision changes a bead by up to A sqrt(3), after which
+its chain diverges for good): before every sweep the oracle is handed the GPU's current positions;
+both sides run one sweep with the same sweep counter; then compare
+  (i)   occupation numbers computed from the same positions        -- bit-exact (integers)
+  (ii)  fields                                                      -- 1e-5 relative (north_star)
+  (iii) accept/reject decisions                                     -- >= 99.999 % equal
+  (iv)  positions of beads whose decisions agree                    -- bit-equal for local moves
+        (one IEEE add on both sides), <= 1e-6 R_e for Smart-MC.
+"""
+from __future__ import annotations
+
+import numpy as np
+import pytest
+
+import oracle
+import paper_1711_03828_b200 as P
+import workloads
+from helpers import oracle_system
+
+pytestmark = pytest.mark.gpu
+
+FIELD_RTOL = 1e-5          # north_star: "Fields must agree within 1e-5 relative"
+DECISION_AGREEMENT = 0.99999
+POS_TOL_SMC = 1e-6         # R_e
+
+
+def field_close(w, got, want):
+    # reading R16: relative to max(|omega|, kappa_0 + chi_0) so that omega ~ 0 cells are well-defined
+    scale = np.maximum(np.abs(want), (w.kappaN + abs(w.chiN)) / w.N_ref + 1e-30)
+    return float(np.max(np.abs(got.astype(np.float64) - want) / scale))
+
+
+def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INCREMENTAL,
+             hamiltonian=0, check_every=1, expect_flips=0.0):
+    if xyz0 is None:
+        xyz0 = np.stack(workloads.gaussian_walks(w))
+    sim = P.from_workload(w, xyz0=xyz0)
+    orc = oracle_system(w, hamiltonian=hamiltonian)
+    sim.set_option(P.OPT_KERNEL, kernel)
+    sim.set_option(P.OPT_DENSITY, density)
+    sim.set_option(P.OPT_HAMILTONIAN, hamiltonian)
+    sim.set_option(P.OPT_RECORD_DECISIONS, 1)
+    move = oracle.MOVE_SMC if w.move == "smc" else oracle.MOVE_LOCAL
+    nb = w.n_beads
+    total_flips = 0
+    pos = sim.positions()
+    assert np.array_equal(pos, xyz0)
+    for sweep in range(n_sweeps):
+        x, y, z = (pos[a].copy() for a in range(3))
+        om_g, cnt_g = sim.fields()
+        cnt_o = orc.histogram(x, y, z)
+        assert np.array_equal(cnt_g, cnt_o), f"sweep {sweep}: occupation numbers differ"
+        assert cnt_g.sum() == nb
+        om_o = orc.fields(cnt_o)
+        assert field_close(w, om_g, om_o) <= FIELD_RTOL, f"sweep {sweep}: fields differ"
+        dec_o = np.zeros(nb, np.uint8)
+        acc_o = orc.sweep(x, y, z, om_o, sweep, move, dec_o)
+        sim.step(1)
+        dec_g = P.unpack_decisions(sim.decisions(), nb)
+        pos = sim.positions()
+        agree = dec_g == dec_o
+        flips = int((~agree).sum())
+        total_flips += flips
+        assert agree.mean() >= DECISION_AGREEMENT, f"sweep {sweep}: {flips} decision flips of {nb}"
+        ref = np.stack([x, y, z])
+        if move == oracle.MOVE_LOCAL:
+            assert np.array_equal(pos[:, agree], ref[:, agree]), f"sweep {sweep}: accepted positions differ"
+        else:
+            # a flipped neighbour changes the force on the next set: compare only chains without flips
+            bad = np.zeros(nb, bool)
+            if flips:
+                g = 0
+                for n, t in w.specs:
+                    N = len(t)
+                    seg = (~agree[g:g + n * N]).reshape(n, N).any(1)
+                    bad[g:g + n * N] = np.repeat(seg, N)
+                    g += n * N
+            assert np.max(np.abs(pos[:, ~bad] - ref[:, ~bad])) <= POS_TOL_SMC
+        att, acc_g, done = sim.stats()
+        assert done == sweep + 1 and att == nb * (sweep + 1)
+    att, acc_total, _ = sim.stats()
+    assert 0 < acc_total <= att
+    sim.destroy()
+    return total_flips
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE configs that the oracle finishes in seconds
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC])
+@pytest.mark.parametrize("density", [P.DENSITY_INCREMENTAL, P.DENSITY_FULL])
+def test_c1_diblock_melt_10_sweeps(kernel, density):
+    lockstep(workloads.c1(), 10, kernel=kernel, density=density)
+
+
+@pytest.mark.parametrize("kappaN", [0.0, 50.0])
+def test_c2_homopolymer_melt(kappaN):
+    lockstep(workloads.c2(kappaN), 4)
+
+
+def test_c1_other_hamiltonian():
+    lockstep(workloads.c1(), 3, hamiltonian=1)
+
+
+@pytest.mark.parametrize("w", workloads.small_cases(), ids=lambda w: w.name)
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC])
+def test_edge_and_ragged_cases(w, kernel):
+    lockstep(w, 4, kernel=kernel)
+
+
+def test_ragged_last_tile_of_the_fused_kernel():
+    # 2051 chains * 32 = 65,632 beads: 512 full tiles + a 96-bead tail; 7 chains of 64 -> 3.5 tiles
+    w = workloads.Workload("ragged", ((2051, workloads.diblock(32, 16)), (7, workloads.diblock(64, 19)),
+                                      (5, workloads.homopolymer(16)), (3, workloads.homopolymer(4)),
+                                      (9, workloads.homopolymer(128)), (11, workloads.homopolymer(8, 1))),
+                           32, 2, (4.0, 4.0, 4.0), (16, 16, 16), 20.0, 50.0, 0.1, 11)
+    lockstep(w, 5, kernel=P.KERNEL_FUSED)
+
+
+def test_unwrapped_coordinates_far_from_the_origin():
+    w = workloads.c1()
+    x, y, z = workloads.gaussian_walks(w)
+    xyz0 = np.stack([x - 37 * 4.0, y + 1000 * 4.0, z + 5.0e6]).astype(np.float32)   # |i_z| > 2^22: integer fold path
+    lockstep(w, 3, xyz0=xyz0)
+
+
+def test_large_step_moves_across_several_cells():
+    w = workloads.Workload("bigA", ((500, workloads.diblock(16, 8)),), 16, 2, (2.0, 2.0, 2.0), (16, 16, 16),
+                           10.0, 20.0, 1.0, 3)
+    lockstep(w, 4)
+
+
+# ---------------------------------------------------------------------------------------------
+# Smart-MC
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC])
+def test_smart_mc_blend(kernel):
+    w = workloads.Workload("smc_blend", ((1200, workloads.diblock(64, 19)), (600, workloads.homopolymer(16))), 64, 2,
+                           (4.0, 4.0, 4.0), (20, 20, 20), 35.0, 50.0, 0.1, 7, move="smc", smc_step=0.05 / 63)
+    lockstep(w, 5, kernel=kernel)
+
+
+def test_smart_mc_literal_step_of_c5():
+    w = workloads.Workload("smc_literal", ((600, workloads.diblock(64, 19)), (300, workloads.homopolymer(16))), 64, 2,
+                           (3.0, 3.0, 3.0), (15, 15, 15), 35.0, 50.0, 0.1, 7, move="smc", smc_step=0.05)
+    lockstep(w, 3)
+
+
+# ---------------------------------------------------------------------------------------------
+# full-size configs in the launch configuration bench.py times
+# ---------------------------------------------------------------------------------------------
+def test_c3_headline_full_size():
+    w = workloads.c3()
+    flips = lockstep(w, 2)
+    assert flips <= 2 * w.n_beads * 1e-5
+
+
+def test_c5_blend_full_size_smart_mc():
+    w = workloads.c5(smc_step=0.05 / 63)
+    lockstep(w, 1)
+
+
+# ---------------------------------------------------------------------------------------------
+# soma_init without positions: device-generated Gaussian walks vs the oracle's definition
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[7]], ids=lambda w: w.name)
+def test_device_generated_start_state(w):
+    sim = P.from_workload(w, xyz0=None)
+    got = sim.positions()
+    want = np.stack(oracle_system(w).init_positions())
+    # double-precision Box-Muller on both sides, one rounding to fp32: equal up to rare 1-ulp cases
+    exact = (got == want).mean()
+    assert exact > 0.9999, exact
+    assert np.max(np.abs(got - want) / np.maximum(np.abs(want), 1.0)) < 2.5e-7
+    om, cnt = sim.fields()
+    x, y, z = (got[a].copy() for a in range(3))
+    orc = oracle_system(w)
+    assert np.array_equal(cnt, orc.histogram(x, y, z))
+    sim.destroy()
+
+
+def test_set_positions_and_sweep_counter_reproduce_a_run():
+    w = workloads.c1()
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    a = P.from_workload(w, xyz0=xyz0)
+    a.step(3)
+    mid = a.positions()
+    a.step(2)
+    end = a.positions()
+    om_end, cnt_end = a.fields()
+    b = P.from_workload(w, xyz0=xyz0)
+    b.set_positions(mid)
+    b.set_option(P.OPT_SWEEP_COUNTER, 3)
+    b.set_option(P.OPT_KERNEL, P.KERNEL_GENERIC)          # different kernel, same trajectory
+    b.set_option(P.OPT_DENSITY, P.DENSITY_FULL)
+    b.step(2)
+    assert np.array_equal(b.positions(), end)
+    om_b, cnt_b = b.fields()
+    assert np.array_equal(cnt_b, cnt_end) and np.array_equal(om_b, om_end)
+    a.destroy()
+    b.destroy()
+
+
+def test_device_buffers_and_timing_hooks():
+    import torch
+    w = workloads.c1()
+    sim = P.from_workload(w, xyz0=np.stack(workloads.gaussian_walks(w)))
+    sim.set_option(P.OPT_TIMING, 1)
+    n0 = sim.launch_count()
+    sim.step(5)
+    ms, n = sim.kernel_times()
+    assert n[P.K_MOVE] == 5 and n[P.K_FIELD] == 5 and ms[P.K_MOVE] > 0
+    assert sim.launch_count() - n0 == 10
+    xyz_d = torch.empty((3, w.n_beads), dtype=torch.float32, device="cuda")
+    om_d = torch.empty((2, w.n_cells), dtype=torch.float32, device="cuda")
+    sim.positions(xyz_d)
+    sim.fields(omega=om_d)
+    sim.sync()
+    assert np.array_equal(xyz_d.cpu().numpy(), sim.positions())
+    assert np.array_equal(om_d.cpu().numpy(), sim.fields()[0])
+    sim.destroy()
