@@ -119,23 +119,25 @@ static int64_t n_cells(const oracle_system *s)
 }
 
 /* ------------------------------------------------------------------------------------------ */
-/* Pi_c of Eq. 4: the cell that contains r.  Reading R7: unwrapped           */
-/* coordinates, floor of one fp32 product, periodic fold of the integer afterwards.             */
+/* Pi_c of Eq. 4: the cell that contains r.  Reading R7: coordinates are      */
+/* stored unwrapped; per axis the position in units of the box length, t = fl32(x * fl32(1/L)),  */
+/* is folded by taking its fractional part fl32(t - floor(t)) in [0,1] (one IEEE subtraction),   */
+/* and the cell is floor(fl32(frac * n)), clamped to n-1 because frac or the product may round up. */
 /* ------------------------------------------------------------------------------------------ */
-static int32_t fold(int32_t i, int32_t n)
+static int32_t axis_cell(float x, float L, int32_t n)
 {
-    const int32_t r = i % n;
-    return r < 0 ? r + n : r;
+    const float inv_L = (float)(1.0 / (double)L);
+    const float t = x * inv_L;
+    const float frac = t - floorf(t);
+    const int32_t i = (int32_t)floorf(frac * (float)n);
+    return i < n - 1 ? i : n - 1;
 }
 
 int64_t soma_oracle_cell_index(const oracle_system *s, float x, float y, float z)
 {
-    const float inv_dx = (float)((double)s->grid[0] / (double)s->box[0]);
-    const float inv_dy = (float)((double)s->grid[1] / (double)s->box[1]);
-    const float inv_dz = (float)((double)s->grid[2] / (double)s->box[2]);
-    const int32_t ix = fold((int32_t)floorf(x * inv_dx), s->grid[0]);
-    const int32_t iy = fold((int32_t)floorf(y * inv_dy), s->grid[1]);
-    const int32_t iz = fold((int32_t)floorf(z * inv_dz), s->grid[2]);
+    const int32_t ix = axis_cell(x, s->box[0], s->grid[0]);
+    const int32_t iy = axis_cell(y, s->box[1], s->grid[1]);
+    const int32_t iz = axis_cell(z, s->box[2], s->grid[2]);
     return ((int64_t)ix * s->grid[1] + iy) * s->grid[2] + iz; /* R8: [ix][iy][iz], z fastest */
 }
 

@@ -118,23 +118,29 @@ __device__ __forceinline__ int wrap1(int c, int n)
     return c < 0 ? c + n : c;
 }
 
-// Old and trial cell of one move.  The trial cell is reached from the old one by the (small)
-// difference of the unfolded indices; soma_init guarantees A <= min(box)/2 so that one wrap is
-// enough.  Returns whether the cell changed.
+// Old and trial cell of one move; returns whether the cell changed.
+// kBounded (local moves): |d| < A <= min(box)/2 (checked by soma_init), so the trial cell is reached
+// from the old one by the small difference of the unfolded indices and one wrap is enough.
+// Otherwise (Smart-MC: Gaussian proposals are unbounded) the trial position is folded from scratch.
+template <bool kBounded>
 __device__ __forceinline__ bool cells_of_move(const GridP& g, float x, float y, float z, float x2,
                                               float y2, float z2, uint32_t& c_old, uint32_t& c_new)
 {
     const float fx = floorf(x * g.inv_d[0]), fy = floorf(y * g.inv_d[1]), fz = floorf(z * g.inv_d[2]);
-    const int dx = (int)(floorf(x2 * g.inv_d[0]) - fx);
-    const int dy = (int)(floorf(y2 * g.inv_d[1]) - fy);
-    const int dz = (int)(floorf(z2 * g.inv_d[2]) - fz);
     const int cx = fold_axis(fx, g.nf[0], g.inv_nf[0], g.n[0]);
     const int cy = fold_axis(fy, g.nf[1], g.inv_nf[1], g.n[1]);
     const int cz = fold_axis(fz, g.nf[2], g.inv_nf[2], g.n[2]);
     c_old = (uint32_t)((cx * g.n[1] + cy) * g.n[2] + cz);
-    const int cx2 = wrap1(cx + dx, g.n[0]), cy2 = wrap1(cy + dy, g.n[1]), cz2 = wrap1(cz + dz, g.n[2]);
-    c_new = (uint32_t)((cx2 * g.n[1] + cy2) * g.n[2] + cz2);
-    return (dx | dy | dz) != 0;
+    if (kBounded) {
+        const int dx = (int)(floorf(x2 * g.inv_d[0]) - fx);
+        const int dy = (int)(floorf(y2 * g.inv_d[1]) - fy);
+        const int dz = (int)(floorf(z2 * g.inv_d[2]) - fz);
+        const int cx2 = wrap1(cx + dx, g.n[0]), cy2 = wrap1(cy + dy, g.n[1]), cz2 = wrap1(cz + dz, g.n[2]);
+        c_new = (uint32_t)((cx2 * g.n[1] + cy2) * g.n[2] + cz2);
+        return (dx | dy | dz) != 0;
+    }
+    c_new = cell_of(g, x2, y2, z2);
+    return c_new != c_old;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -206,7 +212,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 
     // non-bonded: dE_nb = omega_k(c') - omega_k(c), Eq. 15; 0 when the cell is kept
     uint32_t c_old, c_new;
-    const bool moved = cells_of_move(P.g, x, y, z, x2, y2, z2, c_old, c_new);
+    const bool moved = cells_of_move<kMove == 1>(P.g, x, y, z, x2, y2, z2, c_old, c_new);
     float e_nb = 0.0f;
     if (moved) e_nb = __ldg(omega + toff + c_new) - __ldg(omega + toff + c_old);
 

@@ -77,7 +77,10 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
                     seg = (~agree[g:g + n * N]).reshape(n, N).any(1)
                     bad[g:g + n * N] = np.repeat(seg, N)
                     g += n * N
-            assert np.max(np.abs(pos[:, ~bad] - ref[:, ~bad])) <= POS_TOL_SMC
+            # the proposal goes through logf/sincosf (not bit-reproducible across CPU and GPU), so r + d may
+            # round to the neighbouring float: 1e-6 R_e plus one ulp of the stored coordinate (R17)
+            tol = POS_TOL_SMC + np.spacing(np.abs(ref[:, ~bad]))
+            assert np.all(np.abs(pos[:, ~bad] - ref[:, ~bad]) <= tol)
         att, acc_g, done = sim.stats()
         assert done == sweep + 1 and att == nb * (sweep + 1)
     att, acc_total, _ = sim.stats()
