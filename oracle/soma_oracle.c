@@ -121,15 +121,16 @@ static int64_t n_cells(const oracle_system *s)
 /* ------------------------------------------------------------------------------------------ */
 /* Pi_c of Eq. 4: the cell that contains r.  Reading R7: coordinates are      */
 /* stored unwrapped; per axis the position in units of the box length, t = fl32(x * fl32(1/L)),  */
-/* is folded by taking its fractional part fl32(t - floor(t)) in [0,1] (one IEEE subtraction),   */
-/* and the cell is floor(fl32(frac * n)), clamped to n-1 because frac or the product may round up. */
+/* is folded by taking its fractional part frac = fl32(t - floor(t)) in [0,1] (one IEEE           */
+/* subtraction), and the cell is floor(frac * n) with the product taken exactly (24 x 24 bits fit */
+/* a double), clamped to n-1 because frac may round up to 1.                                      */
 /* ------------------------------------------------------------------------------------------ */
 static int32_t axis_cell(float x, float L, int32_t n)
 {
     const float inv_L = (float)(1.0 / (double)L);
     const float t = x * inv_L;
     const float frac = t - floorf(t);
-    const int32_t i = (int32_t)floorf(frac * (float)n);
+    const int32_t i = (int32_t)floor((double)frac * (double)n);
     return i < n - 1 ? i : n - 1;
 }
 

@@ -80,6 +80,7 @@ struct soma_ctx {
 
     // options
     int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0, use_graph = 1;
+    int blocks_per_sm = 6;   // grid of the fused kernel = n_sm * blocks_per_sm (grid-stride over tiles)
     float smc_step = 0.0f;
 
     uint64_t sweep = 0, attempted = 0, launches = 0;
@@ -101,10 +102,10 @@ soma::GridP soma_ctx::gridp() const
 {
     soma::GridP g;
     for (int a = 0; a < 3; ++a) {
-        g.inv_d[a] = (float)((double)grid[a] / (double)box[a]);
+        g.inv_L[a] = (float)(1.0 / (double)box[a]);
         g.nf[a] = (float)grid[a];
-        g.inv_nf[a] = (float)(1.0 / (double)grid[a]);
-        g.n[a] = grid[a];
+        g.n[a] = (uint32_t)grid[a];
+        g.nm1[a] = (uint32_t)grid[a] - 1u;
     }
     g.cells = (uint32_t)cells;
     return g;
@@ -121,8 +122,10 @@ soma::MoveP soma_ctx::movep(uint64_t sweep_no) const
     p.a_s = smc_step;
     p.noise = sqrtf(2.0f * smc_step);
     p.four_as = 4.0f * smc_step;
-    p.key0 = (uint32_t)seed;
-    p.key1 = (uint32_t)(seed >> 32);
+    for (uint32_t r = 0; r < 10; ++r) {
+        p.rk[r][0] = (uint32_t)seed + r * 0x9E3779B9u;
+        p.rk[r][1] = (uint32_t)(seed >> 32) + r * 0xBB67AE85u;
+    }
     p.sweep_lo = (uint32_t)sweep_no;
     p.sweep_hi = (uint32_t)(sweep_no >> 32);
     return p;
@@ -200,27 +203,31 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         if (s.n_beads == 0) continue;
         float *x = c->x + s.off, *y = c->y + s.off, *z = c->z + s.off;
         const uint32_t* toff = c->toff + s.toff_off;
-        if (spec_uses_fused(c, s)) {
-            const uint32_t n_tiles = (uint32_t)((s.n_beads + soma::kTile - 1) / soma::kTile);
+        uint64_t done = 0;   // beads of this architecture handled by the fused kernel
+        if (spec_uses_fused(c, s) && s.n_beads >= soma::kTile) {
+            const uint32_t n_tiles = (uint32_t)(s.n_beads / soma::kTile);
             const int threads = 256, warps_per_block = threads / 32;
-            int max_blocks = c->n_sm * 8;
+            int max_blocks = c->n_sm * c->blocks_per_sm;
             int blocks = (int)((n_tiles + warps_per_block - 1) / warps_per_block);
             if (blocks > max_blocks) blocks = max_blocks;
             Timed t(c, SOMA_K_MOVE, 1);
             soma::fused_sweep_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
-                P, x, y, z, c->omega, c->counts, toff, s.N - 1u, n_tiles, (uint32_t)s.n_beads,
-                (uint32_t)s.gid0, reinterpret_cast<uint8_t*>(c->decisions) + s.gid0 / 8, c->acc_slots);
-        } else {
+                P, x, y, z, c->omega, c->counts, toff, s.N - 1u, n_tiles, (uint32_t)s.gid0,
+                reinterpret_cast<uint8_t*>(c->decisions) + s.gid0 / 8, c->acc_slots);
+            done = (uint64_t)n_tiles * soma::kTile;
+        }
+        if (done < s.n_beads) {   // whole chains the fused kernel does not cover (all of them, or a ragged tail)
+            const uint64_t n_chains = (s.n_beads - done) / s.N;
             for (uint32_t parity = 0; parity < 2; ++parity) {
                 const uint32_t half = parity == 0 ? (s.N + 1) / 2 : s.N / 2;
                 if (half == 0) continue;
-                const uint64_t n_items = s.n_chains * half;
+                const uint64_t n_items = n_chains * half;
                 const int threads = 256;
                 const uint64_t blocks = (n_items + threads - 1) / threads;
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::generic_move_kernel<kMove, kIncr, kRecord><<<(unsigned)blocks, threads, 0, c->stream>>>(
-                    P, x, y, z, c->omega, c->counts, toff, s.N, half, parity, n_items, (uint32_t)s.gid0,
-                    c->decisions, c->acc_slots);
+                    P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity, n_items,
+                    (uint32_t)(s.gid0 + done), c->decisions, c->acc_slots);
             }
         }
         CU(cudaGetLastError());
@@ -341,7 +348,7 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
     uint64_t cells = 1;
     for (int a = 0; a < 3; ++a) {
         if (!(box[a] > 0.0f) || !std::isfinite(box[a])) return fail(SOMA_EINVAL, "soma_init: box[%d] must be > 0", a);
-        if (grid[a] < 1) return fail(SOMA_EINVAL, "soma_init: grid[%d] must be >= 1", a);
+        if (grid[a] < 1 || grid[a] > (1 << 22)) return fail(SOMA_EINVAL, "soma_init: grid[%d] must be in 1..2^22", a);
         min_box = box[a] < min_box ? box[a] : min_box;
         cells *= (uint64_t)grid[a];
         if (cells >= (1ull << 31)) return fail(SOMA_EINVAL, "soma_init: too many grid cells (>= 2^31)");
@@ -589,6 +596,10 @@ int soma_set_option(soma_ctx* c, int key, double value)
             return SOMA_OK;
         case SOMA_OPT_GRAPH:
             c->use_graph = iv != 0;
+            return SOMA_OK;
+        case SOMA_OPT_BLOCKS_PER_SM:
+            if (iv < 1 || iv > 32) return fail(SOMA_EINVAL, "SOMA_OPT_BLOCKS_PER_SM: 1..32");
+            c->blocks_per_sm = iv;
             return SOMA_OK;
         default:
             return fail(SOMA_EINVAL, "soma_set_option: unknown key %d", key);

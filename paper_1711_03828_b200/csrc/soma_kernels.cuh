@@ -22,11 +22,15 @@ constexpr int kMaxTypes = 8;
 constexpr int kTile = 128;          // beads per warp tile in the fused kernel (4 per lane)
 constexpr int kAccSlots = 256;      // spread slots of the accepted-moves counter
 
+#ifndef SOMA_FUSED_MIN_BLOCKS
+#define SOMA_FUSED_MIN_BLOCKS 3      // resident 256-thread blocks per SM the fused kernel is compiled for
+#endif
+
 struct GridP {
-    float inv_d[3];   // cells per unit length, fl32(n_a / L_a)
+    float inv_L[3];   // fl32(1 / L_a)
     float nf[3];      // (float) n_a
-    float inv_nf[3];  // fl32(1 / n_a)
-    int n[3];
+    uint32_t n[3];
+    uint32_t nm1[3];  // n_a - 1
     uint32_t cells;
 };
 
@@ -38,7 +42,7 @@ struct MoveP {
     float a_s;        // Smart-MC step
     float noise;      // sqrt(2 a_s)
     float four_as;    // 4 a_s
-    uint32_t key0, key1;          // Philox key = seed
+    uint32_t rk[10][2];           // Philox round keys: seed + r * (0x9E3779B9, 0xBB67AE85)
     uint32_t sweep_lo, sweep_hi;  // Philox counter words 1, 2
 };
 
@@ -76,6 +80,25 @@ __device__ __forceinline__ void philox4x32_10(uint32_t a, uint32_t b, uint32_t c
     out[0] = a; out[1] = b; out[2] = c; out[3] = d;
 }
 
+// Same generator with the key schedule precomputed on the host (MoveP::rk lives in the kernel's
+// constant bank, so the round keys cost no instruction).
+__device__ __forceinline__ void philox4x32_10_rk(uint32_t a, uint32_t b, uint32_t c, uint32_t d,
+                                                 const uint32_t (&rk)[10][2], uint32_t (&out)[4])
+{
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const unsigned long long pa = (unsigned long long)a * 0xD2511F53ull;
+        const unsigned long long pc = (unsigned long long)c * 0xCD9E8D57ull;
+        const uint32_t na = (uint32_t)(pc >> 32) ^ b ^ rk[r][0];
+        const uint32_t nc = (uint32_t)(pa >> 32) ^ d ^ rk[r][1];
+        b = (uint32_t)pc;
+        d = (uint32_t)pa;
+        a = na;
+        c = nc;
+    }
+    out[0] = a; out[1] = b; out[2] = c; out[3] = d;
+}
+
 // top 23 bits -> float in [1, 2), exact
 __device__ __forceinline__ float u23(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
 
@@ -87,60 +110,32 @@ __device__ __forceinline__ float ex2_approx(float x)
 }
 
 // ------------------------------------------------------------------------------------------------
-// Cell bookkeeping.  i_a = floor(fl32(x_a * inv_d_a)) is kept as a float (exact integer);
-// the periodic fold uses a float quotient with one correction step each way, exact for
-// |i_a| < 2^22, and integer arithmetic beyond.
+// Pi_c of Eq. 4: the cell that contains r, periodic.  Per axis: position in
+// units of the box length t = x * (1/L), folded by its fractional part frac = t - floor(t), cell =
+// floor(frac * n) (exact product) clamped to n-1.
+// FRND and F2I run on the XU pipe (16 lanes/clk/SM, shared with MUFU) and saturated it in the first
+// version of this kernel, so floor and float->int are done on the FMA/ALU pipes instead:
+//   floor(t)       = fl_down(t + 1.5 * 2^23) - 1.5 * 2^23     exact for |t| < 2^22
+//   floor(frac n)  = mantissa of fl_down(frac * n + 2^23)      exact for frac * n < 2^23
+// FMUL, FADD.RM, FADD, FADD, FFMA.RM, IADD, VIMNMX.U32 per axis.  The unsigned min keeps the index
+// in range for every input (also NaN and |t| >= 2^22, which is outside the supported domain:
+// |x_a| < 2^22 L_a, R7).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ int fold_axis(float f, float nf, float inv_nf, int n)
+__device__ __forceinline__ uint32_t axis_cell(float x, float inv_L, float nf, uint32_t n_minus_1)
 {
-    if (fabsf(f) >= 4194304.0f) {
-        const int m = (int)f % n;
-        return m < 0 ? m + n : m;
-    }
-    const float q = floorf(f * inv_nf);
-    float r = fmaf(-q, nf, f);
-    r = r < 0.0f ? r + nf : r;
-    r = r >= nf ? r - nf : r;
-    return (int)r;
+    const float t = x * inv_L;
+    const float fl = __fadd_rd(t, 12582912.0f) - 12582912.0f;
+    const float frac = t - fl;
+    const float s = __fmaf_rd(frac, nf, 8388608.0f);
+    return min(__float_as_uint(s) - 0x4B000000u, n_minus_1);
 }
 
 __device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, float z)
 {
-    const int cx = fold_axis(floorf(x * g.inv_d[0]), g.nf[0], g.inv_nf[0], g.n[0]);
-    const int cy = fold_axis(floorf(y * g.inv_d[1]), g.nf[1], g.inv_nf[1], g.n[1]);
-    const int cz = fold_axis(floorf(z * g.inv_d[2]), g.nf[2], g.inv_nf[2], g.n[2]);
-    return (uint32_t)((cx * g.n[1] + cy) * g.n[2] + cz);
-}
-
-__device__ __forceinline__ int wrap1(int c, int n)
-{
-    c = c >= n ? c - n : c;
-    return c < 0 ? c + n : c;
-}
-
-// Old and trial cell of one move; returns whether the cell changed.
-// kBounded (local moves): |d| < A <= min(box)/2 (checked by soma_init), so the trial cell is reached
-// from the old one by the small difference of the unfolded indices and one wrap is enough.
-// Otherwise (Smart-MC: Gaussian proposals are unbounded) the trial position is folded from scratch.
-template <bool kBounded>
-__device__ __forceinline__ bool cells_of_move(const GridP& g, float x, float y, float z, float x2,
-                                              float y2, float z2, uint32_t& c_old, uint32_t& c_new)
-{
-    const float fx = floorf(x * g.inv_d[0]), fy = floorf(y * g.inv_d[1]), fz = floorf(z * g.inv_d[2]);
-    const int cx = fold_axis(fx, g.nf[0], g.inv_nf[0], g.n[0]);
-    const int cy = fold_axis(fy, g.nf[1], g.inv_nf[1], g.n[1]);
-    const int cz = fold_axis(fz, g.nf[2], g.inv_nf[2], g.n[2]);
-    c_old = (uint32_t)((cx * g.n[1] + cy) * g.n[2] + cz);
-    if (kBounded) {
-        const int dx = (int)(floorf(x2 * g.inv_d[0]) - fx);
-        const int dy = (int)(floorf(y2 * g.inv_d[1]) - fy);
-        const int dz = (int)(floorf(z2 * g.inv_d[2]) - fz);
-        const int cx2 = wrap1(cx + dx, g.n[0]), cy2 = wrap1(cy + dy, g.n[1]), cz2 = wrap1(cz + dz, g.n[2]);
-        c_new = (uint32_t)((cx2 * g.n[1] + cy2) * g.n[2] + cz2);
-        return (dx | dy | dz) != 0;
-    }
-    c_new = cell_of(g, x2, y2, z2);
-    return c_new != c_old;
+    const uint32_t cx = axis_cell(x, g.inv_L[0], g.nf[0], g.nm1[0]);
+    const uint32_t cy = axis_cell(y, g.inv_L[1], g.nf[1], g.nm1[1]);
+    const uint32_t cz = axis_cell(z, g.inv_L[2], g.nf[2], g.nm1[2]);
+    return (cx * g.n[1] + cy) * g.n[2] + cz;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -153,7 +148,8 @@ __device__ __forceinline__ bool cells_of_move(const GridP& g, float x, float y, 
 // kMove 1: local displacement uniform in (-A,A)^3 + Metropolis.
 // kMove 2: Smart-MC, force-biased proposal from the bonded force + Metropolis-Hastings.
 // kIncr: the occupation numbers follow the accepted move (+1 new cell, -1 old cell) -- integer
-// arithmetic, so they stay identical to a fresh histogram (a3).
+// arithmetic, so they stay identical to a fresh histogram (a3).  No branch on the hot path: the
+// gathers and the count updates are predicated, so the two moves of a set interleave (ILP 2).
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr>
 __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
@@ -169,15 +165,15 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
     float dx, dy, dz, u, log_ratio = 0.0f;
     if (kMove == 1) {
         uint32_t w[4];
-        philox4x32_10(gid, P.sweep_lo, P.sweep_hi, 0x100u, P.key0, P.key1, w);
+        philox4x32_10_rk(gid, P.sweep_lo, P.sweep_hi, 0x100u, P.rk, w);
         dx = fmaf(u23(w[0]), P.c1, P.c0);
         dy = fmaf(u23(w[1]), P.c1, P.c0);
         dz = fmaf(u23(w[2]), P.c1, P.c0);
         u = u23(w[3]) - 1.0f;
     } else {
         uint32_t w[4], v[4];
-        philox4x32_10(gid, P.sweep_lo, P.sweep_hi, 0x200u, P.key0, P.key1, w);
-        philox4x32_10(gid, P.sweep_lo, P.sweep_hi, 0x201u, P.key0, P.key1, v);
+        philox4x32_10_rk(gid, P.sweep_lo, P.sweep_hi, 0x200u, P.rk, w);
+        philox4x32_10_rk(gid, P.sweep_lo, P.sweep_hi, 0x201u, P.rk, v);
         const float ra = sqrtf(-2.0f * logf(2.0f - u23(w[0])));
         const float rb = sqrtf(-2.0f * logf(2.0f - u23(w[2])));
         const float two_pi = 6.283185307179586f;
@@ -211,10 +207,15 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
     const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
 
     // non-bonded: dE_nb = omega_k(c') - omega_k(c), Eq. 15; 0 when the cell is kept
-    uint32_t c_old, c_new;
-    const bool moved = cells_of_move<kMove == 1>(P.g, x, y, z, x2, y2, z2, c_old, c_new);
-    float e_nb = 0.0f;
-    if (moved) e_nb = __ldg(omega + toff + c_new) - __ldg(omega + toff + c_old);
+    const uint32_t i_old = toff + cell_of(P.g, x, y, z);
+    const uint32_t i_new = toff + cell_of(P.g, x2, y2, z2);
+    const bool moved = i_new != i_old;
+    float w_new = 0.0f, w_old = 0.0f;
+    if (moved) {
+        w_new = __ldg(omega + i_new);
+        w_old = __ldg(omega + i_old);
+    }
+    const float e_nb = w_new - w_old;
 
     // bonded: dE_b = k_0/2 (2 d.s + m |d|^2), Eq. 2
     const float ds = fmaf(dz, sz, fmaf(dy, sy, dx * sx));
@@ -226,32 +227,32 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 
     // Metropolis: accept iff dE <= 0 or u < exp(-dE)
     const bool acc = (dE <= 0.0f) || (u < ex2_approx(dE * -1.4426950408889634f));
-    if (acc) {
-        x = x2; y = y2; z = z2;
-        if (kIncr && moved) {
-            atomicAdd(counts + toff + c_new, 1u);
-            atomicAdd(counts + toff + c_old, 0xFFFFFFFFu);
-        }
+    x = acc ? x2 : x;
+    y = acc ? y2 : y;
+    z = acc ? z2 : z;
+    if (kIncr && acc && moved) {
+        atomicAdd(counts + i_new, 1u);
+        atomicAdd(counts + i_old, 0xFFFFFFFFu);
     }
     return acc;
 }
 
 // ------------------------------------------------------------------------------------------------
 // a1 + a2 fused, chain-resident.  Requires N in {4, 8, ..., 128} (N | 128) so that a 128-bead warp
-// tile holds whole chains; the architecture's bead array starts 512-byte aligned.
+// tile holds whole chains; the architecture's bead array starts 512-byte aligned.  Only full tiles
+// are processed here; the host sends a ragged tail (< 128 beads, whole chains) to the generic kernel.
 //   x,y,z       base of this architecture's beads (padded layout)
 //   toff_tab    [N] type * cells of every monomer of the chain
-//   n_tiles     tiles of this architecture (n_chains * N / 128, last one may be partial)
-//   n_beads     beads of this architecture (for the ragged last tile)
+//   n_tiles     full tiles of this architecture (n_chains * N / 128)
 //   gid0        global index of the architecture's first bead
 //   dec_bytes   decision bitmap of the architecture (byte view), or unused
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord>
-__global__ void __launch_bounds__(256)
+__global__ void __launch_bounds__(256, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
                    const uint32_t* __restrict__ toff_tab, uint32_t n_mask, uint32_t n_tiles,
-                   uint32_t n_beads, uint32_t gid0, uint8_t* __restrict__ dec_bytes,
+                   uint32_t gid0, uint8_t* __restrict__ dec_bytes,
                    unsigned long long* __restrict__ acc_slots)
 {
     const uint32_t lane = threadIdx.x & 31u;
@@ -266,40 +267,34 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
     for (uint32_t tile = warp; tile < n_tiles; tile += n_warps) {
         const uint32_t i0 = tile * kTile + 4u * lane;
-        const bool live = i0 < n_beads;                       // n_beads is a multiple of N >= 4
-        float4 X = make_float4(0.f, 0.f, 0.f, 0.f), Y = X, Z = X;
-        if (live) {
-            X = *reinterpret_cast<const float4*>(x + i0);
-            Y = *reinterpret_cast<const float4*>(y + i0);
-            Z = *reinterpret_cast<const float4*>(z + i0);
-        }
+        float4 X = *reinterpret_cast<const float4*>(x + i0);
+        float4 Y = *reinterpret_cast<const float4*>(y + i0);
+        float4 Z = *reinterpret_cast<const float4*>(z + i0);
         const uint32_t gid = gid0 + i0;
 
         // ---- set 0: even monomers (slots 0, 2) see the old odd monomers --------------------
         float xl = __shfl_up_sync(0xFFFFFFFFu, X.w, 1), yl = __shfl_up_sync(0xFFFFFFFFu, Y.w, 1),
               zl = __shfl_up_sync(0xFFFFFFFFu, Z.w, 1);
-        if (!has_l0) { xl = X.x; yl = Y.x; zl = Z.x; }
-        bool a0 = false, a1 = false, a2 = false, a3 = false;
-        if (live) {
-            a0 = mc_move<kMove, kIncr>(P, omega, counts, X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, mf0, toff.x, gid);
-            a2 = mc_move<kMove, kIncr>(P, omega, counts, X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, 2.0f, toff.z, gid + 2u);
-        }
+        xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+        const bool a0 = mc_move<kMove, kIncr>(P, omega, counts, X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, mf0, toff.x, gid);
+        const bool a2 = mc_move<kMove, kIncr>(P, omega, counts, X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, 2.0f, toff.z, gid + 2u);
+
         // ---- set 1: odd monomers (slots 1, 3) see the moved even monomers ------------------
         float xr = __shfl_down_sync(0xFFFFFFFFu, X.x, 1), yr = __shfl_down_sync(0xFFFFFFFFu, Y.x, 1),
               zr = __shfl_down_sync(0xFFFFFFFFu, Z.x, 1);
-        if (!has_r3) { xr = X.w; yr = Y.w; zr = Z.w; }
-        if (live) {
-            a1 = mc_move<kMove, kIncr>(P, omega, counts, X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, 2.0f, toff.y, gid + 1u);
-            a3 = mc_move<kMove, kIncr>(P, omega, counts, X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, mf3, toff.w, gid + 3u);
-            *reinterpret_cast<float4*>(x + i0) = X;
-            *reinterpret_cast<float4*>(y + i0) = Y;
-            *reinterpret_cast<float4*>(z + i0) = Z;
-        }
+        xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+        const bool a1 = mc_move<kMove, kIncr>(P, omega, counts, X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, 2.0f, toff.y, gid + 1u);
+        const bool a3 = mc_move<kMove, kIncr>(P, omega, counts, X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, mf3, toff.w, gid + 3u);
+
+        *reinterpret_cast<float4*>(x + i0) = X;
+        *reinterpret_cast<float4*>(y + i0) = Y;
+        *reinterpret_cast<float4*>(z + i0) = Z;
+
         const uint32_t nib = (a0 ? 1u : 0u) | (a1 ? 2u : 0u) | (a2 ? 4u : 0u) | (a3 ? 8u : 0u);
         n_acc += __popc(nib);
         if (kRecord) {
             const uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, nib, 1);
-            if (live && (lane & 1u) == 0u) dec_bytes[i0 >> 3] = (uint8_t)(nib | (hi << 4));
+            if ((lane & 1u) == 0u) dec_bytes[i0 >> 3] = (uint8_t)(nib | (hi << 4));
         }
     }
     n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
