@@ -60,7 +60,7 @@ enum {
     SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */
     SOMA_OPT_SWEEP_COUNTER = 8,    /* set the sweep counter (the "time step" word of the Philox counter)      */
     SOMA_OPT_GRAPH = 9,            /* 1: replay soma_step's launches from a CUDA graph (default 1)            */
-    SOMA_OPT_BLOCKS_PER_SM = 10    /* tuning: grid of the fused kernel = SMs x this many 256-thread blocks    */
+    SOMA_OPT_BLOCKS_PER_SM = 10    /* tuning: grid of the fused kernel = SMs x this many blocks; 0 = resident max */
 };
 
 /* indices of soma_kernel_times */

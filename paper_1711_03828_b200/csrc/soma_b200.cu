@@ -80,7 +80,7 @@ struct soma_ctx {
 
     // options
     int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0, use_graph = 1;
-    int blocks_per_sm = 6;   // grid of the fused kernel = n_sm * blocks_per_sm (grid-stride over tiles)
+    int blocks_per_sm = 0;   // grid of the fused kernel = n_sm * blocks_per_sm; 0 = as many as are resident
     float smc_step = 0.0f;
 
     uint64_t sweep = 0, attempted = 0, launches = 0;
@@ -192,7 +192,6 @@ bool spec_uses_fused(const soma_ctx* c, const Spec& s)
 {
     if (c->kernel_choice == 1) return false;
     if (!s.fused_ok) return false;
-    if (c->record && (s.gid0 % 8) != 0) return false;  // byte view of the decision bitmap needs it
     return true;
 }
 
@@ -206,14 +205,20 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
         if (spec_uses_fused(c, s) && s.n_beads >= soma::kTile) {
             const uint32_t n_tiles = (uint32_t)(s.n_beads / soma::kTile);
-            const int threads = 256, warps_per_block = threads / 32;
-            int max_blocks = c->n_sm * c->blocks_per_sm;
-            int blocks = (int)((n_tiles + warps_per_block - 1) / warps_per_block);
-            if (blocks > max_blocks) blocks = max_blocks;
+            constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
+            int per_sm = c->blocks_per_sm;
+            if (per_sm <= 0) {   // auto: every block resident, one wave
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
+                    &per_sm, soma::fused_sweep_kernel<kMove, kIncr, kRecord>, threads, 0));
+                if (per_sm < 1) per_sm = 1;
+            }
+            int blocks = c->n_sm * per_sm;
+            const int max_useful = (int)((n_tiles + warps_per_block - 1) / warps_per_block);
+            if (blocks > max_useful) blocks = max_useful;
             Timed t(c, SOMA_K_MOVE, 1);
             soma::fused_sweep_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
                 P, x, y, z, c->omega, c->counts, toff, s.N - 1u, n_tiles, (uint32_t)s.gid0,
-                reinterpret_cast<uint8_t*>(c->decisions) + s.gid0 / 8, c->acc_slots);
+                c->decisions, c->acc_slots);
             done = (uint64_t)n_tiles * soma::kTile;
         }
         if (done < s.n_beads) {   // whole chains the fused kernel does not cover (all of them, or a ragged tail)
@@ -598,7 +603,7 @@ int soma_set_option(soma_ctx* c, int key, double value)
             c->use_graph = iv != 0;
             return SOMA_OK;
         case SOMA_OPT_BLOCKS_PER_SM:
-            if (iv < 1 || iv > 32) return fail(SOMA_EINVAL, "SOMA_OPT_BLOCKS_PER_SM: 1..32");
+            if (iv < 0 || iv > 32) return fail(SOMA_EINVAL, "SOMA_OPT_BLOCKS_PER_SM: 0 (auto) .. 32");
             c->blocks_per_sm = iv;
             return SOMA_OK;
         default:

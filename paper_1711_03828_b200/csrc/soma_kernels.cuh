@@ -21,9 +21,13 @@ namespace soma {
 constexpr int kMaxTypes = 8;
 constexpr int kTile = 128;          // beads per warp tile in the fused kernel (4 per lane)
 constexpr int kAccSlots = 256;      // spread slots of the accepted-moves counter
+#ifndef SOMA_FUSED_THREADS
+#define SOMA_FUSED_THREADS 128       // threads per block of the fused kernel
+#endif
+constexpr int kFusedThreads = SOMA_FUSED_THREADS;
 
 #ifndef SOMA_FUSED_MIN_BLOCKS
-#define SOMA_FUSED_MIN_BLOCKS 3      // resident 256-thread blocks per SM the fused kernel is compiled for
+#define SOMA_FUSED_MIN_BLOCKS 5      // resident blocks per SM the fused kernel is compiled for (register cap)
 #endif
 
 struct GridP {
@@ -139,37 +143,29 @@ __device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, fl
 }
 
 // ------------------------------------------------------------------------------------------------
-// One Monte-Carlo move of one bead ("MC scheme for particle ip", Code 2).
-//   (x,y,z)        the bead, updated in place when the move is accepted
-//   (xl..),(xr..)  chain neighbours; an absent neighbour is passed as the bead itself (bond 0)
-//   mf             number of bonded neighbours as float
-//   toff           type * cells, offset of this bead type's plane in omega / counts
-//   gid            global bead index = Philox counter word 0
-// kMove 1: local displacement uniform in (-A,A)^3 + Metropolis.
-// kMove 2: Smart-MC, force-biased proposal from the bonded force + Metropolis-Hastings.
-// kIncr: the occupation numbers follow the accepted move (+1 new cell, -1 old cell) -- integer
-// arithmetic, so they stay identical to a fresh histogram (a3).  No branch on the hot path: the
-// gathers and the count updates are predicated, so the two moves of a set interleave (ILP 2).
+// Pieces of one Monte-Carlo move of one bead ("MC scheme for particle ip", Code 2).
+// They are separate functions so that the fused kernel can run them phase by phase over the four
+// beads a lane owns (all random numbers, then all cell indices, then all field gathers in flight at
+// once, then the decisions), while the generic kernel strings them together for one bead.
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr>
-__device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
-                                        uint32_t* __restrict__ counts, float& x, float& y, float& z,
-                                        float xl, float yl, float zl, float xr, float yr, float zr,
-                                        float mf, uint32_t toff, uint32_t gid)
-{
-    // s = sum over neighbours of (r - r_nb)
-    const float sx = (x - xl) + (x - xr);
-    const float sy = (y - yl) + (y - yr);
-    const float sz = (z - zl) + (z - zr);
+struct Draw {            // what one move takes from Philox
+    float a, b, c;       // local move: trial displacement d;  Smart-MC: the Gaussians g
+    float u;             // acceptance uniform in [0, 1)
+};
 
-    float dx, dy, dz, u, log_ratio = 0.0f;
+// kMove 1: d uniform in (-A,A)^3, 2^23 equidistant values per axis.
+// kMove 2: g ~ N(0,1)^3 by Box-Muller on the words of call sub=0, u from call sub=1.
+template <int kMove>
+__device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
+{
+    Draw r;
     if (kMove == 1) {
         uint32_t w[4];
         philox4x32_10_rk(gid, P.sweep_lo, P.sweep_hi, 0x100u, P.rk, w);
-        dx = fmaf(u23(w[0]), P.c1, P.c0);
-        dy = fmaf(u23(w[1]), P.c1, P.c0);
-        dz = fmaf(u23(w[2]), P.c1, P.c0);
-        u = u23(w[3]) - 1.0f;
+        r.a = fmaf(u23(w[0]), P.c1, P.c0);
+        r.b = fmaf(u23(w[1]), P.c1, P.c0);
+        r.c = fmaf(u23(w[2]), P.c1, P.c0);
+        r.u = u23(w[3]) - 1.0f;
     } else {
         uint32_t w[4], v[4];
         philox4x32_10_rk(gid, P.sweep_lo, P.sweep_hi, 0x200u, P.rk, w);
@@ -180,111 +176,261 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
         float sa, ca, sb, cb;
         sincosf(two_pi * (u23(w[1]) - 1.0f), &sa, &ca);
         sincosf(two_pi * (u23(w[3]) - 1.0f), &sb, &cb);
-        const float gx = ra * ca, gy = ra * sa, gz = rb * cb;
-        u = u23(v[0]) - 1.0f;
-        const float Fx = -P.k0 * sx, Fy = -P.k0 * sy, Fz = -P.k0 * sz;   // bonded force
-        dx = fmaf(P.a_s, Fx, P.noise * gx);
-        dy = fmaf(P.a_s, Fy, P.noise * gy);
-        dz = fmaf(P.a_s, Fz, P.noise * gz);
-        // ln T(r->r') - ln T(r'->r) = ( |d + a_s F'|^2 - |d - a_s F|^2 ) / (4 a_s),  F' = F - k_0 m d
-        const float km = P.k0 * mf;
-        float fwd = 0.0f, rev = 0.0f;
-        {
-            const float ef = dx - P.a_s * Fx, er = dx + P.a_s * (Fx - km * dx);
-            fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-        }
-        {
-            const float ef = dy - P.a_s * Fy, er = dy + P.a_s * (Fy - km * dy);
-            fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-        }
-        {
-            const float ef = dz - P.a_s * Fz, er = dz + P.a_s * (Fz - km * dz);
-            fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-        }
-        log_ratio = (rev - fwd) / P.four_as;
+        r.a = ra * ca; r.b = ra * sa; r.c = rb * cb;
+        r.u = u23(v[0]) - 1.0f;
     }
+    return r;
+}
 
-    const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
-
-    // non-bonded: dE_nb = omega_k(c') - omega_k(c), Eq. 15; 0 when the cell is kept
-    const uint32_t i_old = toff + cell_of(P.g, x, y, z);
-    const uint32_t i_new = toff + cell_of(P.g, x2, y2, z2);
-    const bool moved = i_new != i_old;
+// dE_nb = omega_k(c') - omega_k(c), Eq. 15; exactly 0 when the cell is kept.  The
+// loads are predicated, not branched around, so several moves' gathers are in flight together.
+__device__ __forceinline__ float field_delta(const float* __restrict__ omega, uint32_t i_old, uint32_t i_new)
+{
     float w_new = 0.0f, w_old = 0.0f;
-    if (moved) {
+    if (i_new != i_old) {
         w_new = __ldg(omega + i_new);
         w_old = __ldg(omega + i_old);
     }
-    const float e_nb = w_new - w_old;
+    return w_new - w_old;
+}
 
-    // bonded: dE_b = k_0/2 (2 d.s + m |d|^2), Eq. 2
+// s = sum over bonded neighbours of (r - r_nb); an absent neighbour is passed as the bead itself.
+__device__ __forceinline__ void bond_sum(float x, float y, float z, float xl, float yl, float zl,
+                                         float xr, float yr, float zr, float& sx, float& sy, float& sz)
+{
+    sx = (x - xl) + (x - xr);
+    sy = (y - yl) + (y - yr);
+    sz = (z - zl) + (z - zr);
+}
+
+// bonded: dE_b = k_0/2 (2 d.s + m |d|^2), Eq. 2
+__device__ __forceinline__ float bonded_delta(float half_k0, float mf, float dx, float dy, float dz,
+                                              float sx, float sy, float sz)
+{
     const float ds = fmaf(dz, sz, fmaf(dy, sy, dx * sx));
     const float dd = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    const float e_b = (kMove == 1 ? P.hk : 0.5f * P.k0) * fmaf(2.0f, ds, mf * dd);
+    return half_k0 * fmaf(2.0f, ds, mf * dd);
+}
 
-    float dE = e_b + e_nb;
-    if (kMove == 2) dE = dE + log_ratio;
+// Metropolis: accept iff dE <= 0 or u < exp(-dE)
+__device__ __forceinline__ bool metropolis(float dE, float u)
+{
+    return (dE <= 0.0f) || (u < ex2_approx(dE * -1.4426950408889634f));
+}
 
-    // Metropolis: accept iff dE <= 0 or u < exp(-dE)
-    const bool acc = (dE <= 0.0f) || (u < ex2_approx(dE * -1.4426950408889634f));
-    x = acc ? x2 : x;
-    y = acc ? y2 : y;
-    z = acc ? z2 : z;
-    if (kIncr && acc && moved) {
+// Smart-MC proposal from the bonded force F = -k_0 s (refs [28,29]):
+//   d = a_s F + sqrt(2 a_s) g,   ln T(r->r') - ln T(r'->r) = (|d + a_s F'|^2 - |d - a_s F|^2) / (4 a_s),
+//   F' = F - k_0 m d
+__device__ __forceinline__ void smc_proposal(const MoveP& P, float mf, float sx, float sy, float sz,
+                                             const Draw& g, float& dx, float& dy, float& dz, float& log_ratio)
+{
+    const float Fx = -P.k0 * sx, Fy = -P.k0 * sy, Fz = -P.k0 * sz;
+    dx = fmaf(P.a_s, Fx, P.noise * g.a);
+    dy = fmaf(P.a_s, Fy, P.noise * g.b);
+    dz = fmaf(P.a_s, Fz, P.noise * g.c);
+    const float km = P.k0 * mf;
+    float fwd = 0.0f, rev = 0.0f;
+    {
+        const float ef = dx - P.a_s * Fx, er = dx + P.a_s * (Fx - km * dx);
+        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
+    }
+    {
+        const float ef = dy - P.a_s * Fy, er = dy + P.a_s * (Fy - km * dy);
+        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
+    }
+    {
+        const float ef = dz - P.a_s * Fz, er = dz + P.a_s * (Fz - km * dz);
+        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
+    }
+    log_ratio = (rev - fwd) / P.four_as;
+}
+
+// The occupation numbers follow an accepted move (+1 new cell, -1 old cell): integer arithmetic, so
+// they stay identical to a fresh histogram (a3, Eq. 4).
+__device__ __forceinline__ void count_follow(uint32_t* __restrict__ counts, bool acc, uint32_t i_old, uint32_t i_new)
+{
+    if (acc && i_new != i_old) {
         atomicAdd(counts + i_new, 1u);
         atomicAdd(counts + i_old, 0xFFFFFFFFu);
     }
+}
+
+// One whole move of one bead (generic kernel).  (x,y,z) is updated in place when accepted.
+//   (xl..),(xr..)  chain neighbours; an absent neighbour is passed as the bead itself (bond 0)
+//   mf             number of bonded neighbours as float
+//   toff           type * cells, offset of this bead type's plane in omega / counts
+//   gid            global bead index = Philox counter word 0
+template <int kMove, bool kIncr>
+__device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
+                                        uint32_t* __restrict__ counts, float& x, float& y, float& z,
+                                        float xl, float yl, float zl, float xr, float yr, float zr,
+                                        float mf, uint32_t toff, uint32_t gid)
+{
+    const Draw q = draw_move<kMove>(P, gid);
+    float sx, sy, sz;
+    bond_sum(x, y, z, xl, yl, zl, xr, yr, zr, sx, sy, sz);
+    float dx = q.a, dy = q.b, dz = q.c, log_ratio = 0.0f;
+    if (kMove == 2) smc_proposal(P, mf, sx, sy, sz, q, dx, dy, dz, log_ratio);
+    const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
+    const uint32_t i_old = toff + cell_of(P.g, x, y, z);
+    const uint32_t i_new = toff + cell_of(P.g, x2, y2, z2);
+    const float e_nb = field_delta(omega, i_old, i_new);
+    const float e_b = bonded_delta(kMove == 1 ? P.hk : 0.5f * P.k0, mf, dx, dy, dz, sx, sy, sz);
+    float dE = e_b + e_nb;
+    if (kMove == 2) dE = dE + log_ratio;
+    const bool acc = metropolis(dE, q.u);
+    x = acc ? x2 : x;
+    y = acc ? y2 : y;
+    z = acc ? z2 : z;
+    if (kIncr) count_follow(counts, acc, i_old, i_new);
     return acc;
 }
 
 // ------------------------------------------------------------------------------------------------
-// a1 + a2 fused, chain-resident.  Requires N in {4, 8, ..., 128} (N | 128) so that a 128-bead warp
-// tile holds whole chains; the architecture's bead array starts 512-byte aligned.  Only full tiles
-// are processed here; the host sends a ragged tail (< 128 beads, whole chains) to the generic kernel.
+// a1 + a2 (+ a3) fused, chain-resident.  Requires N in {4, 8, ..., 128} (N | 128) so that a 128-bead
+// warp tile holds whole chains; the architecture's bead array starts 512-byte aligned.  Only full
+// tiles are processed here; the host sends a ragged tail (< 128 beads, whole chains) to the generic
+// kernel.  Block b owns the contiguous tile range [b T / B, (b+1) T / B); its warps take those tiles
+// round-robin.  Per tile and lane (4 consecutive monomers in registers):
+//   1. the next tile's positions are requested (register prefetch, hides the HBM latency);
+//   2. all four Philox draws (they depend on nothing loaded);
+//   3. local move: all four trial positions, all eight cell indices, all eight omega gathers in
+//      flight at once -- dE_nb (Eq. 15) does not depend on the neighbours, only dE_b does;
+//   4. set 0 (even monomers) decides, then set 1 (odd monomers) with the moved even neighbours
+//      (independent sets of Fig. 1 / Code 2); neighbours across lanes by shuffle;
+//   5. count updates for the accepted moves, one 128-bit store per coordinate array.
+// Smart-MC proposals depend on the neighbours, so there steps 3-4 run per set.
 //   x,y,z       base of this architecture's beads (padded layout)
 //   toff_tab    [N] type * cells of every monomer of the chain
 //   n_tiles     full tiles of this architecture (n_chains * N / 128)
 //   gid0        global index of the architecture's first bead
-//   dec_bytes   decision bitmap of the architecture (byte view), or unused
+//   dec_words   decision bitmap (whole system), or unused
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord>
-__global__ void __launch_bounds__(256, SOMA_FUSED_MIN_BLOCKS)
+__global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
                    const uint32_t* __restrict__ toff_tab, uint32_t n_mask, uint32_t n_tiles,
-                   uint32_t gid0, uint8_t* __restrict__ dec_bytes,
+                   uint32_t gid0, uint32_t* __restrict__ dec_words,
                    unsigned long long* __restrict__ acc_slots)
 {
+    constexpr uint32_t kFull = 0xFFFFFFFFu;
     const uint32_t lane = threadIdx.x & 31u;
-    const uint32_t warp = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    const uint32_t n_warps = (gridDim.x * blockDim.x) >> 5;
+    const uint32_t wib = threadIdx.x >> 5;
+    constexpr uint32_t kWarps = kFusedThreads / 32;
+    const uint32_t t_begin = (uint32_t)(((uint64_t)blockIdx.x * n_tiles) / gridDim.x);
+    const uint32_t t_end = (uint32_t)(((uint64_t)(blockIdx.x + 1) * n_tiles) / gridDim.x);
     const uint32_t j0 = (4u * lane) & n_mask;                 // monomer index of slot 0
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
     const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
     const uint4 toff = *reinterpret_cast<const uint4*>(toff_tab + j0);
     const float mf0 = has_l0 ? 2.0f : 1.0f, mf3 = has_r3 ? 2.0f : 1.0f;
+    const float half_k0 = kMove == 1 ? P.hk : 0.5f * P.k0;
     uint32_t n_acc = 0;
 
-    for (uint32_t tile = warp; tile < n_tiles; tile += n_warps) {
+    uint32_t tile = t_begin + wib;
+    float4 X, Y, Z;
+    if (tile < t_end) {
         const uint32_t i0 = tile * kTile + 4u * lane;
-        float4 X = *reinterpret_cast<const float4*>(x + i0);
-        float4 Y = *reinterpret_cast<const float4*>(y + i0);
-        float4 Z = *reinterpret_cast<const float4*>(z + i0);
+        X = *reinterpret_cast<const float4*>(x + i0);
+        Y = *reinterpret_cast<const float4*>(y + i0);
+        Z = *reinterpret_cast<const float4*>(z + i0);
+    }
+    for (; tile < t_end; tile += kWarps) {
+        const uint32_t i0 = tile * kTile + 4u * lane;
         const uint32_t gid = gid0 + i0;
 
-        // ---- set 0: even monomers (slots 0, 2) see the old odd monomers --------------------
-        float xl = __shfl_up_sync(0xFFFFFFFFu, X.w, 1), yl = __shfl_up_sync(0xFFFFFFFFu, Y.w, 1),
-              zl = __shfl_up_sync(0xFFFFFFFFu, Z.w, 1);
-        xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
-        const bool a0 = mc_move<kMove, kIncr>(P, omega, counts, X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, mf0, toff.x, gid);
-        const bool a2 = mc_move<kMove, kIncr>(P, omega, counts, X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, 2.0f, toff.z, gid + 2u);
+        // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
+        const uint32_t tile_n = min(tile + kWarps, t_end - 1u);
+        const uint32_t i0n = tile_n * kTile + 4u * lane;
+        const float4 Xn = *reinterpret_cast<const float4*>(x + i0n);
+        const float4 Yn = *reinterpret_cast<const float4*>(y + i0n);
+        const float4 Zn = *reinterpret_cast<const float4*>(z + i0n);
 
-        // ---- set 1: odd monomers (slots 1, 3) see the moved even monomers ------------------
-        float xr = __shfl_down_sync(0xFFFFFFFFu, X.x, 1), yr = __shfl_down_sync(0xFFFFFFFFu, Y.x, 1),
-              zr = __shfl_down_sync(0xFFFFFFFFu, Z.x, 1);
-        xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
-        const bool a1 = mc_move<kMove, kIncr>(P, omega, counts, X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, 2.0f, toff.y, gid + 1u);
-        const bool a3 = mc_move<kMove, kIncr>(P, omega, counts, X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, mf3, toff.w, gid + 3u);
+        // 2. random numbers of the four moves
+        const Draw q0 = draw_move<kMove>(P, gid), q1 = draw_move<kMove>(P, gid + 1u),
+                   q2 = draw_move<kMove>(P, gid + 2u), q3 = draw_move<kMove>(P, gid + 3u);
+
+        bool a0, a1, a2, a3;
+        if (kMove == 1) {
+            // 3. trial positions r' = fl32(r + d), cells, field differences
+            const float x0n = X.x + q0.a, y0n = Y.x + q0.b, z0n = Z.x + q0.c;
+            const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
+            const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
+            const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
+            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
+            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
+            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
+                        e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
+
+            // 4a. set 0: even monomers (slots 0, 2) see the old odd monomers
+            float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+            xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+            float sx, sy, sz;
+            bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
+            a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
+            bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
+            a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
+            X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
+            X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
+
+            // 4b. set 1: odd monomers (slots 1, 3) see the moved even monomers
+            float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+            xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+            bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
+            a1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, q1.u);
+            bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
+            a3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, q3.u);
+            X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
+            X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
+
+            // 5. occupation numbers follow the accepted moves
+            if (kIncr) {
+                count_follow(counts, a0, o0, n0);
+                count_follow(counts, a1, o1, n1);
+                count_follow(counts, a2, o2, n2);
+                count_follow(counts, a3, o3, n3);
+            }
+        } else {
+            // Smart-MC: the proposal needs the bonded force, i.e. the neighbours as they are now
+            float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+            xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+            float sx0, sy0, sz0, sx2, sy2, sz2, dx0, dy0, dz0, dx2, dy2, dz2, lr0, lr2;
+            bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx0, sy0, sz0);
+            bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx2, sy2, sz2);
+            smc_proposal(P, mf0, sx0, sy0, sz0, q0, dx0, dy0, dz0, lr0);
+            smc_proposal(P, 2.0f, sx2, sy2, sz2, q2, dx2, dy2, dz2, lr2);
+            const float x0n = X.x + dx0, y0n = Y.x + dy0, z0n = Z.x + dz0;
+            const float x2n = X.z + dx2, y2n = Y.z + dy2, z2n = Z.z + dz2;
+            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
+            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const float e0 = field_delta(omega, o0, n0), e2 = field_delta(omega, o2, n2);
+            a0 = metropolis((bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0) + e0) + lr0, q0.u);
+            a2 = metropolis((bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2) + e2) + lr2, q2.u);
+            X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
+            X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
+            if (kIncr) { count_follow(counts, a0, o0, n0); count_follow(counts, a2, o2, n2); }
+
+            float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+            xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+            float sx1, sy1, sz1, sx3, sy3, sz3, dx1, dy1, dz1, dx3, dy3, dz3, lr1, lr3;
+            bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx1, sy1, sz1);
+            bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx3, sy3, sz3);
+            smc_proposal(P, 2.0f, sx1, sy1, sz1, q1, dx1, dy1, dz1, lr1);
+            smc_proposal(P, mf3, sx3, sy3, sz3, q3, dx3, dy3, dz3, lr3);
+            const float x1n = X.y + dx1, y1n = Y.y + dy1, z1n = Z.y + dz1;
+            const float x3n = X.w + dx3, y3n = Y.w + dy3, z3n = Z.w + dz3;
+            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
+            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const float e1 = field_delta(omega, o1, n1), e3 = field_delta(omega, o3, n3);
+            a1 = metropolis((bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1) + e1) + lr1, q1.u);
+            a3 = metropolis((bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3) + e3) + lr3, q3.u);
+            X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
+            X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
+            if (kIncr) { count_follow(counts, a1, o1, n1); count_follow(counts, a3, o3, n3); }
+        }
 
         *reinterpret_cast<float4*>(x + i0) = X;
         *reinterpret_cast<float4*>(y + i0) = Y;
@@ -293,12 +439,16 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         const uint32_t nib = (a0 ? 1u : 0u) | (a1 ? 2u : 0u) | (a2 ? 4u : 0u) | (a3 ? 8u : 0u);
         n_acc += __popc(nib);
         if (kRecord) {
-            const uint32_t hi = __shfl_down_sync(0xFFFFFFFFu, nib, 1);
-            if ((lane & 1u) == 0u) dec_bytes[i0 >> 3] = (uint8_t)(nib | (hi << 4));
+            // bit (b & 31) of word (b >> 5) for bead b; gid is a multiple of 4 only if gid0 is
+            const unsigned long long bits = (unsigned long long)nib << (gid & 31u);
+            if ((uint32_t)bits) atomicOr(dec_words + (gid >> 5), (uint32_t)bits);
+            if ((uint32_t)(bits >> 32)) atomicOr(dec_words + (gid >> 5) + 1u, (uint32_t)(bits >> 32));
         }
+        X = Xn; Y = Yn; Z = Zn;
     }
-    n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
-    if (lane == 0 && n_acc) atomicAdd(acc_slots + (warp % kAccSlots), (unsigned long long)n_acc);
+    n_acc = __reduce_add_sync(kFull, n_acc);
+    if (lane == 0 && n_acc)
+        atomicAdd(acc_slots + ((blockIdx.x * kWarps + wib) % kAccSlots), (unsigned long long)n_acc);
 }
 
 // ------------------------------------------------------------------------------------------------
