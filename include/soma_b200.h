@@ -60,11 +60,17 @@ enum {
     SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */
     SOMA_OPT_SWEEP_COUNTER = 8,    /* set the sweep counter (the "time step" word of the Philox counter)      */
     SOMA_OPT_GRAPH = 9,            /* 1: replay soma_step's launches from a CUDA graph (default 1)            */
-    SOMA_OPT_BLOCKS_PER_SM = 10    /* tuning: grid of the fused kernel = SMs x this many blocks; 0 = resident max */
+    SOMA_OPT_BLOCKS_PER_SM = 10,   /* tuning: grid of the fused kernel = SMs x this many blocks; 0 = resident max */
+    SOMA_OPT_LAYOUT = 11,          /* 0: chains stay in the caller's order in device memory; 1 (default): the  */
+                                   /* library keeps them in Hilbert order of their centres of mass.  Storage   */
+                                   /* only: every result is identical, every API array is in the caller's order */
+    SOMA_OPT_SORT_INTERVAL = 12,   /* re-sort every this many sweeps (default 2000; 0: only at init/set_positions) */
+    SOMA_OPT_WINDOW = 13           /* 1: the fused kernel reads omega through a shared-memory window */
+                                   /* around each group of tiles (needs layout 1); 0 (default): from global memory */
 };
 
 /* indices of soma_kernel_times */
-enum { SOMA_K_MOVE = 0, SOMA_K_DENSITY = 1, SOMA_K_FIELD = 2, SOMA_K_COUNT = 3 };
+enum { SOMA_K_MOVE = 0, SOMA_K_DENSITY = 1, SOMA_K_FIELD = 2, SOMA_K_LAYOUT = 3, SOMA_K_COUNT = 4 };
 
 typedef struct soma_ctx soma_ctx; /* opaque */
 

@@ -8,8 +8,15 @@
 //   toff        uint32 per monomer of every architecture: type * cells
 //   decisions   1 bit per bead (only written with SOMA_OPT_RECORD_DECISIONS)
 //   acc_slots   256 spread 64-bit counters of accepted moves
+//   orig        uint32 per chain slot: the caller's index of the chain stored there (soma_layout.cuh);
+//               chains are kept in Hilbert order of their centres of mass (SOMA_OPT_LAYOUT), re-sorted
+//               every SOMA_OPT_SORT_INTERVAL sweeps; origins = window origin of every group of tiles
 #include "soma_kernels.cuh"
+#include "soma_layout.cuh"
 
+#include <cub/device/device_radix_sort.cuh>
+
+#include <algorithm>
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
@@ -51,6 +58,10 @@ struct Spec {
     uint64_t off = 0;       // offset of the segment in the padded device arrays
     uint32_t toff_off = 0;  // offset into the toff table
     bool fused_ok = false;  // N in {4, ..., 128}, N | 128
+    uint32_t log2N = 0;     // fused_ok only
+    uint64_t chain_off = 0; // offset into orig[]
+    uint64_t group_off = 0; // offset into origins[]
+    uint32_t n_tiles = 0, n_groups = 0;   // full 128-bead tiles; window groups of them (fused_ok only)
 };
 
 constexpr int kEventPool = 2048;
@@ -75,6 +86,25 @@ struct soma_ctx {
     unsigned long long* acc_slots = nullptr;
     unsigned long long* acc_host = nullptr;  // pinned staging for soma_stats
 
+    // layout (soma_layout.cuh)
+    uint32_t* orig = nullptr;        // [n_chains of all architectures]
+    uint32_t* orig_tmp = nullptr;
+    float* scratch = nullptr;        // n_pad floats: target of a permutation, then swapped in
+    float* stage = nullptr;          // 3 * n_beads floats in the caller's order (allocated on first use)
+    uint32_t *sort_keys[2] = {nullptr, nullptr}, *sort_vals[2] = {nullptr, nullptr};
+    void* cub_tmp = nullptr;
+    size_t cub_tmp_bytes = 0;
+    int4* origins = nullptr;
+    uint64_t n_chains_total = 0, max_chains = 0, n_groups_total = 0;
+    int layout = 1;                  // 0: caller's order, 1: Hilbert order
+    int window = 0;                  // shared-memory omega window in the fused kernel (needs layout 1)
+    int sort_interval = 2000;        // sweeps between re-sorts (0: only at init / set_positions)
+    uint64_t sweeps_since_sort = 0;
+    bool sorted = false;
+    soma::WinP win = {};
+    uint32_t win_tiles = 0;          // tiles per window group
+    size_t win_smem = 0;             // dynamic shared memory of the fused kernel with a window
+
     cudaStream_t stream = nullptr;
     int device = 0, n_sm = 0;
 
@@ -90,8 +120,8 @@ struct soma_ctx {
     std::vector<cudaEvent_t> ev;   // pairs
     std::vector<int> ev_class;
     int ev_used = 0;
-    double t_ms[SOMA_K_COUNT] = {0, 0, 0};
-    uint64_t t_launches[SOMA_K_COUNT] = {0, 0, 0};
+    double t_ms[SOMA_K_COUNT] = {};
+    uint64_t t_launches[SOMA_K_COUNT] = {};
 
     soma::GridP gridp() const;
     soma::MoveP movep(uint64_t sweep_no) const;
@@ -128,6 +158,17 @@ soma::MoveP soma_ctx::movep(uint64_t sweep_no) const
     }
     p.sweep_lo = (uint32_t)sweep_no;
     p.sweep_hi = (uint32_t)(sweep_no >> 32);
+    // Philox rounds 1-2 over the counter words every bead shares (philox4x32_10_head)
+    for (uint32_t sub = 0; sub < 2; ++sub) {
+        const uint32_t tag = ((uint32_t)move << 8) | sub;
+        const uint64_t pc1 = (uint64_t)p.sweep_hi * 0xCD9E8D57ull;
+        const uint32_t a1 = (uint32_t)(pc1 >> 32) ^ p.sweep_lo ^ p.rk[0][0];
+        const uint64_t pa2 = (uint64_t)a1 * 0xD2511F53ull;
+        p.head[sub][0] = tag ^ p.rk[0][1];
+        p.head[sub][1] = (uint32_t)pc1 ^ p.rk[1][0];
+        p.head[sub][2] = (uint32_t)(pa2 >> 32) ^ p.rk[1][1];
+        p.head[sub][3] = (uint32_t)pa2;
+    }
     return p;
 }
 
@@ -195,6 +236,31 @@ bool spec_uses_fused(const soma_ctx* c, const Spec& s)
     return true;
 }
 
+template <int kMove, bool kIncr, bool kRecord, bool kWin>
+int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
+{
+    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kWin>;
+    constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
+    const size_t smem = kWin ? c->win_smem : 0;
+    int per_sm = c->blocks_per_sm;
+    if (per_sm <= 0) {   // auto: every block resident, one wave
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
+        if (per_sm < 1) per_sm = 1;
+    }
+    int blocks = c->n_sm * per_sm;
+    soma::WinP W = c->win;
+    W.tiles_per_group = c->win_tiles;
+    W.n_groups = s.n_groups;
+    const int max_useful = kWin ? (int)s.n_groups : (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
+    if (blocks > max_useful) blocks = max_useful;
+    Timed t(c, SOMA_K_MOVE, 1);
+    kernel<<<blocks, threads, smem, c->stream>>>(
+        P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N - 1u, s.n_tiles,
+        (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots, W, c->origins + s.group_off,
+        (uint32_t)c->n_types);
+    return SOMA_OK;
+}
+
 template <int kMove, bool kIncr, bool kRecord>
 int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
 {
@@ -203,23 +269,12 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         float *x = c->x + s.off, *y = c->y + s.off, *z = c->z + s.off;
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
-        if (spec_uses_fused(c, s) && s.n_beads >= soma::kTile) {
-            const uint32_t n_tiles = (uint32_t)(s.n_beads / soma::kTile);
-            constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
-            int per_sm = c->blocks_per_sm;
-            if (per_sm <= 0) {   // auto: every block resident, one wave
-                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(
-                    &per_sm, soma::fused_sweep_kernel<kMove, kIncr, kRecord>, threads, 0));
-                if (per_sm < 1) per_sm = 1;
-            }
-            int blocks = c->n_sm * per_sm;
-            const int max_useful = (int)((n_tiles + warps_per_block - 1) / warps_per_block);
-            if (blocks > max_useful) blocks = max_useful;
-            Timed t(c, SOMA_K_MOVE, 1);
-            soma::fused_sweep_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
-                P, x, y, z, c->omega, c->counts, toff, s.N - 1u, n_tiles, (uint32_t)s.gid0,
-                c->decisions, c->acc_slots);
-            done = (uint64_t)n_tiles * soma::kTile;
+        if (spec_uses_fused(c, s) && s.n_tiles > 0) {
+            const bool win = c->window && c->layout && c->win_tiles && s.n_groups > 0;
+            int rc = win ? launch_fused<kMove, kIncr, kRecord, true>(c, P, s)
+                         : launch_fused<kMove, kIncr, kRecord, false>(c, P, s);
+            if (rc) return rc;
+            done = (uint64_t)s.n_tiles * soma::kTile;
         }
         if (done < s.n_beads) {   // whole chains the fused kernel does not cover (all of them, or a ragged tail)
             const uint64_t n_chains = (s.n_beads - done) / s.N;
@@ -232,7 +287,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::generic_move_kernel<kMove, kIncr, kRecord><<<(unsigned)blocks, threads, 0, c->stream>>>(
                     P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity, n_items,
-                    (uint32_t)(s.gid0 + done), c->decisions, c->acc_slots);
+                    (uint32_t)s.gid0, c->orig + s.chain_off + done / s.N, c->decisions, c->acc_slots);
             }
         }
         CU(cudaGetLastError());
@@ -298,21 +353,91 @@ int stage1(soma_ctx* c)
     return launch_fields(c);
 }
 
+// ---- layout: Hilbert order of the chains, window origins, caller order <-> device order ----------
+int ensure_stage(soma_ctx* c)
+{
+    if (!c->stage) CU(cudaMalloc(&c->stage, sizeof(float) * 3 * c->n_beads));
+    return SOMA_OK;
+}
+
+// Window origin of every group of tiles of every architecture (after a sort, or for the caller's order).
+int launch_origins(soma_ctx* c)
+{
+    if (!c->win_tiles) return SOMA_OK;
+    for (const Spec& s : c->specs) {
+        if (!s.fused_ok || s.n_groups == 0) continue;
+        const uint32_t chains_per_group = c->win_tiles * (soma::kTile / s.N);
+        Timed t(c, SOMA_K_LAYOUT, 1);
+        soma::group_origin_kernel<<<s.n_groups, 128, 0, c->stream>>>(
+            c->x + s.off, c->y + s.off, c->z + s.off, (uint32_t)s.n_chains, s.N, chains_per_group,
+            (float)(1.0 / (double)c->box[0]), (float)(1.0 / (double)c->box[1]), (float)(1.0 / (double)c->box[2]),
+            c->grid[0], c->grid[1], c->grid[2], 1 << c->win.sh[0], 1 << c->win.sh[1], 1 << c->win.sh[2],
+            c->origins + s.group_off);
+    }
+    CU(cudaGetLastError());
+    return SOMA_OK;
+}
+
+// Put the chains of every architecture in Hilbert order of their centres of mass.
+int resort(soma_ctx* c)
+{
+    c->sweeps_since_sort = 0;
+    if (c->layout == 0) return SOMA_OK;
+    int max_n = std::max(c->grid[0], std::max(c->grid[1], c->grid[2]));
+    uint32_t bits = 1;
+    while (bits < 10 && (1 << bits) < max_n) ++bits;
+    for (const Spec& s : c->specs) {
+        if (s.n_chains < 2) continue;
+        const uint32_t n = (uint32_t)s.n_chains;
+        Timed t(c, SOMA_K_LAYOUT, 5);
+        soma::chain_key_kernel<<<(n + 127) / 128, 128, 0, c->stream>>>(
+            c->x + s.off, c->y + s.off, c->z + s.off, n, s.N, (float)(1.0 / (double)c->box[0]),
+            (float)(1.0 / (double)c->box[1]), (float)(1.0 / (double)c->box[2]), bits, c->sort_keys[0], c->sort_vals[0]);
+        size_t tmp = c->cub_tmp_bytes;
+        CU(cub::DeviceRadixSort::SortPairs(c->cub_tmp, tmp, c->sort_keys[0], c->sort_keys[1], c->sort_vals[0],
+                                           c->sort_vals[1], (int)n, 0, (int)(3 * bits), c->stream));
+        const uint32_t* order = c->sort_vals[1];          // order[new slot] = old slot
+        const unsigned blocks = (unsigned)((s.n_beads + 255) / 256);
+        float** arr[3] = {&c->x, &c->y, &c->z};
+        for (int a = 0; a < 3; ++a) {
+            // gather this architecture's segment into the scratch array, then copy it back in place
+            soma::permute_chains_kernel<<<blocks, 256, 0, c->stream>>>(c->scratch + s.off, *arr[a] + s.off, order, s.N, s.n_beads);
+            CU(cudaMemcpyAsync(*arr[a] + s.off, c->scratch + s.off, sizeof(float) * s.n_beads, cudaMemcpyDeviceToDevice, c->stream));
+        }
+        soma::permute_ids_kernel<<<(n + 255) / 256, 256, 0, c->stream>>>(c->orig_tmp, c->orig + s.chain_off, order, n);
+        CU(cudaMemcpyAsync(c->orig + s.chain_off, c->orig_tmp, sizeof(uint32_t) * n, cudaMemcpyDeviceToDevice, c->stream));
+        CU(cudaGetLastError());
+    }
+    c->sorted = true;
+    return launch_origins(c);
+}
+
+// caller's SoA x | y | z  <->  device layout, through orig[]
 int copy_soa(soma_ctx* c, float* dst_user, const float* src_user, bool to_user, bool user_is_device)
 {
-    // user layout: x[nb] | y[nb] | z[nb]; device layout: padded segments
-    float* dev[3] = {c->x, c->y, c->z};
-    for (int a = 0; a < 3; ++a)
-        for (const Spec& s : c->specs) {
-            if (s.n_beads == 0) continue;
-            const size_t bytes = sizeof(float) * s.n_beads;
-            if (to_user)
-                CU(cudaMemcpyAsync(dst_user + (size_t)a * c->n_beads + s.gid0, dev[a] + s.off, bytes,
-                                   user_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
-            else
-                CU(cudaMemcpyAsync(dev[a] + s.off, src_user + (size_t)a * c->n_beads + s.gid0, bytes,
-                                   user_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice, c->stream));
-        }
+    float* user = to_user ? dst_user : const_cast<float*>(src_user);
+    float* dev_user = user;
+    if (!user_is_device) {
+        int rc = ensure_stage(c);
+        if (rc) return rc;
+        dev_user = c->stage;
+        if (!to_user)
+            CU(cudaMemcpyAsync(c->stage, src_user, sizeof(float) * 3 * c->n_beads, cudaMemcpyHostToDevice, c->stream));
+    }
+    for (const Spec& s : c->specs) {
+        if (s.n_beads == 0) continue;
+        const unsigned blocks = (unsigned)((s.n_beads + 255) / 256);
+        Timed t(c, SOMA_K_LAYOUT, 1);
+        if (to_user)
+            soma::reorder_kernel<true><<<blocks, 256, 0, c->stream>>>(dev_user, c->n_beads, c->x + s.off, c->y + s.off,
+                                                                     c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.gid0);
+        else
+            soma::reorder_kernel<false><<<blocks, 256, 0, c->stream>>>(dev_user, c->n_beads, c->x + s.off, c->y + s.off,
+                                                                      c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.gid0);
+    }
+    CU(cudaGetLastError());
+    if (!user_is_device && to_user)
+        CU(cudaMemcpyAsync(dst_user, c->stage, sizeof(float) * 3 * c->n_beads, cudaMemcpyDeviceToHost, c->stream));
     return SOMA_OK;
 }
 
@@ -334,6 +459,9 @@ void soma_destroy(soma_ctx* c)
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
     cudaFree(c->acc_slots);
+    cudaFree(c->orig); cudaFree(c->orig_tmp); cudaFree(c->scratch); cudaFree(c->stage);
+    cudaFree(c->sort_keys[0]); cudaFree(c->sort_keys[1]); cudaFree(c->sort_vals[0]); cudaFree(c->sort_vals[1]);
+    cudaFree(c->cub_tmp); cudaFree(c->origins);
     if (c->acc_host) cudaFreeHost(c->acc_host);
     delete c;
 }
@@ -392,6 +520,17 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         s.off = off;
         s.toff_off = (uint32_t)toff_host.size();
         s.fused_ok = s.N >= 4 && s.N <= 128 && (128 % s.N) == 0;
+        if (s.fused_ok) {
+            while ((1u << s.log2N) < s.N) ++s.log2N;
+            s.n_tiles = (uint32_t)(s.n_chains * s.N / soma::kTile);
+        }
+        s.chain_off = c->n_chains_total;
+        c->n_chains_total += s.n_chains;
+        c->max_chains = std::max<uint64_t>(c->max_chains, s.n_chains);
+        if (s.n_chains >= (1ull << 32)) {
+            delete c;
+            return fail(SOMA_EINVAL, "soma_init: spec %d has 2^32 or more chains", a);
+        }
         for (uint32_t j = 0; j < s.N; ++j) {
             const uint8_t t = s.n_chains ? chains[a].types[j] : 0;
             if (t >= n_types) {
@@ -446,6 +585,55 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         }                                                                              \
     } while (0)
 
+    // Shared-memory window of the fused kernel: powers of two per axis, at most 16 cells and never more
+    // than the axis; shrunk until omega of the box (all types) fits 32 KB, so five blocks stay resident.
+    {
+        uint32_t sh[3];
+        for (int a = 0; a < 3; ++a) {
+            sh[a] = 0;
+            while (sh[a] < 4 && (1 << sh[a]) < grid[a]) ++sh[a];
+        }
+        while (((size_t)n_types << (sh[0] + sh[1] + sh[2])) * sizeof(float) > 32768) {
+            int big = 0;
+            for (int a = 1; a < 3; ++a) if (sh[a] > sh[big]) big = a;
+            if (sh[big] == 0) break;
+            --sh[big];
+        }
+        const size_t lut_words = (size_t)grid[0] + grid[1] + grid[2];
+        const bool whole_grid = (1 << sh[0]) >= grid[0] && (1 << sh[1]) >= grid[1] && (1 << sh[2]) >= grid[2];
+        const uint32_t wcells = 1u << (sh[0] + sh[1] + sh[2]);
+        if (lut_words <= 2048 && wcells >= 64 && (1u << sh[2]) <= (uint32_t)soma::kFusedThreads) {
+            for (int a = 0; a < 3; ++a) c->win.sh[a] = sh[a];
+            c->win_smem = ((size_t)n_types * wcells + lut_words) * sizeof(uint32_t);
+            // 16^3 cells serve 32 tiles (4096 beads: 128 chains of 32 reach ~5 cells beyond their centres);
+            // a window that holds the whole grid serves any number of tiles
+            uint32_t max_tiles = 0;
+            for (const Spec& s : c->specs) max_tiles = std::max(max_tiles, s.n_tiles);
+            const uint32_t per_block = (max_tiles + (uint32_t)c->n_sm * 5u - 1u) / ((uint32_t)c->n_sm * 5u);
+            c->win_tiles = whole_grid ? std::max(4u, per_block) : std::max(4u, wcells / 128u);
+        }
+        for (Spec& s : c->specs) {
+            s.group_off = c->n_groups_total;
+            s.n_groups = (s.fused_ok && c->win_tiles) ? (s.n_tiles + c->win_tiles - 1) / c->win_tiles : 0;
+            c->n_groups_total += s.n_groups;
+        }
+    }
+
+    CUI(cudaMalloc(&c->orig, sizeof(uint32_t) * c->n_chains_total));
+    CUI(cudaMalloc(&c->orig_tmp, sizeof(uint32_t) * c->max_chains));
+    CUI(cudaMalloc(&c->scratch, sizeof(float) * c->n_pad));
+    for (int i = 0; i < 2; ++i) {
+        CUI(cudaMalloc(&c->sort_keys[i], sizeof(uint32_t) * c->max_chains));
+        CUI(cudaMalloc(&c->sort_vals[i], sizeof(uint32_t) * c->max_chains));
+    }
+    CUI(cub::DeviceRadixSort::SortPairs(nullptr, c->cub_tmp_bytes, c->sort_keys[0], c->sort_keys[1], c->sort_vals[0],
+                                        c->sort_vals[1], (int)c->max_chains, 0, 30, c->stream));
+    CUI(cudaMalloc(&c->cub_tmp, c->cub_tmp_bytes + 16));
+    CUI(cudaMalloc(&c->origins, sizeof(int4) * (c->n_groups_total + 1)));
+    CUI(cudaMemsetAsync(c->origins, 0, sizeof(int4) * (c->n_groups_total + 1), c->stream));
+    for (const Spec& s : c->specs)
+        if (s.n_chains)
+            soma::iota_kernel<<<(unsigned)((s.n_chains + 255) / 256), 256, 0, c->stream>>>(c->orig + s.chain_off, (uint32_t)s.n_chains);
     CUI(cudaMalloc(&c->x, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->y, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->z, sizeof(float) * c->n_pad));
@@ -479,6 +667,7 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         }
         if (cudaGetLastError() != cudaSuccess) rc = fail(SOMA_ECUDA, "soma_init: init_walk_kernel launch failed");
     }
+    if (rc == SOMA_OK) rc = resort(c);
     if (rc == SOMA_OK) rc = stage1(c);
     if (rc == SOMA_OK && cudaStreamSynchronize(c->stream) != cudaSuccess)
         rc = fail(SOMA_ECUDA, "soma_init: %s", cudaGetErrorString(cudaGetLastError()));
@@ -502,6 +691,11 @@ int soma_step(soma_ctx* c, int n_sweeps)
     for (int i = 0; i < n_sweeps; ++i) {
         if (c->record)
             CU(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32), c->stream));
+        if (c->layout && c->sort_interval > 0 && c->sweeps_since_sort >= (uint64_t)c->sort_interval) {
+            int rs = resort(c);                            // storage order only: no result depends on it
+            if (rs) return rs;
+        }
+        c->sweeps_since_sort += 1;
         const soma::MoveP P = c->movep(c->sweep);
         int rc = launch_moves(c, P);                       // a1, a2 (or a5) [+ a3 incremental]
         if (rc) return rc;
@@ -543,6 +737,8 @@ int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
 {
     if (!c || !xyz) return fail(SOMA_EINVAL, "soma_set_positions: NULL argument");
     int rc = copy_soa(c, nullptr, xyz, false, src_is_device != 0);
+    if (rc) return rc;
+    rc = resort(c);
     if (rc) return rc;
     rc = stage1(c);
     if (rc) return rc;
@@ -606,6 +802,33 @@ int soma_set_option(soma_ctx* c, int key, double value)
             if (iv < 0 || iv > 32) return fail(SOMA_EINVAL, "SOMA_OPT_BLOCKS_PER_SM: 0 (auto) .. 32");
             c->blocks_per_sm = iv;
             return SOMA_OK;
+        case SOMA_OPT_LAYOUT: {
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_LAYOUT: 0 or 1");
+            if (iv == c->layout) return SOMA_OK;
+            if (iv == 1) {
+                c->layout = 1;
+                return resort(c);
+            }
+            // back to the caller's order: export, reset orig to the identity, import
+            int rc = ensure_stage(c);
+            if (rc) return rc;
+            rc = copy_soa(c, c->stage, nullptr, true, true);
+            if (rc) return rc;
+            for (const Spec& s : c->specs)
+                if (s.n_chains)
+                    soma::iota_kernel<<<(unsigned)((s.n_chains + 255) / 256), 256, 0, c->stream>>>(c->orig + s.chain_off, (uint32_t)s.n_chains);
+            c->layout = 0;
+            c->sorted = false;
+            return copy_soa(c, nullptr, c->stage, false, true);
+        }
+        case SOMA_OPT_SORT_INTERVAL:
+            if (iv < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SORT_INTERVAL: must be >= 0");
+            c->sort_interval = iv;
+            return SOMA_OK;
+        case SOMA_OPT_WINDOW:
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_WINDOW: 0 or 1");
+            c->window = iv;
+            return SOMA_OK;
         default:
             return fail(SOMA_EINVAL, "soma_set_option: unknown key %d", key);
     }
@@ -654,6 +877,14 @@ uint64_t soma_launch_count(const soma_ctx* c) { return c ? c->launches : 0; }
 uint64_t soma_n_beads(const soma_ctx* c) { return c ? c->n_beads : 0; }
 uint64_t soma_n_cells(const soma_ctx* c) { return c ? c->cells : 0; }
 int soma_n_types(const soma_ctx* c) { return c ? c->n_types : 0; }
+
+#ifdef SOMA_DBG_FALLBACK
+int soma_debug(unsigned long long* out)
+{
+    cudaDeviceSynchronize();
+    return (int)cudaMemcpyFromSymbol(out, soma::g_dbg, sizeof(unsigned long long) * 4);
+}
+#endif
 
 int soma_sync(soma_ctx* c)
 {
