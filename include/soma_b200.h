@@ -64,9 +64,7 @@ enum {
     SOMA_OPT_LAYOUT = 11,          /* 0: chains stay in the caller's order in device memory; 1 (default): the  */
                                    /* library keeps them in Hilbert order of their centres of mass.  Storage   */
                                    /* only: every result is identical, every API array is in the caller's order */
-    SOMA_OPT_SORT_INTERVAL = 12,   /* re-sort every this many sweeps (default 2000; 0: only at init/set_positions) */
-    SOMA_OPT_WINDOW = 13           /* 1: the fused kernel reads omega through a shared-memory window */
-                                   /* around each group of tiles (needs layout 1); 0 (default): from global memory */
+    SOMA_OPT_SORT_INTERVAL = 12    /* re-sort every this many sweeps (default 2000; 0: only at init/set_positions) */
 };
 
 /* indices of soma_kernel_times */

@@ -10,7 +10,7 @@
 //   acc_slots   256 spread 64-bit counters of accepted moves
 //   orig        uint32 per chain slot: the caller's index of the chain stored there (soma_layout.cuh);
 //               chains are kept in Hilbert order of their centres of mass (SOMA_OPT_LAYOUT), re-sorted
-//               every SOMA_OPT_SORT_INTERVAL sweeps; origins = window origin of every group of tiles
+//               every SOMA_OPT_SORT_INTERVAL sweeps
 #include "soma_kernels.cuh"
 #include "soma_layout.cuh"
 
@@ -60,8 +60,7 @@ struct Spec {
     bool fused_ok = false;  // N in {4, ..., 128}, N | 128
     uint32_t log2N = 0;     // fused_ok only
     uint64_t chain_off = 0; // offset into orig[]
-    uint64_t group_off = 0; // offset into origins[]
-    uint32_t n_tiles = 0, n_groups = 0;   // full 128-bead tiles; window groups of them (fused_ok only)
+    uint32_t n_tiles = 0;   // full 128-bead tiles (fused_ok only)
 };
 
 constexpr int kEventPool = 2048;
@@ -94,16 +93,10 @@ struct soma_ctx {
     uint32_t *sort_keys[2] = {nullptr, nullptr}, *sort_vals[2] = {nullptr, nullptr};
     void* cub_tmp = nullptr;
     size_t cub_tmp_bytes = 0;
-    int4* origins = nullptr;
-    uint64_t n_chains_total = 0, max_chains = 0, n_groups_total = 0;
+    uint64_t n_chains_total = 0, max_chains = 0;
     int layout = 1;                  // 0: caller's order, 1: Hilbert order
-    int window = 0;                  // shared-memory omega window in the fused kernel (needs layout 1)
     int sort_interval = 2000;        // sweeps between re-sorts (0: only at init / set_positions)
     uint64_t sweeps_since_sort = 0;
-    bool sorted = false;
-    soma::WinP win = {};
-    uint32_t win_tiles = 0;          // tiles per window group
-    size_t win_smem = 0;             // dynamic shared memory of the fused kernel with a window
 
     cudaStream_t stream = nullptr;
     int device = 0, n_sm = 0;
@@ -236,28 +229,23 @@ bool spec_uses_fused(const soma_ctx* c, const Spec& s)
     return true;
 }
 
-template <int kMove, bool kIncr, bool kRecord, bool kWin>
+template <int kMove, bool kIncr, bool kRecord>
 int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
-    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kWin>;
+    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
-    const size_t smem = kWin ? c->win_smem : 0;
     int per_sm = c->blocks_per_sm;
     if (per_sm <= 0) {   // auto: every block resident, one wave
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, smem));
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0));
         if (per_sm < 1) per_sm = 1;
     }
     int blocks = c->n_sm * per_sm;
-    soma::WinP W = c->win;
-    W.tiles_per_group = c->win_tiles;
-    W.n_groups = s.n_groups;
-    const int max_useful = kWin ? (int)s.n_groups : (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
+    const int max_useful = (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
     if (blocks > max_useful) blocks = max_useful;
     Timed t(c, SOMA_K_MOVE, 1);
-    kernel<<<blocks, threads, smem, c->stream>>>(
+    kernel<<<blocks, threads, 0, c->stream>>>(
         P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N - 1u, s.n_tiles,
-        (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots, W, c->origins + s.group_off,
-        (uint32_t)c->n_types);
+        (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots);
     return SOMA_OK;
 }
 
@@ -270,9 +258,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
         if (spec_uses_fused(c, s) && s.n_tiles > 0) {
-            const bool win = c->window && c->layout && c->win_tiles && s.n_groups > 0;
-            int rc = win ? launch_fused<kMove, kIncr, kRecord, true>(c, P, s)
-                         : launch_fused<kMove, kIncr, kRecord, false>(c, P, s);
+            int rc = launch_fused<kMove, kIncr, kRecord>(c, P, s);
             if (rc) return rc;
             done = (uint64_t)s.n_tiles * soma::kTile;
         }
@@ -353,28 +339,10 @@ int stage1(soma_ctx* c)
     return launch_fields(c);
 }
 
-// ---- layout: Hilbert order of the chains, window origins, caller order <-> device order ----------
+// ---- layout: Hilbert order of the chains, caller order <-> device order ---------------------------
 int ensure_stage(soma_ctx* c)
 {
     if (!c->stage) CU(cudaMalloc(&c->stage, sizeof(float) * 3 * c->n_beads));
-    return SOMA_OK;
-}
-
-// Window origin of every group of tiles of every architecture (after a sort, or for the caller's order).
-int launch_origins(soma_ctx* c)
-{
-    if (!c->win_tiles) return SOMA_OK;
-    for (const Spec& s : c->specs) {
-        if (!s.fused_ok || s.n_groups == 0) continue;
-        const uint32_t chains_per_group = c->win_tiles * (soma::kTile / s.N);
-        Timed t(c, SOMA_K_LAYOUT, 1);
-        soma::group_origin_kernel<<<s.n_groups, 128, 0, c->stream>>>(
-            c->x + s.off, c->y + s.off, c->z + s.off, (uint32_t)s.n_chains, s.N, chains_per_group,
-            (float)(1.0 / (double)c->box[0]), (float)(1.0 / (double)c->box[1]), (float)(1.0 / (double)c->box[2]),
-            c->grid[0], c->grid[1], c->grid[2], 1 << c->win.sh[0], 1 << c->win.sh[1], 1 << c->win.sh[2],
-            c->origins + s.group_off);
-    }
-    CU(cudaGetLastError());
     return SOMA_OK;
 }
 
@@ -408,8 +376,7 @@ int resort(soma_ctx* c)
         CU(cudaMemcpyAsync(c->orig + s.chain_off, c->orig_tmp, sizeof(uint32_t) * n, cudaMemcpyDeviceToDevice, c->stream));
         CU(cudaGetLastError());
     }
-    c->sorted = true;
-    return launch_origins(c);
+    return SOMA_OK;
 }
 
 // caller's SoA x | y | z  <->  device layout, through orig[]
@@ -461,7 +428,7 @@ void soma_destroy(soma_ctx* c)
     cudaFree(c->acc_slots);
     cudaFree(c->orig); cudaFree(c->orig_tmp); cudaFree(c->scratch); cudaFree(c->stage);
     cudaFree(c->sort_keys[0]); cudaFree(c->sort_keys[1]); cudaFree(c->sort_vals[0]); cudaFree(c->sort_vals[1]);
-    cudaFree(c->cub_tmp); cudaFree(c->origins);
+    cudaFree(c->cub_tmp);
     if (c->acc_host) cudaFreeHost(c->acc_host);
     delete c;
 }
@@ -585,40 +552,6 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         }                                                                              \
     } while (0)
 
-    // Shared-memory window of the fused kernel: powers of two per axis, at most 16 cells and never more
-    // than the axis; shrunk until omega of the box (all types) fits 32 KB, so five blocks stay resident.
-    {
-        uint32_t sh[3];
-        for (int a = 0; a < 3; ++a) {
-            sh[a] = 0;
-            while (sh[a] < 4 && (1 << sh[a]) < grid[a]) ++sh[a];
-        }
-        while (((size_t)n_types << (sh[0] + sh[1] + sh[2])) * sizeof(float) > 32768) {
-            int big = 0;
-            for (int a = 1; a < 3; ++a) if (sh[a] > sh[big]) big = a;
-            if (sh[big] == 0) break;
-            --sh[big];
-        }
-        const size_t lut_words = (size_t)grid[0] + grid[1] + grid[2];
-        const bool whole_grid = (1 << sh[0]) >= grid[0] && (1 << sh[1]) >= grid[1] && (1 << sh[2]) >= grid[2];
-        const uint32_t wcells = 1u << (sh[0] + sh[1] + sh[2]);
-        if (lut_words <= 2048 && wcells >= 64 && (1u << sh[2]) <= (uint32_t)soma::kFusedThreads) {
-            for (int a = 0; a < 3; ++a) c->win.sh[a] = sh[a];
-            c->win_smem = ((size_t)n_types * wcells + lut_words) * sizeof(uint32_t);
-            // 16^3 cells serve 32 tiles (4096 beads: 128 chains of 32 reach ~5 cells beyond their centres);
-            // a window that holds the whole grid serves any number of tiles
-            uint32_t max_tiles = 0;
-            for (const Spec& s : c->specs) max_tiles = std::max(max_tiles, s.n_tiles);
-            const uint32_t per_block = (max_tiles + (uint32_t)c->n_sm * 5u - 1u) / ((uint32_t)c->n_sm * 5u);
-            c->win_tiles = whole_grid ? std::max(4u, per_block) : std::max(4u, wcells / 128u);
-        }
-        for (Spec& s : c->specs) {
-            s.group_off = c->n_groups_total;
-            s.n_groups = (s.fused_ok && c->win_tiles) ? (s.n_tiles + c->win_tiles - 1) / c->win_tiles : 0;
-            c->n_groups_total += s.n_groups;
-        }
-    }
-
     CUI(cudaMalloc(&c->orig, sizeof(uint32_t) * c->n_chains_total));
     CUI(cudaMalloc(&c->orig_tmp, sizeof(uint32_t) * c->max_chains));
     CUI(cudaMalloc(&c->scratch, sizeof(float) * c->n_pad));
@@ -629,8 +562,6 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
     CUI(cub::DeviceRadixSort::SortPairs(nullptr, c->cub_tmp_bytes, c->sort_keys[0], c->sort_keys[1], c->sort_vals[0],
                                         c->sort_vals[1], (int)c->max_chains, 0, 30, c->stream));
     CUI(cudaMalloc(&c->cub_tmp, c->cub_tmp_bytes + 16));
-    CUI(cudaMalloc(&c->origins, sizeof(int4) * (c->n_groups_total + 1)));
-    CUI(cudaMemsetAsync(c->origins, 0, sizeof(int4) * (c->n_groups_total + 1), c->stream));
     for (const Spec& s : c->specs)
         if (s.n_chains)
             soma::iota_kernel<<<(unsigned)((s.n_chains + 255) / 256), 256, 0, c->stream>>>(c->orig + s.chain_off, (uint32_t)s.n_chains);
@@ -818,16 +749,11 @@ int soma_set_option(soma_ctx* c, int key, double value)
                 if (s.n_chains)
                     soma::iota_kernel<<<(unsigned)((s.n_chains + 255) / 256), 256, 0, c->stream>>>(c->orig + s.chain_off, (uint32_t)s.n_chains);
             c->layout = 0;
-            c->sorted = false;
             return copy_soa(c, nullptr, c->stage, false, true);
         }
         case SOMA_OPT_SORT_INTERVAL:
             if (iv < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SORT_INTERVAL: must be >= 0");
             c->sort_interval = iv;
-            return SOMA_OK;
-        case SOMA_OPT_WINDOW:
-            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_WINDOW: 0 or 1");
-            c->window = iv;
             return SOMA_OK;
         default:
             return fail(SOMA_EINVAL, "soma_set_option: unknown key %d", key);
@@ -877,14 +803,6 @@ uint64_t soma_launch_count(const soma_ctx* c) { return c ? c->launches : 0; }
 uint64_t soma_n_beads(const soma_ctx* c) { return c ? c->n_beads : 0; }
 uint64_t soma_n_cells(const soma_ctx* c) { return c ? c->cells : 0; }
 int soma_n_types(const soma_ctx* c) { return c ? c->n_types : 0; }
-
-#ifdef SOMA_DBG_FALLBACK
-int soma_debug(unsigned long long* out)
-{
-    cudaDeviceSynchronize();
-    return (int)cudaMemcpyFromSymbol(out, soma::g_dbg, sizeof(unsigned long long) * 4);
-}
-#endif
 
 int soma_sync(soma_ctx* c)
 {

@@ -301,75 +301,11 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 }
 
 // ------------------------------------------------------------------------------------------------
-// Shared-memory window of the fields (fused kernel, kWin).  With the chains stored along a Hilbert
-// curve (soma_layout.cuh) the tiles of one group lie in a small region of the grid.  Before a block
-// works on a group it copies omega of a box of w[0] x w[1] x w[2] cells (powers of two) around that
-// region into shared memory with coalesced loads; the per-move gathers then read shared memory, and
-// only a bead outside the box goes to global memory (same value either way: the result does not
-// depend on the window).  Motivation: the scattered gathers were 38 % of all L2 requests of the
-// kernel, and L2 request slots were its busiest resource (profiles/r01b).
-//   lut[a][c]   per axis: (c - origin[a] mod n[a]) * stride[a] if that is < w[a], else kOutside; the
-//               sum of the three entries is the slot in the window, or >= kOutside
-// ------------------------------------------------------------------------------------------------
-constexpr uint32_t kOutside = 0x20000000u;
-#ifdef SOMA_DBG_FALLBACK
-__device__ unsigned long long g_dbg[4];
-#endif
-
-struct WinP {
-    uint32_t sh[3];            // log2 of the window size per axis
-    uint32_t tiles_per_group;  // tiles that share one window
-    uint32_t n_groups;
-};
-
-struct CellRef {
-    uint32_t idx;   // element of omega / counts: type * cells + cell
-    uint32_t loc;   // element of the window: type * wcells + slot, or >= kOutside (kWin only)
-};
-
-template <bool kWin>
-__device__ __forceinline__ CellRef locate(const GridP& g, const uint32_t* lut, float x, float y, float z,
-                                          uint32_t toff, uint32_t twoff)
-{
-    const uint32_t cx = axis_cell(x, g.inv_L[0], g.nf[0], g.nm1[0]);
-    const uint32_t cy = axis_cell(y, g.inv_L[1], g.nf[1], g.nm1[1]);
-    const uint32_t cz = axis_cell(z, g.inv_L[2], g.nf[2], g.nm1[2]);
-    CellRef r;
-    r.idx = toff + (cx * g.n[1] + cy) * g.n[2] + cz;
-    r.loc = kWin ? twoff + lut[cx] + lut[g.n[0] + cy] + lut[g.n[0] + g.n[1] + cz] : 0u;
-    return r;
-}
-
-// dE_nb = omega_k(c') - omega_k(c), Eq. 15, through the window where it covers the cell
-template <bool kWin>
-__device__ __forceinline__ float field_delta_ref(const float* __restrict__ omega, const float* om_w,
-                                                 const CellRef& o, const CellRef& n)
-{
-    float w_new = 0.0f, w_old = 0.0f;
-    if (n.idx != o.idx) {
-        if (kWin) {
-#ifdef SOMA_DBG_FALLBACK
-            atomicAdd(&g_dbg[0], 2ull);
-            atomicAdd(&g_dbg[1], (unsigned long long)((n.loc >= kOutside) + (o.loc >= kOutside)));
-#endif
-            w_new = n.loc < kOutside ? om_w[n.loc] : __ldg(omega + n.idx);
-            w_old = o.loc < kOutside ? om_w[o.loc] : __ldg(omega + o.idx);
-        } else {
-            w_new = __ldg(omega + n.idx);
-            w_old = __ldg(omega + o.idx);
-        }
-    }
-    return w_new - w_old;
-}
-
-// ------------------------------------------------------------------------------------------------
 // a1 + a2 (+ a3) fused, chain-resident.  Requires N in {4, 8, ..., 128} (N | 128) so that a 128-bead
 // warp tile holds whole chains; the architecture's bead array starts 512-byte aligned.  Only full
 // tiles are processed here; the host sends a ragged tail (< 128 beads, whole chains) to the generic
-// kernel.  The tiles are dealt out in groups: without a window (kWin false) block b's group is the
-// contiguous range [b T / B, (b+1) T / B); with a window the groups are W.tiles_per_group tiles long
-// and taken grid-stride.  A group's tiles go to the block's warps round-robin.  Per tile and lane
-// (4 consecutive monomers in registers):
+// kernel.  Block b owns the contiguous tile range [b T / B, (b+1) T / B); its warps take those tiles
+// round-robin.  Per tile and lane (4 consecutive monomers in registers):
 //   1. the next tile's positions are requested (register prefetch, hides the HBM latency);
 //   2. all four Philox draws (they depend on nothing loaded);
 //   3. local move: all four trial positions, all eight cell indices, all eight omega gathers in
@@ -384,19 +320,15 @@ __device__ __forceinline__ float field_delta_ref(const float* __restrict__ omega
 //   gid0        global index of the architecture's first bead
 //   orig        [n_chains] the caller's chain index of the chain in each slot (Philox counter, bitmap)
 //   dec_words   decision bitmap (whole system), or unused
-//   origin      [W.n_groups] window origin (cell) of every group (kWin)
-// Dynamic shared memory (kWin): n_types << (sh0+sh1+sh2) floats of omega, then n0+n1+n2 LUT words.
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord, bool kWin>
+template <int kMove, bool kIncr, bool kRecord>
 __global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
                    const uint32_t* __restrict__ toff_tab, uint32_t n_mask, uint32_t n_tiles,
                    uint32_t gid0, const uint32_t* __restrict__ orig, uint32_t log2N,
-                   uint32_t* __restrict__ dec_words, unsigned long long* __restrict__ acc_slots,
-                   const WinP W, const int4* __restrict__ origin, uint32_t n_types)
+                   uint32_t* __restrict__ dec_words, unsigned long long* __restrict__ acc_slots)
 {
-    extern __shared__ __align__(16) uint32_t smem_u32[];
     constexpr uint32_t kFull = 0xFFFFFFFFu;
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t wib = threadIdx.x >> 5;
@@ -409,26 +341,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const float half_k0 = kMove == 1 ? P.hk : 0.5f * P.k0;
     uint32_t n_acc = 0;
 
-    // window: omega of the group's box, per-axis LUTs, window plane of this lane's four monomers
-    const uint32_t wcells = kWin ? 1u << (W.sh[0] + W.sh[1] + W.sh[2]) : 0u;
-    float* om_w = reinterpret_cast<float*>(smem_u32);
-    uint32_t* lut = smem_u32 + n_types * wcells;
-    uint4 tw = make_uint4(0u, 0u, 0u, 0u);
-    if (kWin) {
-        tw.x = toff.x / P.g.cells * wcells; tw.y = toff.y / P.g.cells * wcells;
-        tw.z = toff.z / P.g.cells * wcells; tw.w = toff.w / P.g.cells * wcells;
-    }
-
-    const uint32_t n_groups = kWin ? W.n_groups : gridDim.x;
-    for (uint32_t grp = blockIdx.x; grp < n_groups; grp += gridDim.x) {
-    uint32_t t_begin, t_end;
-    if (kWin) {
-        t_begin = grp * W.tiles_per_group;
-        t_end = min(t_begin + W.tiles_per_group, n_tiles);
-    } else {
-        t_begin = (uint32_t)(((uint64_t)grp * n_tiles) / gridDim.x);
-        t_end = (uint32_t)(((uint64_t)(grp + 1u) * n_tiles) / gridDim.x);
-    }
+    const uint32_t t_begin = (uint32_t)(((uint64_t)blockIdx.x * n_tiles) / gridDim.x);
+    const uint32_t t_end = (uint32_t)(((uint64_t)(blockIdx.x + 1) * n_tiles) / gridDim.x);
     uint32_t tile = t_begin + wib;
     float4 X, Y, Z;
     uint32_t C = 0u;                                          // the caller's index of this lane's chain
@@ -438,41 +352,6 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         Y = *reinterpret_cast<const float4*>(y + i0);
         Z = *reinterpret_cast<const float4*>(z + i0);
         C = orig[i0 >> log2N];
-    }
-    if (kWin) {
-        __syncthreads();                                      // the previous group's window is no longer read
-        const int4 o = origin[grp];
-        const uint32_t g0 = P.g.n[0], g1 = P.g.n[1], g2 = P.g.n[2];
-        for (uint32_t i = threadIdx.x; i < g0 + g1 + g2; i += kFusedThreads) {
-            const uint32_t a = i < g0 ? 0u : (i < g0 + g1 ? 1u : 2u);
-            const uint32_t c = i - (a == 0u ? 0u : (a == 1u ? g0 : g0 + g1));
-            const uint32_t na = a == 0u ? g0 : (a == 1u ? g1 : g2);
-            const uint32_t oa = a == 0u ? (uint32_t)o.x : (a == 1u ? (uint32_t)o.y : (uint32_t)o.z);
-            const uint32_t d = c >= oa ? c - oa : c + na - oa;
-            const uint32_t stride_sh = a == 0u ? W.sh[1] + W.sh[2] : (a == 1u ? W.sh[2] : 0u);
-            lut[i] = d < (1u << W.sh[a]) ? d << stride_sh : kOutside;
-        }
-        // rows of the box along z are contiguous in omega: lane -> z offset, coalesced
-        const uint32_t dz = threadIdx.x & ((1u << W.sh[2]) - 1u), dy0 = threadIdx.x >> W.sh[2];
-        const uint32_t rows_per_pass = kFusedThreads >> W.sh[2];
-        const uint32_t ex = min(1u << W.sh[0], g0), ey = min(1u << W.sh[1], g1);
-        if (dz < g2) {
-            uint32_t cz = (uint32_t)o.z + dz;
-            cz = cz >= g2 ? cz - g2 : cz;
-            for (uint32_t dy = dy0; dy < ey; dy += rows_per_pass) {
-                uint32_t cy = (uint32_t)o.y + dy;
-                cy = cy >= g1 ? cy - g1 : cy;
-                const uint32_t row = cy * g2 + cz, slot_row = (dy << W.sh[2]) + dz;
-                uint32_t cx = (uint32_t)o.x;
-                for (uint32_t dx = 0; dx < ex; ++dx) {
-                    const uint32_t src = cx * g1 * g2 + row, dst = (dx << (W.sh[1] + W.sh[2])) + slot_row;
-                    for (uint32_t t = 0; t < n_types; ++t)
-                        om_w[t * wcells + dst] = __ldg(omega + t * P.g.cells + src);
-                    cx = cx + 1u == g0 ? 0u : cx + 1u;
-                }
-            }
-        }
-        __syncthreads();
     }
     for (; tile < t_end; tile += kWarps) {
         const uint32_t i0 = tile * kTile + 4u * lane;
@@ -497,12 +376,12 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
             const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
             const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
-            const CellRef o0 = locate<kWin>(P.g, lut, X.x, Y.x, Z.x, toff.x, tw.x), n0 = locate<kWin>(P.g, lut, x0n, y0n, z0n, toff.x, tw.x);
-            const CellRef o1 = locate<kWin>(P.g, lut, X.y, Y.y, Z.y, toff.y, tw.y), n1 = locate<kWin>(P.g, lut, x1n, y1n, z1n, toff.y, tw.y);
-            const CellRef o2 = locate<kWin>(P.g, lut, X.z, Y.z, Z.z, toff.z, tw.z), n2 = locate<kWin>(P.g, lut, x2n, y2n, z2n, toff.z, tw.z);
-            const CellRef o3 = locate<kWin>(P.g, lut, X.w, Y.w, Z.w, toff.w, tw.w), n3 = locate<kWin>(P.g, lut, x3n, y3n, z3n, toff.w, tw.w);
-            const float e0 = field_delta_ref<kWin>(omega, om_w, o0, n0), e1 = field_delta_ref<kWin>(omega, om_w, o1, n1),
-                        e2 = field_delta_ref<kWin>(omega, om_w, o2, n2), e3 = field_delta_ref<kWin>(omega, om_w, o3, n3);
+            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
+            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
+            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
+                        e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 
             // 4a. set 0: even monomers (slots 0, 2) see the old odd monomers
             float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
@@ -527,10 +406,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
             // 5. occupation numbers follow the accepted moves
             if (kIncr) {
-                count_follow(counts, a0, o0.idx, n0.idx);
-                count_follow(counts, a1, o1.idx, n1.idx);
-                count_follow(counts, a2, o2.idx, n2.idx);
-                count_follow(counts, a3, o3.idx, n3.idx);
+                count_follow(counts, a0, o0, n0);
+                count_follow(counts, a1, o1, n1);
+                count_follow(counts, a2, o2, n2);
+                count_follow(counts, a3, o3, n3);
             }
         } else {
             // Smart-MC: the proposal needs the bonded force, i.e. the neighbours as they are now
@@ -543,14 +422,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, 2.0f, sx2, sy2, sz2, q2, dx2, dy2, dz2, lr2);
             const float x0n = X.x + dx0, y0n = Y.x + dy0, z0n = Z.x + dz0;
             const float x2n = X.z + dx2, y2n = Y.z + dy2, z2n = Z.z + dz2;
-            const CellRef o0 = locate<kWin>(P.g, lut, X.x, Y.x, Z.x, toff.x, tw.x), n0 = locate<kWin>(P.g, lut, x0n, y0n, z0n, toff.x, tw.x);
-            const CellRef o2 = locate<kWin>(P.g, lut, X.z, Y.z, Z.z, toff.z, tw.z), n2 = locate<kWin>(P.g, lut, x2n, y2n, z2n, toff.z, tw.z);
-            const float e0 = field_delta_ref<kWin>(omega, om_w, o0, n0), e2 = field_delta_ref<kWin>(omega, om_w, o2, n2);
+            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
+            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const float e0 = field_delta(omega, o0, n0), e2 = field_delta(omega, o2, n2);
             a0 = metropolis((bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0) + e0) + lr0, q0.u);
             a2 = metropolis((bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2) + e2) + lr2, q2.u);
             X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
             X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
-            if (kIncr) { count_follow(counts, a0, o0.idx, n0.idx); count_follow(counts, a2, o2.idx, n2.idx); }
+            if (kIncr) { count_follow(counts, a0, o0, n0); count_follow(counts, a2, o2, n2); }
 
             float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
             xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
@@ -561,14 +440,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, mf3, sx3, sy3, sz3, q3, dx3, dy3, dz3, lr3);
             const float x1n = X.y + dx1, y1n = Y.y + dy1, z1n = Z.y + dz1;
             const float x3n = X.w + dx3, y3n = Y.w + dy3, z3n = Z.w + dz3;
-            const CellRef o1 = locate<kWin>(P.g, lut, X.y, Y.y, Z.y, toff.y, tw.y), n1 = locate<kWin>(P.g, lut, x1n, y1n, z1n, toff.y, tw.y);
-            const CellRef o3 = locate<kWin>(P.g, lut, X.w, Y.w, Z.w, toff.w, tw.w), n3 = locate<kWin>(P.g, lut, x3n, y3n, z3n, toff.w, tw.w);
-            const float e1 = field_delta_ref<kWin>(omega, om_w, o1, n1), e3 = field_delta_ref<kWin>(omega, om_w, o3, n3);
+            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
+            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const float e1 = field_delta(omega, o1, n1), e3 = field_delta(omega, o3, n3);
             a1 = metropolis((bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1) + e1) + lr1, q1.u);
             a3 = metropolis((bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3) + e3) + lr3, q3.u);
             X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
             X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
-            if (kIncr) { count_follow(counts, a1, o1.idx, n1.idx); count_follow(counts, a3, o3.idx, n3.idx); }
+            if (kIncr) { count_follow(counts, a1, o1, n1); count_follow(counts, a3, o3, n3); }
         }
 
         *reinterpret_cast<float4*>(x + i0) = X;
@@ -585,7 +464,6 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         }
         X = Xn; Y = Yn; Z = Zn; C = Cn;
     }
-    }   // groups
     n_acc = __reduce_add_sync(kFull, n_acc);
     if (lane == 0 && n_acc)
         atomicAdd(acc_slots + ((blockIdx.x * kWarps + wib) % kAccSlots), (unsigned long long)n_acc);

@@ -3,16 +3,15 @@
 // Nothing here is part of the method's arithmetic (PAPER.md has no counterpart): it only decides
 // WHERE a chain is stored.  A chain keeps its identity -- orig[slot] is the chain's index in the
 // caller's order, and that index (not the slot) enters the Philox counter and the decision bitmap --
-// so results do not depend on the layout.  Why a layout at all: the omega gathers and the count
-// updates of the move kernel are the kernel's L2-request bottleneck; with chains
-// ordered along a Hilbert curve through their centres of mass, a block's tiles live in a small
-// region of the grid, and that region's omega and count updates fit in shared memory.
+// so results do not depend on the layout.  Why a layout at all: with chains ordered along a Hilbert
+// curve through their centres of mass, the tiles a block works on live in a small region of the grid,
+// so the omega gathers and count updates of the move kernel hit in L1/L2 and touch fewer L2 slices
+// (~3 % faster at C3; chains diffuse ~R_e per 1e5 sweeps, so the order ages slowly).
 //
 //   chain_key_kernel      Hilbert index of the centre of mass of every chain
 //   (sort by key: cub::DeviceRadixSort in soma_b200.cu -- a library sort, off the hot path)
 //   permute_chains_kernel gather one coordinate array into the new order
 //   permute_ids_kernel    carry orig[] along
-//   group_origin_kernel   where to put the shared-memory window of each group of tiles
 //   import/export kernels caller order <-> device order for soma_set_positions / soma_positions
 #pragma once
 #include <cuda_runtime.h>
@@ -126,57 +125,6 @@ reorder_kernel(float* __restrict__ user, uint64_t user_stride, float* __restrict
         x[i] = user[g];
         y[i] = user[user_stride + g];
         z[i] = user[2 * user_stride + g];
-    }
-}
-
-// Window origin of every group of `chains_per_group` consecutive chain slots: the cell in the
-// middle of the range the chains' mean cells span (minimum image relative to the group's first
-// chain), minus half the window.  One block per group.  Purely a placement heuristic: beads that
-// fall outside the window take the global-memory path of the move kernel.
-__global__ void __launch_bounds__(128)
-group_origin_kernel(const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
-                    uint32_t n_chains, uint32_t N, uint32_t chains_per_group, float inv_Lx, float inv_Ly,
-                    float inv_Lz, int nx, int ny, int nz, int wx, int wy, int wz, int4* __restrict__ origin)
-{
-    __shared__ int s_ref[3], s_lo[3], s_hi[3];
-    const uint32_t first = blockIdx.x * chains_per_group;
-    const uint32_t last = min(first + chains_per_group, n_chains);
-    const int n[3] = {nx, ny, nz};
-    const float inv_L[3] = {inv_Lx, inv_Ly, inv_Lz};
-    auto mean_cell = [&](uint32_t c, int (&cell)[3]) {
-        const size_t b = (size_t)c * N;
-        float s[3] = {0.f, 0.f, 0.f};
-        for (uint32_t j = 0; j < N; ++j) { s[0] += x[b + j]; s[1] += y[b + j]; s[2] += z[b + j]; }
-        for (int a = 0; a < 3; ++a)
-            cell[a] = min((int)(box_fraction(s[a] / (float)N, inv_L[a]) * (float)n[a]), n[a] - 1);
-    };
-    if (threadIdx.x == 0) {
-        int c0[3];
-        mean_cell(first, c0);
-        for (int a = 0; a < 3; ++a) { s_ref[a] = c0[a]; s_lo[a] = 0; s_hi[a] = 0; }
-    }
-    __syncthreads();
-    for (uint32_t c = first + threadIdx.x; c < last; c += blockDim.x) {
-        int cell[3];
-        mean_cell(c, cell);
-        for (int a = 0; a < 3; ++a) {
-            int d = cell[a] - s_ref[a];
-            if (2 * d > n[a]) d -= n[a];
-            if (2 * d < -n[a]) d += n[a];
-            atomicMin(&s_lo[a], d);
-            atomicMax(&s_hi[a], d);
-        }
-    }
-    __syncthreads();
-    if (threadIdx.x == 0) {
-        const int w[3] = {wx, wy, wz};
-        int o[3];
-        for (int a = 0; a < 3; ++a) {
-            const int mid = s_ref[a] + (s_lo[a] + s_hi[a]) / 2;
-            o[a] = ((mid - w[a] / 2) % n[a] + n[a]) % n[a];
-            if (w[a] >= n[a]) o[a] = 0;              // the window holds the whole axis
-        }
-        origin[blockIdx.x] = make_int4(o[0], o[1], o[2], 0);
     }
 }
 

@@ -224,3 +224,60 @@ def test_device_buffers_and_timing_hooks():
     assert np.array_equal(xyz_d.cpu().numpy(), sim.positions())
     assert np.array_equal(om_d.cpu().numpy(), sim.fields()[0])
     sim.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# storage order of the chains (soma_layout.cuh): never visible in any result
+# ---------------------------------------------------------------------------------------------
+def _trajectory(w, xyz0, n_sweeps, layout, sort_interval, kernel=P.KERNEL_AUTO):
+    sim = P.from_workload(w, xyz0=xyz0)
+    sim.set_option(P.OPT_LAYOUT, layout)
+    sim.set_option(P.OPT_SORT_INTERVAL, sort_interval)
+    sim.set_option(P.OPT_KERNEL, kernel)
+    sim.set_option(P.OPT_RECORD_DECISIONS, 1)
+    out = []
+    for _ in range(n_sweeps):
+        sim.step(1)
+        om, cnt = sim.fields()
+        out.append((sim.positions().copy(), sim.decisions().copy(), om.copy(), cnt.copy()))
+    stats = sim.stats()
+    sim.destroy()
+    return out, stats
+
+
+@pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[7], workloads.small_cases()[3]],
+                         ids=lambda w: w.name)
+def test_hilbert_layout_and_resorting_leave_every_result_unchanged(w):
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    ref, st_ref = _trajectory(w, xyz0, 6, layout=0, sort_interval=0)
+    for layout, interval, kernel in [(1, 0, P.KERNEL_AUTO), (1, 2, P.KERNEL_AUTO), (1, 1, P.KERNEL_GENERIC)]:
+        got, st = _trajectory(w, xyz0, 6, layout, interval, kernel)
+        assert st == st_ref
+        for (p0, d0, o0, c0), (p1, d1, o1, c1) in zip(ref, got):
+            assert np.array_equal(p0, p1) and np.array_equal(d0, d1)
+            assert np.array_equal(c0, c1) and np.array_equal(o0, o1)
+
+
+def test_switching_the_layout_mid_run_and_device_side_import_export():
+    import torch
+    w = workloads.small_cases()[7]                      # blend: three architectures, ragged tiles
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    a = P.from_workload(w, xyz0=xyz0)
+    b = P.from_workload(w, xyz0=xyz0)
+    b.set_option(P.OPT_LAYOUT, 0)
+    assert np.array_equal(a.positions(), xyz0) and np.array_equal(b.positions(), xyz0)
+    a.step(2); b.step(2)
+    b.set_option(P.OPT_LAYOUT, 1)                       # caller's order -> Hilbert order
+    a.set_option(P.OPT_LAYOUT, 0)                       # and back
+    a.step(2); b.step(2)
+    assert np.array_equal(a.positions(), b.positions())
+    xyz_d = torch.empty((3, w.n_beads), dtype=torch.float32, device="cuda")
+    b.positions(xyz_d)                                  # device-side export through orig[]
+    b.sync()
+    assert np.array_equal(xyz_d.cpu().numpy(), a.positions())
+    a.set_positions(xyz_d)                              # device-side import
+    a.set_option(P.OPT_SWEEP_COUNTER, 4)
+    a.step(1); b.step(1)
+    assert np.array_equal(a.positions(), b.positions())
+    assert np.array_equal(a.fields()[1], b.fields()[1])
+    a.destroy(); b.destroy()
