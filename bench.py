@@ -35,6 +35,7 @@ METRIC = "attempted bead moves/s (full SCMF step)"
 UNIT = "moves/s"
 MOVE_BYTES_PER_BEAD = 24.0   # fused move kernel: read 12 B + write 12 B per bead per sweep
 FIELD_BYTES_PER_CELL = 16.0  # field kernel: read n_t counts + write n_t omegas (n_t = 2), DESIGN.md
+INSTR_PER_MOVE = 155.6       # SASS warp instructions per 32 local moves of the fused kernel (profiles/r01c_README.md)
 
 
 def peaks():
@@ -216,12 +217,24 @@ def main():
                                          "field": kms[P.K_FIELD] / max(1e-12, sum(kms))},
                 "full_step_frac": (MOVE_BYTES_PER_BEAD * nb + FIELD_BYTES_PER_CELL * w.n_cells) * args.steps
                                   / (ms_total * 1e-3) / 1e9 / peak}
+    # dram bytes per launch of the move kernel from the committed ncu --set full capture (profiles/r01c_README.md)
     traffic_file = ROOT / "profiles" / "traffic.json"
     if traffic_file.exists():
         try:
             roofline["traffic"] = json.loads(traffic_file.read_text()).get(w.name)
         except Exception:
             pass
+    # second roof: warp-instruction issue.  155.6 SASS warp instructions per 32 moves
+    # (ncu smsp__inst_executed.sum / launch), 4 schedulers per SM, one instruction per cycle each.
+    clocks_now = clk.summary()
+    if clocks_now.get("sm_mhz") and w.move == "local":
+        inst_per_launch = INSTR_PER_MOVE * nb / 32.0
+        peak_ips = 148 * 4 * clocks_now["sm_mhz"] * 1e6
+        roofline["issue"] = {"bound": "alu", "achieved": inst_per_launch / (move_ms * 1e-3) / 1e12,
+                             "peak": peak_ips / 1e12, "unit": "T warp-instr/s",
+                             "frac": inst_per_launch / (move_ms * 1e-3) / peak_ips,
+                             "instr_per_move": INSTR_PER_MOVE,
+                             "note": "issue slots of 148 SMs x 4 schedulers at the sampled SM clock; DESIGN.md 6.1"}
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------
     n_e2e = max(3, min(args.steps, 20))

@@ -669,8 +669,11 @@ int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
     if (!c || !xyz) return fail(SOMA_EINVAL, "soma_set_positions: NULL argument");
     int rc = copy_soa(c, nullptr, xyz, false, src_is_device != 0);
     if (rc) return rc;
-    rc = resort(c);
-    if (rc) return rc;
+    // The new positions keep the old storage order (usually they are a configuration this context
+    // exported); if they are unrelated the order is stale, which only costs cache hits: bring the
+    // next periodic re-sort forward to eight sweeps from now instead of sorting on every call.
+    if (c->layout && c->sort_interval > 8)
+        c->sweeps_since_sort = std::max<uint64_t>(c->sweeps_since_sort, (uint64_t)c->sort_interval - 8);
     rc = stage1(c);
     if (rc) return rc;
     if (!src_is_device) CU(cudaStreamSynchronize(c->stream));  // caller may reuse its buffer
