@@ -54,6 +54,8 @@ class _System(C.Structure):
         ("seed", C.c_uint64),
         ("hamiltonian", C.c_int32),
         ("smc_step", C.c_float),
+        ("set_order", C.c_int32),
+        ("field_every", C.c_uint32),
     ]
 
 
@@ -92,6 +94,8 @@ def lib():
         L.soma_oracle_smc_delta.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, C.c_int,
                                             C.c_uint32, fp, fp, fp, fp, fp]
         L.soma_oracle_smc_delta.restype = None
+        L.soma_oracle_first_set.argtypes = [sysp, C.c_uint64, C.c_uint64]
+        L.soma_oracle_first_set.restype = C.c_uint32
         L.soma_oracle_sweep.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, u8p]
         L.soma_oracle_sweep.restype = C.c_uint64
         L.soma_oracle_step.argtypes = [sysp, fp, fp, fp, u32p, fp, C.c_uint64, C.c_uint32, C.c_int, u8p]
@@ -170,6 +174,8 @@ class OracleSystem:
     seed: int = 0
     hamiltonian: int = 0
     smc_step: float = 0.0
+    set_order: int = 0          # 0: even set then odd set; 1: random order per chain and sweep
+    field_every: int = 1        # fields refreshed after every field_every-th sweep
     _keep: list = field(default_factory=list, repr=False)
 
     def __post_init__(self):
@@ -205,6 +211,8 @@ class OracleSystem:
         s.seed = int(self.seed)
         s.hamiltonian = int(self.hamiltonian)
         s.smc_step = float(self.smc_step)
+        s.set_order = int(self.set_order)
+        s.field_every = int(self.field_every)
 
     # -- sizes -------------------------------------------------------------------------------
     @property
@@ -268,6 +276,10 @@ class OracleSystem:
         lib().soma_oracle_smc_delta(self.ref, _fp(x), _fp(y), _fp(z), _fp(omega), bead, int(has_l),
                                     int(has_r), type_, _fp(g), _fp(d), C.byref(dE), C.byref(lr), _fp(rn))
         return d, float(dE.value), float(lr.value), rn
+
+    def first_set(self, first_bead: int, sweep: int) -> int:
+        """Which set of the chain that starts at ``first_bead`` moves first in ``sweep`` (0 even, 1 odd)."""
+        return int(lib().soma_oracle_first_set(self.ref, first_bead, sweep))
 
     def sweep(self, x, y, z, omega, sweep: int, move_kind: int = MOVE_LOCAL,
               decisions: Optional[np.ndarray] = None) -> int:

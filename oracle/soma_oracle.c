@@ -57,6 +57,9 @@ typedef struct {
     uint64_t        seed;
     int32_t         hamiltonian;   /* 0: K^0_inter (Eq. 7), 1: K^1_inter (Eq. 8)                 */
     float           smc_step;      /* Smart-MC step a_s in R_e0^2                                */
+    int32_t         set_order;     /* 0: sets in the order even, odd (R11); 1: random order per   */
+                                   /*    molecule and sweep (Code 2; R21)        */
+    uint32_t        field_every;   /* omega refreshed after every field_every-th sweep (R22); 0, 1: every sweep */
 } oracle_system;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -373,11 +376,25 @@ static int mc_smc(const oracle_system *s, float *x, float *y, float *z, const fl
     return 1;
 }
 
+/* "Generate random permutation of the sets" (Code 2; "a pre-defined random order",
+ * PAPER.md:294).  A linear chain has two sets, so the permutation is one fair bit per molecule and
+ * sweep.  Reading R21: bit 31 of word 0 of Philox(counter = (global index of the molecule's first
+ * bead, sweep lo32, sweep hi32, kind 3 << 8)); it names the set that goes first (0 even, 1 odd).
+ * The bit does not depend on the configuration, so global balance holds. */
+uint32_t soma_oracle_first_set(const oracle_system *s, uint64_t first_bead, uint64_t sweep)
+{
+    if (s->set_order == 0) return 0u;
+    uint32_t w[4];
+    draw(s, first_bead, sweep, 3u, 0u, w);
+    return w[0] >> 31;
+}
+
 /* ------------------------------------------------------------------------------------------ */
 /* Stage 2: one MC sweep, omega frozen.  Code 2: parallel loop over           */
 /* molecules; inside a molecule the independent sets one after the other; for a linear chain the */
 /* sets are the even and the odd monomers (Fig. 1).  Reading R11: the set order is */
-/* even, then odd, every sweep.  decisions (nullable): one byte per bead, 1 = accepted.          */
+/* even, then odd, every sweep, unless set_order = 1 (soma_oracle_first_set).                    */
+/* decisions (nullable): one byte per bead, 1 = accepted.                                        */
 /* move_kind: 1 = local displacement, 2 = Smart-MC.  Returns the number of accepted moves.       */
 /* ------------------------------------------------------------------------------------------ */
 uint64_t soma_oracle_sweep(const oracle_system *s, float *x, float *y, float *z, const float *omega,
@@ -394,8 +411,10 @@ uint64_t soma_oracle_sweep(const oracle_system *s, float *x, float *y, float *z,
 #endif
         for (int64_t mol = 0; mol < n_mol; ++mol) {
             const uint64_t first = spec_first_bead + (uint64_t)mol * N;
-            for (uint32_t i_set = 0; i_set < 2; ++i_set) {      /* sets in fixed order (R11) */
-                for (uint32_t ip = i_set; ip < N; ip += 2) {     /* members of the set         */
+            const uint32_t first_set = soma_oracle_first_set(s, first, sweep);
+            for (uint32_t k_set = 0; k_set < 2; ++k_set) {      /* the two sets, one after the other */
+                const uint32_t i_set = k_set ^ first_set;       /* set_permutation[k_set]            */
+                for (uint32_t ip = i_set; ip < N; ip += 2) {     /* members of the set                */
                     const uint64_t bead = first + ip;
                     const int has_l = ip > 0, has_r = ip + 1 < N;
                     const int acc = move_kind == 2
@@ -422,7 +441,10 @@ uint64_t soma_oracle_step(const oracle_system *s, float *x, float *y, float *z, 
     for (uint32_t i = 0; i < n_sweeps; ++i) {
         accepted += soma_oracle_sweep(s, x, y, z, omega, sweep0 + i, move_kind, decisions);
         soma_oracle_histogram(s, x, y, z, counts);
-        soma_oracle_fields(s, counts, omega);
+        /* Reading R22: with field_every = k > 1 the fields are the "frequently updated" ones of
+         * PAPER.md:200 refreshed only after sweeps number k, 2k, ... (counted from 1) */
+        if (s->field_every <= 1 || (sweep0 + i + 1) % s->field_every == 0)
+            soma_oracle_fields(s, counts, omega);
     }
     return accepted;
 }

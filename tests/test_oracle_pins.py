@@ -569,3 +569,112 @@ def test_init_positions_statistics():
     # reproducible from (seed, bead index) alone
     x2, _, _ = s.init_positions()
     assert np.array_equal(x, x2)
+
+
+# ----------------------------------------------------------------------------------------------
+# P12  random order of the independent sets (Code 2) and field interval
+# ----------------------------------------------------------------------------------------------
+def test_first_set_is_the_documented_philox_bit_and_fair():
+    """Reading R21: bit 31 of word 0 of Philox(counter = (first bead, sweep lo, sweep hi, 3 << 8)).
+    Philox itself is pinned by P1, so this pins counter layout, kind and bit; fixed order gives 0."""
+    seed = 0xDEADBEEF12345678
+    s = OracleSystem(specs=[(4, np.zeros(4, np.uint8))], N_ref=4, n_types=1, box=(1.0,) * 3, grid=(2, 2, 2),
+                     seed=seed, set_order=1)
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    for bead, sweep in [(0, 0), (4, 0), (8, 7), (123456, 2**32 + 5), (2**32 - 4, 2**40 + 1)]:
+        w = oracle.philox4x32_10((bead, sweep & 0xFFFFFFFF, sweep >> 32, 3 << 8), key)
+        assert s.first_set(bead, sweep) == w[0] >> 31
+    bits = np.array([[s.first_set(4 * c, sw) for c in range(4000)] for sw in range(4)])
+    assert abs(bits.mean() - 0.5) < 4 * 0.5 / math.sqrt(bits.size)          # fair
+    assert abs(np.corrcoef(bits[0], bits[1])[0, 1]) < 4 / math.sqrt(4000)      # fresh every sweep
+    assert abs(np.corrcoef(bits[0][:-1], bits[0][1:])[0, 1]) < 4 / math.sqrt(4000)   # and per chain
+    s.set_order = 0
+    assert all(s.first_set(4 * c, 3) == 0 for c in range(50))
+
+
+def test_sweep_with_random_set_order_replayed_by_brute_force():
+    """Replay of a sweep with set_order = 1, chain by chain, in the order first_set() names (pinned
+    above), with float64 brute-force energies: the set that goes second sees the moved beads of the
+    set that went first, whichever that was."""
+    specs = [(4, np.array([0, 0, 1, 1, 1], np.uint8)), (3, np.array([0, 1] * 4, np.uint8))]
+    box, grid = (2.0, 2.0, 2.0), (4, 4, 4)
+    s, chains, pos, omega = _tiny_system(21, specs, 8, box, grid, A=0.3, set_order=1)
+    types = s.bead_types()
+    k0 = 3.0 * (s.N_ref - 1)
+    seen = set()
+    compared = 0
+    for sweep in range(8):
+        x, y, z = (np.ascontiguousarray(pos[:, a]) for a in range(3))
+        dec = np.zeros(len(pos), np.uint8)
+        s.sweep(x, y, z, omega, sweep, MOVE_LOCAL, dec)
+        ref = pos.copy()
+        ref_dec = np.zeros(len(pos), np.uint8)
+        fragile = False
+        for first, N in chains:
+            bit = s.first_set(first, sweep)
+            seen.add(bit)
+            for parity in (bit, 1 - bit):
+                for j in range(parity, N, 2):
+                    g = first + j
+                    d, u = s.local_proposal(g, sweep)
+                    rn = ref[g] + d
+                    p64 = ref.astype(np.float64)
+                    H0 = _total_H(p64, chains, types, omega, k0, box, grid)
+                    p64[g] = rn
+                    dE = _total_H(p64, chains, types, omega, k0, box, grid) - H0
+                    thr = math.exp(-dE) if dE > 0 else 2.0
+                    if abs(u - thr) < 1e-5 or abs(dE) < 1e-6:
+                        fragile = True
+                    if dE <= 0 or u < thr:
+                        ref[g] = rn
+                        ref_dec[g] = 1
+        if not fragile:
+            compared += 1
+            assert np.array_equal(dec, ref_dec)
+            assert np.array_equal(np.stack([x, y, z], 1), ref)
+        pos = np.stack([x, y, z], 1)
+    assert seen == {0, 1} and compared >= 3
+
+
+def test_random_set_order_keeps_ideal_chains_in_equilibrium():
+    """Global balance: the sequence of moves does not depend on the configuration, so
+    stretched chains still relax to <b^2> = 1/(N-1), <Re^2> = 1 with a random set order."""
+    n, N = 12000, 8
+    s = OracleSystem(specs=[(n, np.zeros(N, np.uint8))], N_ref=N, n_types=1, box=(8.0,) * 3, grid=(8, 8, 8),
+                     A=0.2, seed=77, set_order=1)
+    rng = np.random.default_rng(6)
+    steps = rng.standard_normal((n, N, 3)) * 1.6 / math.sqrt(3 * (N - 1))
+    steps[:, 0] = rng.random((n, 3)) * 8
+    P = np.cumsum(steps, 1).reshape(-1, 3)
+    x, y, z = (np.ascontiguousarray(P[:, a], dtype=np.float32) for a in range(3))
+    omega = np.zeros((1, s.n_cells), np.float32)
+    for sweep in range(400):
+        s.sweep(x, y, z, omega, sweep, MOVE_LOCAL)
+    b, re2, _ = _chain_stats(x, y, z, n, N)
+    b2 = (b**2).sum(-1)
+    assert abs(b2.mean() * (N - 1) - 1) < 0.012
+    assert abs(re2.mean() - 1.0) < 5 * math.sqrt(2 / 3 / n)
+
+
+def test_field_interval_refreshes_omega_after_every_kth_sweep():
+    """Reading R22: step() with field_every = 3 is sweep + histogram every sweep, fields after sweeps
+    3, 6, ... only -- composed here from the separately pinned pieces."""
+    kw = dict(specs=[(200, np.array([0] * 4 + [1] * 4, np.uint8))], N_ref=8, n_types=2, box=(2.0,) * 3,
+              grid=(4, 4, 4), chiN=15.0, kappaN=30.0, A=0.2, seed=3)
+    rng = np.random.default_rng(8)
+    P = np.cumsum(rng.standard_normal((200, 8, 3)) * 0.2 + (rng.random((200, 1, 3)) * 2) * (np.arange(8)[None, :, None] == 0), 1)
+    xyz = [np.ascontiguousarray(P.reshape(-1, 3)[:, a], dtype=np.float32) for a in range(3)]
+    a = OracleSystem(field_every=3, **kw)
+    xa = [v.copy() for v in xyz]
+    ca = a.histogram(*xa)
+    oa = a.fields(ca)
+    a.step(*xa, ca, oa, 0, 7)
+    b = OracleSystem(**kw)
+    xb = [v.copy() for v in xyz]
+    ob = b.fields(b.histogram(*xb))
+    for sweep in range(7):
+        b.sweep(*xb, ob, sweep)
+        if (sweep + 1) % 3 == 0:
+            ob = b.fields(b.histogram(*xb))
+    assert all(np.array_equal(u, v) for u, v in zip(xa, xb))
+    assert np.array_equal(oa, ob) and np.array_equal(ca, b.histogram(*xb))
