@@ -64,7 +64,13 @@ enum {
     SOMA_OPT_LAYOUT = 11,          /* 0: chains stay in the caller's order in device memory; 1 (default): the  */
                                    /* library keeps them in Hilbert order of their centres of mass.  Storage   */
                                    /* only: every result is identical, every API array is in the caller's order */
-    SOMA_OPT_SORT_INTERVAL = 12    /* re-sort every this many sweeps (default 2000; 0: only at init/set_positions) */
+    SOMA_OPT_SORT_INTERVAL = 12,   /* re-sort every this many sweeps (default 2000; 0: only at init/set_positions) */
+    SOMA_OPT_SET_ORDER = 13,       /* 0 (default): even monomers, then odd monomers, every sweep; 1: the order */
+                                   /* of the two sets is drawn per chain and sweep ("random permutation of the */
+                                   /* sets", Code 2): Philox kind 3, counter word 0 = global */
+                                   /* index of the chain's first bead, bit 31 of word 0, 1 = odd set first     */
+    SOMA_OPT_FIELD_INTERVAL = 14   /* k >= 1 (default 1): omega is refreshed after sweeps number k, 2k, ...    */
+                                   /* (counted from 1); the occupation numbers are current after every sweep   */
 };
 
 /* indices of soma_kernel_times */

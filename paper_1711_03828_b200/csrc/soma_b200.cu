@@ -95,6 +95,8 @@ struct soma_ctx {
     size_t cub_tmp_bytes = 0;
     uint64_t n_chains_total = 0, max_chains = 0;
     int layout = 1;                  // 0: caller's order, 1: Hilbert order
+    int set_order = 0;               // 0: even set then odd set; 1: random per chain and sweep (R21)
+    int field_interval = 1;          // omega refreshed after every field_interval-th sweep (R22)
     int sort_interval = 2000;        // sweeps between re-sorts (0: only at init / set_positions)
     uint64_t sweeps_since_sort = 0;
 
@@ -225,14 +227,15 @@ struct Timed {
 bool spec_uses_fused(const soma_ctx* c, const Spec& s)
 {
     if (c->kernel_choice == 1) return false;
+    if (c->move == 2 && c->set_order == 1) return false;   // Smart-MC in random set order: generic kernel only
     if (!s.fused_ok) return false;
     return true;
 }
 
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kOrder>
 int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
-    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord>;
+    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
     int per_sm = c->blocks_per_sm;
     if (per_sm <= 0) {   // auto: every block resident, one wave
@@ -258,21 +261,22 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
         if (spec_uses_fused(c, s) && s.n_tiles > 0) {
-            int rc = launch_fused<kMove, kIncr, kRecord>(c, P, s);
+            int rc = (kMove == 1 && c->set_order == 1) ? launch_fused<kMove, kIncr, kRecord, kMove == 1>(c, P, s)
+                                                       : launch_fused<kMove, kIncr, kRecord, false>(c, P, s);
             if (rc) return rc;
             done = (uint64_t)s.n_tiles * soma::kTile;
         }
         if (done < s.n_beads) {   // whole chains the fused kernel does not cover (all of them, or a ragged tail)
             const uint64_t n_chains = (s.n_beads - done) / s.N;
             for (uint32_t parity = 0; parity < 2; ++parity) {
-                const uint32_t half = parity == 0 ? (s.N + 1) / 2 : s.N / 2;
-                if (half == 0) continue;
+                const uint32_t half = (s.N + 1) / 2;
                 const uint64_t n_items = n_chains * half;
                 const int threads = 256;
                 const uint64_t blocks = (n_items + threads - 1) / threads;
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::generic_move_kernel<kMove, kIncr, kRecord><<<(unsigned)blocks, threads, 0, c->stream>>>(
-                    P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity, n_items,
+                    P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity,
+                    (uint32_t)c->set_order, n_items,
                     (uint32_t)s.gid0, c->orig + s.chain_off + done / s.N, c->decisions, c->acc_slots);
             }
         }
@@ -634,8 +638,10 @@ int soma_step(soma_ctx* c, int n_sweeps)
             rc = launch_histogram(c);                      // a3 from scratch
             if (rc) return rc;
         }
-        rc = launch_fields(c);                             // a4
-        if (rc) return rc;
+        if (c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
+            rc = launch_fields(c);                         // a4
+            if (rc) return rc;
+        }
         c->sweep += 1;
         c->attempted += c->n_beads;
         c->decisions_valid = c->record != 0;
@@ -754,6 +760,16 @@ int soma_set_option(soma_ctx* c, int key, double value)
             c->layout = 0;
             return copy_soa(c, nullptr, c->stage, false, true);
         }
+        case SOMA_OPT_SET_ORDER:
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_SET_ORDER: 0 (even, odd) or 1 (random per chain and sweep)");
+            if (iv == 1 && c->kernel_choice == 2 && c->move == 2)
+                return fail(SOMA_EINVAL, "SOMA_OPT_SET_ORDER=1 with Smart-MC needs the generic kernel (SOMA_OPT_KERNEL 0 or 1)");
+            c->set_order = iv;
+            return SOMA_OK;
+        case SOMA_OPT_FIELD_INTERVAL:
+            if (iv < 1) return fail(SOMA_EINVAL, "SOMA_OPT_FIELD_INTERVAL: must be >= 1");
+            c->field_interval = iv;
+            return SOMA_OK;
         case SOMA_OPT_SORT_INTERVAL:
             if (iv < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SORT_INTERVAL: must be >= 0");
             c->sort_interval = iv;

@@ -116,6 +116,18 @@ __device__ __forceinline__ void philox4x32_10_head(uint32_t gid, const uint32_t 
     out[0] = a; out[1] = b; out[2] = c; out[3] = d;
 }
 
+// "Generate random permutation of the sets" (Code 2): a linear chain has two sets, so
+// the permutation is one bit per chain and sweep, bit 31 of word 0 of the Philox call with counter
+// (global index of the chain's first bead, sweep, kind 3) -- DESIGN.md reading R21.  0: the even
+// monomers move first, 1: the odd ones.
+__device__ __forceinline__ uint32_t first_set_bit(uint32_t first_gid, uint32_t sweep_lo, uint32_t sweep_hi,
+                                                  uint32_t key0, uint32_t key1)
+{
+    uint32_t w[4];
+    philox4x32_10(first_gid, sweep_lo, sweep_hi, 0x300u, key0, key1, w);
+    return w[0] >> 31;
+}
+
 // top 23 bits -> float in [1, 2), exact
 __device__ __forceinline__ float u23(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
 
@@ -321,7 +333,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 //   orig        [n_chains] the caller's chain index of the chain in each slot (Philox counter, bitmap)
 //   dec_words   decision bitmap (whole system), or unused
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kOrder>
 __global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -383,26 +395,57 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
                         e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 
-            // 4a. set 0: even monomers (slots 0, 2) see the old odd monomers
-            float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
-            xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
-            float sx, sy, sz;
-            bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
-            a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
-            bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
-            a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
-            X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
-            X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
+            if (!kOrder) {
+                // 4a. set 0: even monomers (slots 0, 2) see the old odd monomers
+                float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+                xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+                float sx, sy, sz;
+                bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
+                a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
+                bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
+                a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
+                X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
+                X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
 
-            // 4b. set 1: odd monomers (slots 1, 3) see the moved even monomers
-            float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
-            xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
-            bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
-            a1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, q1.u);
-            bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
-            a3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, q3.u);
-            X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
-            X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
+                // 4b. set 1: odd monomers (slots 1, 3) see the moved even monomers
+                float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+                xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+                bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
+                a1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, q1.u);
+                bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
+                a3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, q3.u);
+                X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
+                X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
+            } else {
+                // 4'. random set order (SOMA_OPT_SET_ORDER = 1): the chain's bit says which set moves
+                // first.  Lanes of one warp hold different chains, so every slot is evaluated in both
+                // phases and takes part in the one its parity is due in.
+                const uint32_t bit = first_set_bit(gid0 + (C << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]);
+                a0 = a1 = a2 = a3 = false;
+#pragma unroll
+                for (uint32_t phase = 0; phase < 2u; ++phase) {
+                    const bool odd_now = (phase ^ bit) != 0u, even_now = !odd_now;
+                    float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+                    float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+                    xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+                    xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+                    float sx, sy, sz;
+                    bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
+                    const bool b0 = even_now && metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
+                    bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
+                    const bool b2 = even_now && metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
+                    bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
+                    const bool b1 = odd_now && metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, q1.u);
+                    bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
+                    const bool b3 = odd_now && metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, q3.u);
+                    // members of one set are not bonded to each other: all four updates at once
+                    X.x = b0 ? x0n : X.x; Y.x = b0 ? y0n : Y.x; Z.x = b0 ? z0n : Z.x;
+                    X.y = b1 ? x1n : X.y; Y.y = b1 ? y1n : Y.y; Z.y = b1 ? z1n : Z.y;
+                    X.z = b2 ? x2n : X.z; Y.z = b2 ? y2n : Y.z; Z.z = b2 ? z2n : Z.z;
+                    X.w = b3 ? x3n : X.w; Y.w = b3 ? y3n : Y.w; Z.w = b3 ? z3n : Z.w;
+                    a0 = a0 || b0; a1 = a1 || b1; a2 = a2 || b2; a3 = a3 || b3;
+                }
+            }
 
             // 5. occupation numbers follow the accepted moves
             if (kIncr) {
@@ -472,21 +515,28 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 // ------------------------------------------------------------------------------------------------
 // a1 or a2 for any chain length: one thread per monomer of parity `parity` (set 0 / set 1).  The
 // other parity is not written during this launch, so neighbours can be read from global memory.
-//   half  = monomers of this parity per chain; n_items = n_chains * half
+//   half  = ceil(N / 2) threads per chain; n_items = n_chains * half; parity = 0, 1: first, second set
+//   set_order  0: the first set is the even monomers; 1: the chain's first_set_bit decides
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord>
 __global__ void __launch_bounds__(256)
 generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                     const float* __restrict__ omega, uint32_t* __restrict__ counts,
                     const uint32_t* __restrict__ toff_tab, uint32_t N, uint32_t half, uint32_t parity,
-                    uint64_t n_items, uint32_t gid0, const uint32_t* __restrict__ orig,
+                    uint32_t set_order, uint64_t n_items, uint32_t gid0, const uint32_t* __restrict__ orig,
                     uint32_t* __restrict__ dec_words, unsigned long long* __restrict__ acc_slots)
 {
     const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
     bool acc = false;
+    uint64_t chain = 0;
+    uint32_t j = N;
     if (t < n_items) {
-        const uint64_t chain = t / half;
-        const uint32_t j = 2u * (uint32_t)(t - chain * half) + parity;
+        chain = t / half;
+        uint32_t set = parity;       // launch 0 moves the first set of every chain, launch 1 the second
+        if (set_order) set ^= first_set_bit(gid0 + orig[chain] * N, P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]);
+        j = 2u * (uint32_t)(t - chain * half) + set;
+    }
+    if (j < N) {                     // half = ceil(N / 2): the odd set of an odd-length chain has one member fewer
         const uint64_t i = chain * N + j;
         const bool has_l = j > 0u, has_r = j + 1u < N;
         float px = x[i], py = y[i], pz = z[i];

@@ -33,11 +33,13 @@ def field_close(w, got, want):
 
 
 def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INCREMENTAL,
-             hamiltonian=0, check_every=1, expect_flips=0.0):
+             hamiltonian=0, check_every=1, expect_flips=0.0, set_order=0, field_every=1):
     if xyz0 is None:
         xyz0 = np.stack(workloads.gaussian_walks(w))
     sim = P.from_workload(w, xyz0=xyz0)
-    orc = oracle_system(w, hamiltonian=hamiltonian)
+    orc = oracle_system(w, hamiltonian=hamiltonian, set_order=set_order)
+    sim.set_option(P.OPT_SET_ORDER, set_order)
+    sim.set_option(P.OPT_FIELD_INTERVAL, field_every)
     sim.set_option(P.OPT_KERNEL, kernel)
     sim.set_option(P.OPT_DENSITY, density)
     sim.set_option(P.OPT_HAMILTONIAN, hamiltonian)
@@ -53,7 +55,8 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
         cnt_o = orc.histogram(x, y, z)
         assert np.array_equal(cnt_g, cnt_o), f"sweep {sweep}: occupation numbers differ"
         assert cnt_g.sum() == nb
-        om_o = orc.fields(cnt_o)
+        if sweep % field_every == 0:            # refreshed after sweeps number k, 2k, ... and at init (R22)
+            om_o = orc.fields(cnt_o)
         assert field_close(w, om_g, om_o) <= FIELD_RTOL, f"sweep {sweep}: fields differ"
         dec_o = np.zeros(nb, np.uint8)
         acc_o = orc.sweep(x, y, z, om_o, sweep, move, dec_o)
@@ -149,6 +152,40 @@ def test_smart_mc_literal_step_of_c5():
     w = workloads.Workload("smc_literal", ((600, workloads.diblock(64, 19)), (300, workloads.homopolymer(16))), 64, 2,
                            (3.0, 3.0, 3.0), (15, 15, 15), 35.0, 50.0, 0.1, 7, move="smc", smc_step=0.05)
     lockstep(w, 3)
+
+
+# ---------------------------------------------------------------------------------------------
+# random order of the two sets per chain and sweep (Code 2); field interval
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC])
+@pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[2], workloads.small_cases()[3],
+                               workloads.small_cases()[7]], ids=lambda w: w.name)
+def test_random_set_order(w, kernel):
+    lockstep(w, 5, kernel=kernel, set_order=1)
+
+
+def test_random_set_order_smart_mc_runs_in_the_generic_kernel():
+    w = workloads.Workload("smc_order", ((300, workloads.diblock(64, 19)), (150, workloads.homopolymer(16))), 64, 2,
+                           (3.0, 3.0, 3.0), (15, 15, 15), 35.0, 50.0, 0.1, 7, move="smc", smc_step=0.05 / 63)
+    lockstep(w, 3, set_order=1)
+
+
+def test_random_set_order_differs_from_fixed_order_and_ragged_tiles():
+    w = workloads.Workload("ragged_order", ((2051, workloads.diblock(32, 16)), (7, workloads.diblock(64, 19)),
+                                            (3, workloads.homopolymer(4)), (11, workloads.homopolymer(9, 1))),
+                           32, 2, (4.0, 4.0, 4.0), (16, 16, 16), 20.0, 50.0, 0.1, 11)
+    lockstep(w, 3, set_order=1)
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    a, b = P.from_workload(w, xyz0=xyz0), P.from_workload(w, xyz0=xyz0)
+    b.set_option(P.OPT_SET_ORDER, 1)
+    a.step(1); b.step(1)
+    assert not np.array_equal(a.positions(), b.positions())
+    a.destroy(); b.destroy()
+
+
+@pytest.mark.parametrize("density", [P.DENSITY_INCREMENTAL, P.DENSITY_FULL])
+def test_field_interval(density):
+    lockstep(workloads.c1(), 7, density=density, field_every=3)
 
 
 # ---------------------------------------------------------------------------------------------
