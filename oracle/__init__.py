@@ -56,6 +56,8 @@ class _System(C.Structure):
         ("smc_step", C.c_float),
         ("set_order", C.c_int32),
         ("field_every", C.c_uint32),
+        ("ext_field", C.POINTER(C.c_float)),
+        ("forbidden", C.POINTER(C.c_uint8)),
     ]
 
 
@@ -176,6 +178,8 @@ class OracleSystem:
     smc_step: float = 0.0
     set_order: int = 0          # 0: even set then odd set; 1: random order per chain and sweep
     field_every: int = 1        # fields refreshed after every field_every-th sweep
+    ext_field: Optional[np.ndarray] = None    # (n_types, n_cells) float32 static field added to omega
+    forbidden: Optional[np.ndarray] = None    # (n_cells,) uint8, 1 = no particle may enter the cell
     _keep: list = field(default_factory=list, repr=False)
 
     def __post_init__(self):
@@ -213,6 +217,16 @@ class OracleSystem:
         s.smc_step = float(self.smc_step)
         s.set_order = int(self.set_order)
         s.field_every = int(self.field_every)
+        if self.ext_field is not None:
+            self._ext = np.ascontiguousarray(self.ext_field, dtype=np.float32).reshape(self.n_types, -1)
+            s.ext_field = self._ext.ctypes.data_as(C.POINTER(C.c_float))
+        else:
+            s.ext_field = C.POINTER(C.c_float)()
+        if self.forbidden is not None:
+            self._forb = np.ascontiguousarray(self.forbidden, dtype=np.uint8).reshape(-1)
+            s.forbidden = self._forb.ctypes.data_as(C.POINTER(C.c_uint8))
+        else:
+            s.forbidden = C.POINTER(C.c_uint8)()
 
     # -- sizes -------------------------------------------------------------------------------
     @property

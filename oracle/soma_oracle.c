@@ -60,6 +60,8 @@ typedef struct {
     int32_t         set_order;     /* 0: sets in the order even, odd (R11); 1: random order per   */
                                    /*    molecule and sweep (Code 2; R21)        */
     uint32_t        field_every;   /* omega refreshed after every field_every-th sweep (R22); 0, 1: every sweep */
+    const float    *ext_field;     /* nullable, [n_types][cells]: static external field added to omega   */
+    const uint8_t  *forbidden;     /* nullable, [cells]: 1 = no particle may enter this cell             */
 } oracle_system;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -182,11 +184,20 @@ void soma_oracle_histogram(const oracle_system *s, const float *x, const float *
 /* chi_0 = chiN / N_ref, kappa_0 = kappaN / N_ref.  Reading R9: each unordered    */
 /* pair once in Eq. 7-8, so Eq. 12 holds as printed.  omega[type][cell], fp32.                   */
 /* ------------------------------------------------------------------------------------------ */
+/* External fields, reading R23.  "The second specifies a linear attraction for the */
+/* particle of a specific type": a static, type-specific field ext_i(c) added to omega_i(c).  "The   */
+/* first prevents any particle from entering a specific grid cell": omega_i(c) = +infinity for every */
+/* type in such a cell, so Eq. 15 gives dE_nb = +inf for a move into it and the Metropolis rule       */
+/* rejects it (a bead that starts inside may leave: dE_nb = -inf).  The mean occupancy rho_0 DeltaL^3 */
+/* of PAPER.md:125, 241 then refers to the accessible volume: beads / (cells - forbidden cells).      */
 void soma_oracle_fields(const oracle_system *s, const uint32_t *counts, float *omega)
 {
     const int64_t cells = n_cells(s);
     const uint32_t nt = s->n_types;
-    const float inv_nbar = (float)((double)cells / (double)soma_oracle_n_beads(s));
+    int64_t allowed = cells;
+    if (s->forbidden)
+        for (int64_t c = 0; c < cells; ++c) allowed -= s->forbidden[c] ? 1 : 0;
+    const float inv_nbar = (float)((double)allowed / (double)soma_oracle_n_beads(s));
     const float kappa0 = (float)((double)s->kappaN / (double)s->N_ref);
     float chi0[ORACLE_MAX_TYPES][ORACLE_MAX_TYPES], half_chi0[ORACLE_MAX_TYPES][ORACLE_MAX_TYPES];
     for (uint32_t i = 0; i < nt; ++i)
@@ -209,6 +220,8 @@ void soma_oracle_fields(const oracle_system *s, const uint32_t *counts, float *o
                 else
                     w = w + chi0[i][k] * phi[k];                 /* Eq. 12, K^1 line */
             }
+            if (s->ext_field) w = w + s->ext_field[(int64_t)i * cells + c];
+            if (s->forbidden && s->forbidden[c]) w = INFINITY;
             omega[(int64_t)i * cells + c] = w;
         }
     }

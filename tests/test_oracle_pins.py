@@ -678,3 +678,57 @@ def test_field_interval_refreshes_omega_after_every_kth_sweep():
             ob = b.fields(b.histogram(*xb))
     assert all(np.array_equal(u, v) for u, v in zip(xa, xb))
     assert np.array_equal(oa, ob) and np.array_equal(ca, b.histogram(*xb))
+
+
+# ----------------------------------------------------------------------------------------------
+# P13  external fields: forbidden cells and a type-specific static field
+# ----------------------------------------------------------------------------------------------
+def test_external_field_hand_values():
+    """omega = Eq. 12 + ext; forbidden cells are +inf for every type; phi is normalised with the
+    accessible volume, so a melt that fills the allowed half of a box uniformly has omega = ext."""
+    grid = (2, 2, 2)
+    forb = np.array([1, 0, 1, 0, 1, 0, 1, 0], np.uint8)                    # every cell with iz = 0
+    ext = np.arange(16, dtype=np.float32).reshape(2, 8) * 0.25
+    s = OracleSystem(specs=[(8, np.array([0, 0, 1, 1], np.uint8))], N_ref=4, n_types=2, box=(1.0,) * 3, grid=grid,
+                     chiN=12.0, kappaN=40.0, ext_field=ext, forbidden=forb)
+    counts = np.zeros((2, 8), np.uint32)
+    counts[:, forb == 0] = 4                                               # 32 beads over 4 allowed cells
+    om = s.fields(counts)
+    assert np.all(np.isposinf(om[:, forb == 1]))
+    assert np.allclose(om[:, forb == 0], ext[:, forb == 0], atol=1e-6)      # phi_A = phi_B = 1/2: Eq. 12 gives 0
+    s2 = OracleSystem(specs=[(8, np.array([0, 0, 1, 1], np.uint8))], N_ref=4, n_types=2, box=(1.0,) * 3, grid=grid,
+                      chiN=12.0, kappaN=40.0)
+    counts2 = np.full((2, 8), 2, np.uint32)
+    assert np.allclose(s2.fields(counts2), 0.0, atol=1e-6)                   # same melt without walls
+    s3 = OracleSystem(specs=[(8, np.array([0, 0, 1, 1], np.uint8))], N_ref=4, n_types=2, box=(1.0,) * 3, grid=grid,
+                      chiN=12.0, kappaN=40.0, ext_field=ext)
+    assert np.allclose(s3.fields(counts2), ext, atol=1e-6)
+
+
+def test_confined_free_beads_stay_out_of_forbidden_cells_and_follow_the_external_field():
+    """Free beads (N = 1, chi = kappa = 0) in a slit: walls = the two outer z layers, a two-level
+    attraction inside.  Through step() (fields refreshed every sweep): no bead ever enters a wall
+    cell, and the occupation ratio of the two levels is exp(-delta) (Boltzmann)."""
+    n, grid, box = 20000, (4, 4, 8), (2.0, 2.0, 4.0)
+    cells = 4 * 4 * 8
+    iz = np.arange(cells) % 8
+    forb = ((iz == 0) | (iz == 7)).astype(np.uint8)
+    delta = 0.7
+    ext = np.where((iz == 1) | (iz == 6), -delta, 0.0).astype(np.float32)[None, :]   # attraction next to the walls
+    s = OracleSystem(specs=[(n, np.zeros(1, np.uint8))], N_ref=1, n_types=1, box=box, grid=grid, A=0.4, seed=17,
+                     ext_field=ext, forbidden=forb)
+    rng = np.random.default_rng(9)
+    x = (rng.random(n) * 2).astype(np.float32); y = (rng.random(n) * 2).astype(np.float32)
+    z = (0.5 + rng.random(n) * 3.0).astype(np.float32)                       # inside the slit
+    counts = s.histogram(x, y, z)
+    omega = s.fields(counts)
+    occ_lo = occ_hi = 0
+    for block in range(30):
+        s.step(x, y, z, counts, omega, 10 * block, 10)
+        assert counts[0, forb == 1].sum() == 0
+        if block >= 5:
+            occ_lo += int(counts[0, (iz == 1) | (iz == 6)].sum())
+            occ_hi += int(counts[0, (iz >= 2) & (iz <= 5)].sum())
+    # 2 attractive layers vs 4 neutral layers: ratio of per-cell occupations = exp(delta)
+    ratio = (occ_lo / 2) / (occ_hi / 4)
+    assert abs(ratio / math.exp(delta) - 1) < 0.03
