@@ -122,6 +122,15 @@ int soma_set_positions(soma_ctx *ctx, const float *xyz, int src_is_device);
 /* Set chi_ij N = chi_ji N for one type pair (i != j) and refresh omega. */
 int soma_set_chi(soma_ctx *ctx, int i, int j, float chiN_ij);
 
+/* External fields.  ext_field: float32 [n_types][cells], a static field added to
+ * omega_i(c) ("a linear attraction for the particle of a specific type"), or NULL for none.
+ * forbidden: uint8 [cells], non-zero = no particle may enter that cell ("geometric confinements"), or
+ * NULL for none: omega is +inf there for every type, so every move into such a cell is rejected, and
+ * phi_i is normalised with the accessible volume, rho_0 DeltaL^3 = beads / (cells - forbidden cells).
+ * Beads that already sit in a forbidden cell are not moved out by this call (they may leave, never
+ * return).  Both arrays are copied; omega is refreshed.  SOMA_EINVAL if every cell is forbidden. */
+int soma_set_external(soma_ctx *ctx, const float *ext_field, const uint8_t *forbidden, int src_is_device);
+
 int soma_set_option(soma_ctx *ctx, int key, double value);
 
 /* attempted / accepted moves since soma_init and the current sweep counter (synchronises). */

@@ -25,7 +25,7 @@ K_MOVE, K_DENSITY, K_FIELD, K_LAYOUT, K_COUNT = 0, 1, 2, 3, 4
 # every symbol include/soma_b200.h declares (tests check that the library exports all of them)
 SYMBOLS = (
     "soma_init", "soma_step", "soma_fields", "soma_positions", "soma_set_positions", "soma_set_chi",
-    "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
+    "soma_set_external", "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
     "soma_version",
 )
@@ -59,6 +59,7 @@ def load() -> C.CDLL:
     L.soma_positions.argtypes = [vp, vp, i32]
     L.soma_set_positions.argtypes = [vp, vp, i32]
     L.soma_set_chi.argtypes = [vp, i32, i32, C.c_float]
+    L.soma_set_external.argtypes = [vp, vp, vp, i32]
     L.soma_set_option.argtypes = [vp, i32, C.c_double]
     L.soma_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.POINTER(u64)]
     L.soma_decisions.argtypes = [vp, vp, i32]
@@ -157,6 +158,14 @@ class Soma:
 
     def set_chi(self, i: int, j: int, chiN: float) -> None:
         _check(self._L.soma_set_chi(self._h, i, j, C.c_float(chiN)))
+
+    def set_external(self, ext_field=None, forbidden=None) -> None:
+        """ext_field: float32 (n_types, n_cells) or None; forbidden: uint8 (n_cells,) or None."""
+        pe, de = _ptr(ext_field) if ext_field is not None else (None, None)
+        pf, df = _ptr(forbidden) if forbidden is not None else (None, None)
+        assert de is None or df is None or de == df
+        dev = de if de is not None else df
+        _check(self._L.soma_set_external(self._h, C.c_void_p(pe), C.c_void_p(pf), int(bool(dev))))
 
     def set_option(self, key: int, value: float) -> None:
         _check(self._L.soma_set_option(self._h, int(key), C.c_double(value)))

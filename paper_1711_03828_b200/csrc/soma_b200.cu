@@ -81,6 +81,9 @@ struct soma_ctx {
     uint32_t* counts = nullptr;
     float* omega = nullptr;
     uint32_t* toff = nullptr;
+    float* ext = nullptr;            // [n_types][cells] static external field, or null
+    uint8_t* forbidden = nullptr;    // [cells] 1 = no particle may enter, or null
+    uint64_t n_forbidden = 0;
     uint32_t* decisions = nullptr;
     unsigned long long* acc_slots = nullptr;
     unsigned long long* acc_host = nullptr;  // pinned staging for soma_stats
@@ -170,7 +173,7 @@ soma::MoveP soma_ctx::movep(uint64_t sweep_no) const
 soma::FieldP soma_ctx::fieldp() const
 {
     soma::FieldP f;
-    f.inv_nbar = (float)((double)cells / (double)n_beads);
+    f.inv_nbar = (float)((double)(cells - n_forbidden) / (double)n_beads);   // accessible volume (R23)
     f.kappa0 = (float)((double)kappaN / (double)N_ref);
     for (int i = 0; i < soma::kMaxTypes; ++i)
         for (int k = 0; k < soma::kMaxTypes; ++k) {
@@ -328,9 +331,9 @@ int launch_fields(soma_ctx* c)
     const unsigned blocks = (unsigned)((c->cells + threads - 1) / threads);
     Timed t(c, SOMA_K_FIELD, 1);
     switch (c->n_types) {
-        case 1: soma::field_kernel<1><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
-        case 2: soma::field_kernel<2><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
-        default: soma::field_kernel<0><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega); break;
+        case 1: soma::field_kernel<1><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega, c->ext, c->forbidden); break;
+        case 2: soma::field_kernel<2><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega, c->ext, c->forbidden); break;
+        default: soma::field_kernel<0><<<blocks, threads, 0, c->stream>>>(F, c->counts, c->omega, c->ext, c->forbidden); break;
     }
     CU(cudaGetLastError());
     return SOMA_OK;
@@ -429,6 +432,7 @@ void soma_destroy(soma_ctx* c)
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
+    cudaFree(c->ext); cudaFree(c->forbidden);
     cudaFree(c->acc_slots);
     cudaFree(c->orig); cudaFree(c->orig_tmp); cudaFree(c->scratch); cudaFree(c->stage);
     cudaFree(c->sort_keys[0]); cudaFree(c->sort_keys[1]); cudaFree(c->sort_vals[0]); cudaFree(c->sort_vals[1]);
@@ -693,6 +697,45 @@ int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
         return fail(SOMA_EINVAL, "soma_set_chi: need 0 <= i != j < n_types and a finite value");
     c->chiN[i][j] = c->chiN[j][i] = chiN_ij;
     return launch_fields(c);
+}
+
+int soma_set_external(soma_ctx* c, const float* ext_field, const uint8_t* forbidden, int src_is_device)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_set_external: ctx is NULL");
+    const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+    const size_t n = (size_t)c->cells * c->n_types;
+    if (ext_field) {
+        if (!c->ext) CU(cudaMalloc(&c->ext, sizeof(float) * n));
+        CU(cudaMemcpyAsync(c->ext, ext_field, sizeof(float) * n, kind, c->stream));
+    } else if (c->ext) {
+        CU(cudaStreamSynchronize(c->stream));
+        CU(cudaFree(c->ext));
+        c->ext = nullptr;
+    }
+    c->n_forbidden = 0;
+    if (forbidden) {
+        if (!c->forbidden) CU(cudaMalloc(&c->forbidden, c->cells));
+        CU(cudaMemcpyAsync(c->forbidden, forbidden, c->cells, kind, c->stream));
+        // the accessible volume normalises phi: count the forbidden cells on the host (one byte per cell)
+        std::vector<uint8_t> h(c->cells);
+        CU(cudaMemcpyAsync(h.data(), c->forbidden, c->cells, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        for (uint8_t v : h) c->n_forbidden += v ? 1 : 0;
+        if (c->n_forbidden >= c->cells) {
+            c->n_forbidden = 0;
+            CU(cudaFree(c->forbidden));
+            c->forbidden = nullptr;
+            return fail(SOMA_EINVAL, "soma_set_external: every cell is forbidden");
+        }
+    } else if (c->forbidden) {
+        CU(cudaStreamSynchronize(c->stream));
+        CU(cudaFree(c->forbidden));
+        c->forbidden = nullptr;
+    }
+    int rc = launch_fields(c);
+    if (rc) return rc;
+    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));   // the caller may reuse its buffers
+    return SOMA_OK;
 }
 
 int soma_set_option(soma_ctx* c, int key, double value)

@@ -572,10 +572,13 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
 // a4  omega_i(c) from n_i(c), Eq. 12: phi_i = n_i / (rho_0 DeltaL^3),
 //     K^0: omega_i = kappa_0 (sum phi - 1) - sum_{k != i} chi_0ik/2 (phi_i - phi_k)
 //     K^1: omega_i = kappa_0 (sum phi - 1) + sum_{k != i} chi_0ik phi_k
+//     + ext_i(c) if an external field is set; +inf in forbidden cells, so that Eq. 15 makes every move
+//     into such a cell cost +inf and the Metropolis rule rejects it (R23)
 // ------------------------------------------------------------------------------------------------
 template <int kTypes>
 __global__ void __launch_bounds__(256)
-field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega)
+field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
+             const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
 {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= F.cells) return;
@@ -601,6 +604,9 @@ field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restr
             else
                 w = w + F.chi0[i][k] * phi[k];
         }
+        // external fields: a static type-specific field; +inf where no particle may enter
+        if (ext) w = w + ext[(size_t)i * F.cells + c];
+        if (forbidden && forbidden[c]) w = __int_as_float(0x7F800000);
         omega[(size_t)i * F.cells + c] = w;
     }
 }

@@ -28,16 +28,23 @@ POS_TOL_SMC = 1e-6         # R_e
 
 def field_close(w, got, want):
     # reading R16: relative to max(|omega|, kappa_0 + chi_0) so that omega ~ 0 cells are well-defined
+    inf = np.isinf(want)
+    if not np.array_equal(inf, np.isinf(got)) or not np.array_equal(got[inf], want[inf]):
+        return float("inf")                      # forbidden cells: +inf on both sides, nowhere else
+    got, want = got[~inf], want[~inf]
     scale = np.maximum(np.abs(want), (w.kappaN + abs(w.chiN)) / w.N_ref + 1e-30)
     return float(np.max(np.abs(got.astype(np.float64) - want) / scale))
 
 
 def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INCREMENTAL,
-             hamiltonian=0, check_every=1, expect_flips=0.0, set_order=0, field_every=1):
+             hamiltonian=0, check_every=1, expect_flips=0.0, set_order=0, field_every=1, ext_field=None,
+             forbidden=None):
     if xyz0 is None:
         xyz0 = np.stack(workloads.gaussian_walks(w))
     sim = P.from_workload(w, xyz0=xyz0)
-    orc = oracle_system(w, hamiltonian=hamiltonian, set_order=set_order)
+    orc = oracle_system(w, hamiltonian=hamiltonian, set_order=set_order, ext_field=ext_field, forbidden=forbidden)
+    if ext_field is not None or forbidden is not None:
+        sim.set_external(ext_field, forbidden)
     sim.set_option(P.OPT_SET_ORDER, set_order)
     sim.set_option(P.OPT_FIELD_INTERVAL, field_every)
     sim.set_option(P.OPT_KERNEL, kernel)
@@ -186,6 +193,53 @@ def test_random_set_order_differs_from_fixed_order_and_ragged_tiles():
 @pytest.mark.parametrize("density", [P.DENSITY_INCREMENTAL, P.DENSITY_FULL])
 def test_field_interval(density):
     lockstep(workloads.c1(), 7, density=density, field_every=3)
+
+
+# ---------------------------------------------------------------------------------------------
+# external fields: a thin film between two walls with a type-selective attraction
+# ---------------------------------------------------------------------------------------------
+def _thin_film():
+    w = workloads.Workload("film", ((3000, workloads.diblock(32, 16)), (41, workloads.homopolymer(5))), 32, 2,
+                           (4.0, 4.0, 2.0), (16, 16, 10), 20.0, 50.0, 0.1, 13)
+    x, y, z = workloads.gaussian_walks(w)
+    lay = workloads  # noqa: F841
+    # squeeze every chain into the slit 0.3 < z < 1.7 (walls: the outer z layers, 0.2 thick each)
+    g = 0
+    for n, t in w.specs:
+        N = len(t)
+        zz = z[g:g + n * N].reshape(n, N)
+        zz[:] = 1.0 + 0.25 * (zz - zz.mean(1, keepdims=True))
+        g += n * N
+    iz = np.arange(w.n_cells) % 10
+    forbidden = ((iz == 0) | (iz == 9)).astype(np.uint8)
+    ext = np.zeros((2, w.n_cells), np.float32)
+    ext[0, (iz == 1) | (iz == 8)] = -0.5            # the walls attract A
+    ext[1, (iz == 1) | (iz == 8)] = +0.25           # and repel B
+    return w, np.stack([x, y, z]).astype(np.float32), ext, forbidden
+
+
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC])
+def test_thin_film_with_walls_and_selective_attraction(kernel):
+    w, xyz0, ext, forbidden = _thin_film()
+    assert oracle_system(w).histogram(*[xyz0[a].copy() for a in range(3)])[:, forbidden == 1].sum() == 0
+    lockstep(w, 6, xyz0=xyz0, kernel=kernel, ext_field=ext, forbidden=forbidden)
+
+
+def test_walls_hold_and_external_fields_can_be_removed():
+    w, xyz0, ext, forbidden = _thin_film()
+    sim = P.from_workload(w, xyz0=xyz0)
+    sim.set_external(ext, forbidden)
+    sim.step(200)
+    om, cnt = sim.fields()
+    assert cnt[:, forbidden == 1].sum() == 0 and np.all(np.isposinf(om[:, forbidden == 1]))
+    assert np.all(np.isfinite(om[:, forbidden == 0]))
+    sim.set_external(None, None)
+    om2, _ = sim.fields()
+    orc = oracle_system(w)
+    assert field_close(w, om2, orc.fields(cnt)) <= FIELD_RTOL
+    with pytest.raises(P.SomaError):
+        sim.set_external(None, np.ones(w.n_cells, np.uint8))
+    sim.destroy()
 
 
 # ---------------------------------------------------------------------------------------------
