@@ -56,6 +56,7 @@ class _System(C.Structure):
         ("smc_step", C.c_float),
         ("set_order", C.c_int32),
         ("field_every", C.c_uint32),
+        ("scheme", C.c_int32),
         ("ext_field", C.POINTER(C.c_float)),
         ("forbidden", C.POINTER(C.c_uint8)),
     ]
@@ -100,6 +101,10 @@ def lib():
         L.soma_oracle_first_set.restype = C.c_uint32
         L.soma_oracle_sweep.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, u8p]
         L.soma_oracle_sweep.restype = C.c_uint64
+        L.soma_oracle_pick.argtypes = [sysp, C.c_uint64, C.c_uint64, C.c_uint32]
+        L.soma_oracle_pick.restype = C.c_uint32
+        L.soma_oracle_sweep_molecules.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, u8p]
+        L.soma_oracle_sweep_molecules.restype = C.c_uint64
         L.soma_oracle_step.argtypes = [sysp, fp, fp, fp, u32p, fp, C.c_uint64, C.c_uint32, C.c_int, u8p]
         L.soma_oracle_step.restype = C.c_uint64
         L.soma_oracle_init_positions.argtypes = [sysp, fp, fp, fp]
@@ -178,6 +183,7 @@ class OracleSystem:
     smc_step: float = 0.0
     set_order: int = 0          # 0: even set then odd set; 1: random order per chain and sweep
     field_every: int = 1        # fields refreshed after every field_every-th sweep
+    scheme: int = 0             # 0: independent sets (Code 2); 1: molecule-parallel random picks (Code 1)
     ext_field: Optional[np.ndarray] = None    # (n_types, n_cells) float32 static field added to omega
     forbidden: Optional[np.ndarray] = None    # (n_cells,) uint8, 1 = no particle may enter the cell
     _keep: list = field(default_factory=list, repr=False)
@@ -217,6 +223,7 @@ class OracleSystem:
         s.smc_step = float(self.smc_step)
         s.set_order = int(self.set_order)
         s.field_every = int(self.field_every)
+        s.scheme = int(self.scheme)
         if self.ext_field is not None:
             self._ext = np.ascontiguousarray(self.ext_field, dtype=np.float32).reshape(self.n_types, -1)
             s.ext_field = self._ext.ctypes.data_as(C.POINTER(C.c_float))
@@ -300,6 +307,16 @@ class OracleSystem:
         """One MC sweep in place (omega frozen). Returns the number of accepted moves."""
         return int(lib().soma_oracle_sweep(self.ref, _fp(x), _fp(y), _fp(z), _fp(omega), sweep,
                                            move_kind, _u8p(decisions)))
+
+    def pick(self, attempt_id: int, sweep: int, N: int) -> int:
+        """Particle chosen by attempt ``attempt_id`` (= first bead + k) of a chain of N beads (Code 1)."""
+        return int(lib().soma_oracle_pick(self.ref, attempt_id, sweep, N))
+
+    def sweep_molecules(self, x, y, z, omega, sweep: int, move_kind: int = MOVE_LOCAL,
+                        decisions: Optional[np.ndarray] = None) -> int:
+        """One sweep of the molecule-parallel scheme (Code 1) in place. decisions: one byte per attempt."""
+        return int(lib().soma_oracle_sweep_molecules(self.ref, _fp(x), _fp(y), _fp(z), _fp(omega), sweep,
+                                                     move_kind, _u8p(decisions)))
 
     def step(self, x, y, z, counts, omega, sweep0: int, n_sweeps: int, move_kind: int = MOVE_LOCAL,
              decisions: Optional[np.ndarray] = None) -> int:

@@ -60,6 +60,8 @@ typedef struct {
     int32_t         set_order;     /* 0: sets in the order even, odd (R11); 1: random order per   */
                                    /*    molecule and sweep (Code 2; R21)        */
     uint32_t        field_every;   /* omega refreshed after every field_every-th sweep (R22); 0, 1: every sweep */
+    int32_t         scheme;        /* 0: independent sets (Code 2); 1: molecule-parallel, N random picks */
+                                   /*    per molecule and sweep (Code 1; R24)           */
     const float    *ext_field;     /* nullable, [n_types][cells]: static external field added to omega   */
     const uint8_t  *forbidden;     /* nullable, [cells]: 1 = no particle may enter this cell             */
 } oracle_system;
@@ -444,6 +446,55 @@ uint64_t soma_oracle_sweep(const oracle_system *s, float *x, float *y, float *z,
     return accepted;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* Stage 2, first scheme of the paper (Code 1): molecules in parallel; inside a  */
+/* molecule "sequentially choosing a particle of this molecule at random for a MC move", N times, */
+/* so that "on average, each particle of the molecules is attempted to be moved once during a MC  */
+/* step".  Reading R24: attempt k = 0..N-1 of the molecule whose first bead has global index f    */
+/* owns the Philox counter word f + k (unique per sweep); the particle is                          */
+/* i = floor(w0 N / 2^32) with w0 = word 0 of the call of kind 4, and the move itself (local or    */
+/* Smart-MC) takes its random numbers from the calls of kind 1 / 2 with that same counter word.    */
+/* decisions[f + k] = outcome of attempt k.                                                        */
+/* ------------------------------------------------------------------------------------------ */
+uint32_t soma_oracle_pick(const oracle_system *s, uint64_t attempt_id, uint64_t sweep, uint32_t N)
+{
+    uint32_t w[4];
+    draw(s, attempt_id, sweep, 4u, 0u, w);
+    return (uint32_t)(((uint64_t)w[0] * (uint64_t)N) >> 32);
+}
+
+uint64_t soma_oracle_sweep_molecules(const oracle_system *s, float *x, float *y, float *z,
+                                     const float *omega, uint64_t sweep, int move_kind, uint8_t *decisions)
+{
+    uint64_t accepted = 0;
+    uint64_t spec_first_bead = 0;
+    const uint8_t *types = s->types;
+    for (uint32_t a = 0; a < s->n_specs; ++a) {
+        const uint32_t N = s->spec_n_beads[a];
+        const int64_t n_mol = (int64_t)s->spec_n_chains[a];
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : accepted)
+#endif
+        for (int64_t mol = 0; mol < n_mol; ++mol) {
+            const uint64_t first = spec_first_bead + (uint64_t)mol * N;
+            for (uint32_t mono = 0; mono < N; ++mono) {          /* sequential iteration of particles */
+                const uint64_t attempt = first + mono;
+                const uint32_t ip = soma_oracle_pick(s, attempt, sweep, N);   /* select random particle */
+                const uint64_t bead = first + ip;
+                const int has_l = ip > 0, has_r = ip + 1 < N;
+                const int acc = move_kind == 2
+                    ? mc_smc(s, x, y, z, omega, bead, attempt, has_l, has_r, types[ip], sweep)
+                    : mc_local(s, x, y, z, omega, bead, attempt, has_l, has_r, types[ip], sweep);
+                accepted += (uint64_t)acc;
+                if (decisions) decisions[attempt] = (uint8_t)acc;
+            }
+        }
+        spec_first_bead += (uint64_t)n_mol * N;
+        types += N;
+    }
+    return accepted;
+}
+
 /* One SCMF cycle as soma_step runs it: sweep with the current omega, then stage 1 for the new
  * configuration (fields refreshed "after each MC step"; reading R12). */
 uint64_t soma_oracle_step(const oracle_system *s, float *x, float *y, float *z, uint32_t *counts,
@@ -452,7 +503,9 @@ uint64_t soma_oracle_step(const oracle_system *s, float *x, float *y, float *z, 
 {
     uint64_t accepted = 0;
     for (uint32_t i = 0; i < n_sweeps; ++i) {
-        accepted += soma_oracle_sweep(s, x, y, z, omega, sweep0 + i, move_kind, decisions);
+        accepted += s->scheme == 1
+            ? soma_oracle_sweep_molecules(s, x, y, z, omega, sweep0 + i, move_kind, decisions)
+            : soma_oracle_sweep(s, x, y, z, omega, sweep0 + i, move_kind, decisions);
         soma_oracle_histogram(s, x, y, z, counts);
         /* Reading R22: with field_every = k > 1 the fields are the "frequently updated" ones of
          * PAPER.md:200 refreshed only after sweeps number k, 2k, ... (counted from 1) */

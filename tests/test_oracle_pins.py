@@ -732,3 +732,84 @@ def test_confined_free_beads_stay_out_of_forbidden_cells_and_follow_the_external
     # 2 attractive layers vs 4 neutral layers: ratio of per-cell occupations = exp(delta)
     ratio = (occ_lo / 2) / (occ_hi / 4)
     assert abs(ratio / math.exp(delta) - 1) < 0.03
+
+
+# ----------------------------------------------------------------------------------------------
+# P14  molecule-parallel scheme: N random picks per molecule and sweep (Code 1)
+# ----------------------------------------------------------------------------------------------
+def test_pick_is_the_documented_philox_word_and_uniform():
+    """Reading R24: i = floor(w0 N / 2^32), w0 = word 0 of Philox(counter = (attempt id, sweep, kind 4));
+    uniform over 0..N-1, so "on average each particle is attempted once per MC step"."""
+    seed = 0x0123456789ABCDEF
+    s = OracleSystem(specs=[(4, np.zeros(5, np.uint8))], N_ref=5, n_types=1, box=(1.0,) * 3, grid=(2, 2, 2), seed=seed)
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    for attempt, sweep, N in [(0, 0, 5), (7, 3, 32), (2**32 - 1, 2**33 + 9, 100), (12345, 1, 1)]:
+        w = oracle.philox4x32_10((attempt, sweep & 0xFFFFFFFF, sweep >> 32, 4 << 8), key)
+        assert s.pick(attempt, sweep, N) == (w[0] * N) >> 32 < N
+    N, n = 7, 70000
+    picks = np.array([s.pick(a, 5, N) for a in range(n)])
+    hist = np.bincount(picks, minlength=N)
+    assert hist.min() > 0 and np.all(np.abs(hist - n / N) < 4.5 * math.sqrt(n / N))
+    assert abs(np.corrcoef(picks[:-1], picks[1:])[0, 1]) < 4 / math.sqrt(n)
+
+
+def test_molecule_sweep_replayed_by_brute_force():
+    """Replay of Code 1 attempt by attempt with float64 brute-force energies: the k-th attempt of a
+    chain moves the particle pick() names with the random numbers of counter word first + k, and sees
+    every earlier accepted move of its chain (also of the same particle picked twice)."""
+    specs = [(4, np.array([0, 0, 1, 1, 1], np.uint8)), (3, np.array([0, 1] * 4, np.uint8))]
+    box, grid = (2.0, 2.0, 2.0), (4, 4, 4)
+    s, chains, pos, omega = _tiny_system(31, specs, 8, box, grid, A=0.3)
+    types = s.bead_types()
+    k0 = 3.0 * (s.N_ref - 1)
+    compared, repeats = 0, 0
+    for sweep in range(8):
+        x, y, z = (np.ascontiguousarray(pos[:, a]) for a in range(3))
+        dec = np.zeros(len(pos), np.uint8)
+        acc = s.sweep_molecules(x, y, z, omega, sweep, MOVE_LOCAL, dec)
+        ref = pos.copy()
+        ref_dec = np.zeros(len(pos), np.uint8)
+        fragile = False
+        for first, N in chains:
+            picked = [s.pick(first + k, sweep, N) for k in range(N)]
+            repeats += N - len(set(picked))
+            for k, i in enumerate(picked):
+                g = first + i
+                d, u = s.local_proposal(first + k, sweep)
+                rn = ref[g] + d
+                p64 = ref.astype(np.float64)
+                H0 = _total_H(p64, chains, types, omega, k0, box, grid)
+                p64[g] = rn
+                dE = _total_H(p64, chains, types, omega, k0, box, grid) - H0
+                thr = math.exp(-dE) if dE > 0 else 2.0
+                if abs(u - thr) < 1e-5 or abs(dE) < 1e-6:
+                    fragile = True
+                if dE <= 0 or u < thr:
+                    ref[g] = rn
+                    ref_dec[first + k] = 1
+        if not fragile:
+            compared += 1
+            assert np.array_equal(dec, ref_dec) and acc == int(ref_dec.sum())
+            assert np.array_equal(np.stack([x, y, z], 1), ref)
+        pos = np.stack([x, y, z], 1)
+    assert compared >= 3 and repeats > 0
+
+
+def test_molecule_scheme_relaxes_ideal_chains():
+    """Each single move satisfies detailed balance and the pick does not depend on the configuration,
+    so stretched ideal chains relax to <b^2> = 1/(N-1), <Re^2> = 1 under Code 1 as under Code 2."""
+    n, N = 12000, 8
+    s = OracleSystem(specs=[(n, np.zeros(N, np.uint8))], N_ref=N, n_types=1, box=(8.0,) * 3, grid=(8, 8, 8),
+                     A=0.2, seed=78, scheme=1)
+    rng = np.random.default_rng(7)
+    steps = rng.standard_normal((n, N, 3)) * 1.6 / math.sqrt(3 * (N - 1))
+    steps[:, 0] = rng.random((n, 3)) * 8
+    P = np.cumsum(steps, 1).reshape(-1, 3)
+    x, y, z = (np.ascontiguousarray(P[:, a], dtype=np.float32) for a in range(3))
+    counts = s.histogram(x, y, z)
+    omega = s.fields(counts)                      # chi = kappa = 0: identically zero
+    s.step(x, y, z, counts, omega, 0, 600)        # step() dispatches on scheme
+    b, re2, _ = _chain_stats(x, y, z, n, N)
+    b2 = (b**2).sum(-1)
+    assert abs(b2.mean() * (N - 1) - 1) < 0.012
+    assert abs(re2.mean() - 1.0) < 5 * math.sqrt(2 / 3 / n)
