@@ -98,6 +98,7 @@ struct soma_ctx {
     size_t cub_tmp_bytes = 0;
     uint64_t n_chains_total = 0, max_chains = 0;
     int layout = 1;                  // 0: caller's order, 1: Hilbert order
+    int scheme = 0;                  // 0: independent sets (Code 2); 1: molecule-parallel random picks (Code 1, R24)
     int set_order = 0;               // 0: even set then odd set; 1: random per chain and sweep (R21)
     int field_interval = 1;          // omega refreshed after every field_interval-th sweep (R22)
     int sort_interval = 2000;        // sweeps between re-sorts (0: only at init / set_positions)
@@ -260,6 +261,16 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
 {
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
+        if (c->scheme == 1) {   // Code 1: one thread per molecule
+            const int threads = 128;
+            const unsigned blocks = (unsigned)((s.n_chains + threads - 1) / threads);
+            Timed t(c, SOMA_K_MOVE, 1);
+            soma::molecule_move_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
+                P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N,
+                s.n_chains, (uint32_t)s.gid0, c->orig + s.chain_off, c->decisions, c->acc_slots);
+            CU(cudaGetLastError());
+            continue;
+        }
         float *x = c->x + s.off, *y = c->y + s.off, *z = c->z + s.off;
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
@@ -803,6 +814,10 @@ int soma_set_option(soma_ctx* c, int key, double value)
             c->layout = 0;
             return copy_soa(c, nullptr, c->stage, false, true);
         }
+        case SOMA_OPT_SCHEME:
+            if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_SCHEME: 0 (independent sets) or 1 (molecule-parallel)");
+            c->scheme = iv;
+            return SOMA_OK;
         case SOMA_OPT_SET_ORDER:
             if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_SET_ORDER: 0 (even, odd) or 1 (random per chain and sweep)");
             if (iv == 1 && c->kernel_choice == 2 && c->move == 2)

@@ -6,6 +6,7 @@
 //                         (independent sets of Fig. 1 / Code 2), neighbours by
 //                         warp shuffle, each position read and written once per sweep.
 //   generic_move_kernel   a1 or a2 for any chain length: one thread per monomer of one parity.
+//   molecule_move_kernel  the paper's other scheme (Code 1): one thread per molecule, N random picks
 //   histogram_kernel      a3  n_i(c), Eq. 4
 //   field_kernel          a4  omega_i(c), Eq. 12
 //   init_walk_kernel      Gaussian-walk start state (BASELINE.json configs)
@@ -551,6 +552,52 @@ generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y,
     const uint32_t n_acc = __popc(__ballot_sync(0xFFFFFFFFu, acc));
     if ((threadIdx.x & 31u) == 0 && n_acc)
         atomicAdd(acc_slots + ((t >> 5) % kAccSlots), (unsigned long long)n_acc);
+}
+
+// ------------------------------------------------------------------------------------------------
+// Molecule-parallel scheme (Code 1): one thread per molecule, which N times picks
+// one of its particles at random and attempts to move it; attempts of one molecule are sequential
+// (a particle picked twice, or a neighbour moved earlier, is seen in its new place), molecules are
+// independent while omega is frozen.  Attempt k of the chain whose first bead has global index f owns
+// the Philox counter word f + k: kind 4 picks the particle, i = floor(w0 N / 2^32); kind 1 / 2 gives
+// the move's random numbers (R24).  The chain's 3 N floats are touched N times by the same
+// thread, so they stay in L1; lanes of a warp work on 32 consecutive chains.
+//   dec_words   bit of attempt f + k (not of a bead), or unused
+// ------------------------------------------------------------------------------------------------
+template <int kMove, bool kIncr, bool kRecord>
+__global__ void __launch_bounds__(128)
+molecule_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+                     const float* __restrict__ omega, uint32_t* __restrict__ counts,
+                     const uint32_t* __restrict__ toff_tab, uint32_t N, uint64_t n_chains, uint32_t gid0,
+                     const uint32_t* __restrict__ orig, uint32_t* __restrict__ dec_words,
+                     unsigned long long* __restrict__ acc_slots)
+{
+    const uint64_t chain = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t n_acc = 0;
+    if (chain < n_chains) {
+        const uint64_t base = chain * N;
+        const uint32_t first = gid0 + orig[chain] * N;
+        for (uint32_t k = 0; k < N; ++k) {                    // "sequential iteration of particles"
+            const uint32_t attempt = first + k;
+            uint32_t w[4];
+            philox4x32_10(attempt, P.sweep_lo, P.sweep_hi, 0x400u, P.rk[0][0], P.rk[0][1], w);
+            const uint32_t j = __umulhi(w[0], N);             // "select random particle to move"
+            const uint64_t i = base + j;
+            const bool has_l = j > 0u, has_r = j + 1u < N;
+            float px = x[i], py = y[i], pz = z[i];
+            const float xl = has_l ? x[i - 1] : px, yl = has_l ? y[i - 1] : py, zl = has_l ? z[i - 1] : pz;
+            const float xr = has_r ? x[i + 1] : px, yr = has_r ? y[i + 1] : py, zr = has_r ? z[i + 1] : pz;
+            const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
+            const bool acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
+                                                   toff_tab[j], attempt);
+            if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
+            if (kRecord && acc) atomicOr(dec_words + (attempt >> 5), 1u << (attempt & 31u));
+            n_acc += acc ? 1u : 0u;
+        }
+    }
+    n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
+    if ((threadIdx.x & 31u) == 0 && n_acc)
+        atomicAdd(acc_slots + ((chain >> 5) % kAccSlots), (unsigned long long)n_acc);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -38,7 +38,7 @@ def field_close(w, got, want):
 
 def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INCREMENTAL,
              hamiltonian=0, check_every=1, expect_flips=0.0, set_order=0, field_every=1, ext_field=None,
-             forbidden=None):
+             forbidden=None, scheme=0):
     if xyz0 is None:
         xyz0 = np.stack(workloads.gaussian_walks(w))
     sim = P.from_workload(w, xyz0=xyz0)
@@ -47,6 +47,7 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
         sim.set_external(ext_field, forbidden)
     sim.set_option(P.OPT_SET_ORDER, set_order)
     sim.set_option(P.OPT_FIELD_INTERVAL, field_every)
+    sim.set_option(P.OPT_SCHEME, scheme)
     sim.set_option(P.OPT_KERNEL, kernel)
     sim.set_option(P.OPT_DENSITY, density)
     sim.set_option(P.OPT_HAMILTONIAN, hamiltonian)
@@ -66,7 +67,7 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
             om_o = orc.fields(cnt_o)
         assert field_close(w, om_g, om_o) <= FIELD_RTOL, f"sweep {sweep}: fields differ"
         dec_o = np.zeros(nb, np.uint8)
-        acc_o = orc.sweep(x, y, z, om_o, sweep, move, dec_o)
+        acc_o = (orc.sweep_molecules if scheme == 1 else orc.sweep)(x, y, z, om_o, sweep, move, dec_o)
         sim.step(1)
         dec_g = P.unpack_decisions(sim.decisions(), nb)
         pos = sim.positions()
@@ -75,7 +76,16 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
         total_flips += flips
         assert agree.mean() >= DECISION_AGREEMENT, f"sweep {sweep}: {flips} decision flips of {nb}"
         ref = np.stack([x, y, z])
-        if move == oracle.MOVE_LOCAL:
+        if move == oracle.MOVE_LOCAL and scheme == 1:
+            # decisions belong to attempts, not beads: compare the chains without a flipped attempt
+            bad = np.zeros(nb, bool)
+            g = 0
+            for n, t in w.specs:
+                N = len(t)
+                bad[g:g + n * N] = np.repeat((~agree[g:g + n * N]).reshape(n, N).any(1), N)
+                g += n * N
+            assert np.array_equal(pos[:, ~bad], ref[:, ~bad]), f"sweep {sweep}: positions differ"
+        elif move == oracle.MOVE_LOCAL:
             assert np.array_equal(pos[:, agree], ref[:, agree]), f"sweep {sweep}: accepted positions differ"
         else:
             # a flipped neighbour changes the force on the next set: compare only chains without flips
@@ -193,6 +203,34 @@ def test_random_set_order_differs_from_fixed_order_and_ragged_tiles():
 @pytest.mark.parametrize("density", [P.DENSITY_INCREMENTAL, P.DENSITY_FULL])
 def test_field_interval(density):
     lockstep(workloads.c1(), 7, density=density, field_every=3)
+
+
+# ---------------------------------------------------------------------------------------------
+# molecule-parallel scheme (Code 1)
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[0], workloads.small_cases()[2],
+                               workloads.small_cases()[5], workloads.small_cases()[7]], ids=lambda w: w.name)
+def test_molecule_parallel_scheme(w):
+    lockstep(w, 4, scheme=1)
+
+
+def test_molecule_parallel_scheme_smart_mc_and_layout():
+    w = workloads.Workload("smc_mol", ((300, workloads.diblock(64, 19)), (150, workloads.homopolymer(16))), 64, 2,
+                           (3.0, 3.0, 3.0), (15, 15, 15), 35.0, 50.0, 0.1, 7, move="smc", smc_step=0.05 / 63)
+    lockstep(w, 3, scheme=1)
+    # storage order must not matter here either
+    w = workloads.c1()
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    out = []
+    for layout in (0, 1):
+        sim = P.from_workload(w, xyz0=xyz0)
+        sim.set_option(P.OPT_LAYOUT, layout)
+        sim.set_option(P.OPT_SORT_INTERVAL, 2)
+        sim.set_option(P.OPT_SCHEME, 1)
+        sim.step(5)
+        out.append((sim.positions(), sim.fields()[1], sim.stats()))
+        sim.destroy()
+    assert np.array_equal(out[0][0], out[1][0]) and np.array_equal(out[0][1], out[1][1]) and out[0][2] == out[1][2]
 
 
 # ---------------------------------------------------------------------------------------------
