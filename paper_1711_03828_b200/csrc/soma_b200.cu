@@ -262,6 +262,24 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
         if (c->scheme == 1) {   // Code 1: one thread per molecule
+            const size_t per_warp = sizeof(float) * 96 * (size_t)s.N;     // 32 chains x 3 coordinates
+            const int warps = (int)std::min<size_t>(4, (200 * 1024) / per_warp);
+            if (warps >= 1 && c->kernel_choice != 1) {   // chains staged in shared memory
+                auto kernel = soma::molecule_staged_kernel<kMove, kIncr, kRecord>;
+                const size_t smem = per_warp * warps;
+                if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                int per_sm = 1;
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, warps * 32, smem));
+                if (per_sm < 1) per_sm = 1;
+                const uint64_t n_groups = (s.n_chains + 31) / 32;
+                const uint64_t blocks = std::min<uint64_t>((uint64_t)c->n_sm * per_sm, (n_groups + warps - 1) / warps);
+                Timed t(c, SOMA_K_MOVE, 1);
+                kernel<<<(unsigned)blocks, warps * 32, smem, c->stream>>>(
+                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N,
+                    s.n_chains, (uint32_t)s.gid0, c->orig + s.chain_off, c->decisions, c->acc_slots);
+                CU(cudaGetLastError());
+                continue;
+            }
             const int threads = 128;
             const unsigned blocks = (unsigned)((s.n_chains + threads - 1) / threads);
             Timed t(c, SOMA_K_MOVE, 1);

@@ -600,6 +600,69 @@ molecule_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y
         atomicAdd(acc_slots + ((chain >> 5) % kAccSlots), (unsigned long long)n_acc);
 }
 
+// The same scheme with the chains staged in shared memory: a warp copies 32 consecutive chains
+// (32 N consecutive beads per coordinate array) with coalesced loads, every lane then runs the N
+// attempts of its own chain out of shared memory, and the warp writes the 32 chains back coalesced --
+// each position crosses HBM once per sweep, as in the fused kernel.  Dynamic shared memory:
+// warps_per_block * 3 * 32 N floats.
+template <int kMove, bool kIncr, bool kRecord>
+__global__ void __launch_bounds__(128)
+molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+                       const float* __restrict__ omega, uint32_t* __restrict__ counts,
+                       const uint32_t* __restrict__ toff_tab, uint32_t N, uint64_t n_chains, uint32_t gid0,
+                       const uint32_t* __restrict__ orig, uint32_t* __restrict__ dec_words,
+                       unsigned long long* __restrict__ acc_slots)
+{
+    extern __shared__ __align__(16) float stage_f[];
+    const uint32_t lane = threadIdx.x & 31u, wib = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    float* sx = stage_f + (size_t)wib * 96u * N;              // this warp's 3 x 32 N floats
+    float* sy = sx + 32u * N;
+    float* sz = sy + 32u * N;
+    const uint64_t n_groups = (n_chains + 31u) / 32u;
+    uint32_t n_acc = 0;
+    for (uint64_t grp = (uint64_t)blockIdx.x * warps + wib; grp < n_groups; grp += (uint64_t)gridDim.x * warps) {
+        const uint64_t chain0 = grp * 32u, base = chain0 * N;
+        const uint32_t n_here = (uint32_t)min((uint64_t)32u, n_chains - chain0), n_floats = n_here * N;
+        for (uint32_t e = lane; e < n_floats; e += 32u) {
+            sx[e] = x[base + e];
+            sy[e] = y[base + e];
+            sz[e] = z[base + e];
+        }
+        __syncwarp();
+        if (lane < n_here) {
+            const uint32_t mine = lane * N;
+            const uint32_t first = gid0 + orig[chain0 + lane] * N;
+            for (uint32_t k = 0; k < N; ++k) {                // "sequential iteration of particles"
+                const uint32_t attempt = first + k;
+                uint32_t w[4];
+                philox4x32_10(attempt, P.sweep_lo, P.sweep_hi, 0x400u, P.rk[0][0], P.rk[0][1], w);
+                const uint32_t j = __umulhi(w[0], N);         // "select random particle to move"
+                const uint32_t i = mine + j;
+                const bool has_l = j > 0u, has_r = j + 1u < N;
+                float px = sx[i], py = sy[i], pz = sz[i];
+                const float xl = has_l ? sx[i - 1] : px, yl = has_l ? sy[i - 1] : py, zl = has_l ? sz[i - 1] : pz;
+                const float xr = has_r ? sx[i + 1] : px, yr = has_r ? sy[i + 1] : py, zr = has_r ? sz[i + 1] : pz;
+                const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
+                const bool acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
+                                                       toff_tab[j], attempt);
+                if (acc) { sx[i] = px; sy[i] = py; sz[i] = pz; }
+                if (kRecord && acc) atomicOr(dec_words + (attempt >> 5), 1u << (attempt & 31u));
+                n_acc += acc ? 1u : 0u;
+            }
+        }
+        __syncwarp();
+        for (uint32_t e = lane; e < n_floats; e += 32u) {
+            x[base + e] = sx[e];
+            y[base + e] = sy[e];
+            z[base + e] = sz[e];
+        }
+        __syncwarp();
+    }
+    n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
+    if (lane == 0 && n_acc)
+        atomicAdd(acc_slots + ((blockIdx.x * warps + wib) % kAccSlots), (unsigned long long)n_acc);
+}
+
 // ------------------------------------------------------------------------------------------------
 // a3  occupation numbers from scratch (Eq. 4): counts[type][cell] += 1 per bead.
 // ------------------------------------------------------------------------------------------------

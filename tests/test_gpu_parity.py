@@ -209,9 +209,11 @@ def test_field_interval(density):
 # molecule-parallel scheme (Code 1)
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[0], workloads.small_cases()[2],
-                               workloads.small_cases()[5], workloads.small_cases()[7]], ids=lambda w: w.name)
-def test_molecule_parallel_scheme(w):
-    lockstep(w, 4, scheme=1)
+                               workloads.small_cases()[5], workloads.small_cases()[6], workloads.small_cases()[7]],
+                         ids=lambda w: w.name)
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC], ids=["staged", "direct"])
+def test_molecule_parallel_scheme(w, kernel):
+    lockstep(w, 4, scheme=1, kernel=kernel)
 
 
 def test_molecule_parallel_scheme_smart_mc_and_layout():
