@@ -26,6 +26,10 @@ constexpr int kAccSlots = 256;      // spread slots of the accepted-moves counte
 #define SOMA_FUSED_THREADS 128       // threads per block of the fused kernel
 #endif
 constexpr int kFusedThreads = SOMA_FUSED_THREADS;
+#ifndef SOMA_MOL_UNROLL
+#define SOMA_MOL_UNROLL 4
+#endif
+constexpr int kMolUnroll = SOMA_MOL_UNROLL;   // attempts of the staged molecule kernel unrolled together
 
 #ifndef SOMA_FUSED_MIN_BLOCKS
 #define SOMA_FUSED_MIN_BLOCKS 5      // resident blocks per SM the fused kernel is compiled for (register cap)
@@ -632,6 +636,7 @@ molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__
         if (lane < n_here) {
             const uint32_t mine = lane * N;
             const uint32_t first = gid0 + orig[chain0 + lane] * N;
+            #pragma unroll kMolUnroll
             for (uint32_t k = 0; k < N; ++k) {                // "sequential iteration of particles"
                 const uint32_t attempt = first + k;
                 uint32_t w[4];
