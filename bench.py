@@ -119,6 +119,22 @@ def oracle_rate(w, steps: int, warmup: int, budget_s: float = 20.0):
                       f"warm-up, OpenMP over chains"}, dt / steps * 1e3
 
 
+def max_over_ranks(value: float, dist, device) -> float:
+    """Timing rule: a multi-GPU number is the slowest rank's.  dist = torch.distributed or None."""
+    if dist is None:
+        return float(value)
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_moves_per_s(n_beads: int, steps: int, world: int, ms_total_max: float) -> float:
+    """Whole-job throughput of `world` independent replicas (replicas only): all moves of
+    all ranks divided by the slowest rank's time."""
+    return world * n_beads * steps / (ms_total_max * 1e-3)
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -190,11 +206,8 @@ def main():
         barrier()
     ms_total = e0.elapsed_time(e1)
     launches = sim.launch_count() - l0
-    t = torch.tensor([ms_total], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_total = float(t.item())
-    value = world * nb * args.steps / (ms_total * 1e-3)
+    ms_total = max_over_ranks(ms_total, dist, "cuda")
+    value = aggregate_moves_per_s(nb, args.steps, world, ms_total)
     att, acc, sweeps = sim.stats()
 
     # ---- roofline of the dominant kernel (move kernel), CUDA events inside the library ---------
@@ -253,10 +266,8 @@ def main():
         sim.fields(om_h, cn_h)            # D2H omega + counts
     barrier()
     dt = time.perf_counter() - t0
-    t = torch.tensor([dt], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    e2e = {"value": world * nb * n_e2e / float(t.item()), "unit": UNIT, "h2d_bytes_per_step": 12 * nb,
+    dt = max_over_ranks(dt, dist, "cuda")
+    e2e = {"value": world * nb * n_e2e / dt, "unit": UNIT, "h2d_bytes_per_step": 12 * nb,
            "d2h_bytes_per_step": 12 * nb + 8 * w.n_types * w.n_cells, "steps": n_e2e}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
