@@ -412,3 +412,49 @@ def test_switching_the_layout_mid_run_and_device_side_import_export():
     assert np.array_equal(a.positions(), b.positions())
     assert np.array_equal(a.fields()[1], b.fields()[1])
     a.destroy(); b.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
+# BASELINE config C2: statistics of the free-running GPU path over 1000 sweeps (no oracle involved:
+# closed forms for ideal chains; kappa N = 50 must suppress the density fluctuations)
+# ---------------------------------------------------------------------------------------------
+def _c2_statistics(kappaN):
+    w = workloads.c2(kappaN)
+    sim = P.from_workload(w, xyz0=np.stack(workloads.gaussian_walks(w)))
+    sim.step(1000)
+    pos = sim.positions().astype(np.float64)
+    _, cnt = sim.fields()
+    att, acc, n = sim.stats()
+    sim.destroy()
+    n_ch, N = w.specs[0][0], 32
+    Pm = pos.T.reshape(n_ch, N, 3)
+    b = Pm[:, 1:] - Pm[:, :-1]
+    re2 = ((Pm[:, -1] - Pm[:, 0]) ** 2).sum(-1)
+    return w, b, re2, cnt[0].astype(np.float64), acc / att
+
+
+def test_c2_ideal_chains_1000_sweeps_bond_statistics_and_re2():
+    w, b, re2, cnt, acc = _c2_statistics(0.0)
+    N, n_ch = 32, w.specs[0][0]
+    b2 = (b**2).sum(-1)
+    assert abs(b2.mean() * (N - 1) - 1) < 0.005                        # <b^2> = R_e0^2 / (N - 1)
+    assert abs((b2**2).mean() / b2.mean() ** 2 - 5 / 3) < 0.01          # Gaussian bonds
+    for a in range(3):
+        assert abs(b[..., a].var() * 3 * (N - 1) - 1) < 0.01 and abs(b[..., a].mean()) < 1e-3
+    assert abs(re2.mean() - 1.0) < 5 * np.sqrt(2 / 3 / n_ch)             # <R_e^2> = R_e0^2
+    assert cnt.sum() == w.n_beads and abs(cnt.mean() - 32.0) < 1e-9     # 32 beads per cell on average
+    assert 0.3 < acc < 0.9
+
+
+def test_c2_compressibility_suppresses_density_fluctuations():
+    _, _, _, cnt0, _ = _c2_statistics(0.0)
+    _, b, re2, cnt50, _ = _c2_statistics(50.0)
+    f0, f50 = cnt0.var() / cnt0.mean(), cnt50.var() / cnt50.mean()
+    # ideal chains: a chain puts several of its beads into the same cell (b_0 = 0.18 < DeltaL = 0.25), so
+    # Var(n)/<n> is that multiplicity (~2.8), not the Poisson 1; kappa_0 = 50/32 must push it well below
+    print(f"Var(n)/<n>: kappaN=0 {f0:.3f}, kappaN=50 {f50:.3f}")
+    assert 1.5 < f0 < 4.0
+    assert f50 < 0.5 * f0
+    # the compressibility term acts on beads of the same chain too (they share cells), so the bonds are
+    # stretched by a few per cent relative to the ideal chain -- not a closed form, only a sanity band
+    assert abs(((b**2).sum(-1)).mean() * 31 - 1) < 0.06
