@@ -57,6 +57,8 @@ class _System(C.Structure):
         ("set_order", C.c_int32),
         ("field_every", C.c_uint32),
         ("scheme", C.c_int32),
+        ("spec_n_bonds", C.POINTER(C.c_uint32)),
+        ("bonds", C.POINTER(C.c_uint32)),
         ("ext_field", C.POINTER(C.c_float)),
         ("forbidden", C.POINTER(C.c_uint8)),
     ]
@@ -101,6 +103,8 @@ def lib():
         L.soma_oracle_first_set.restype = C.c_uint32
         L.soma_oracle_sweep.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, u8p]
         L.soma_oracle_sweep.restype = C.c_uint64
+        L.soma_oracle_sets.argtypes = [sysp, C.c_uint32, u32p]
+        L.soma_oracle_sets.restype = C.c_uint32
         L.soma_oracle_pick.argtypes = [sysp, C.c_uint64, C.c_uint64, C.c_uint32]
         L.soma_oracle_pick.restype = C.c_uint32
         L.soma_oracle_sweep_molecules.argtypes = [sysp, fp, fp, fp, fp, C.c_uint64, C.c_int, u8p]
@@ -183,6 +187,7 @@ class OracleSystem:
     smc_step: float = 0.0
     set_order: int = 0          # 0: even set then odd set; 1: random order per chain and sweep
     field_every: int = 1        # fields refreshed after every field_every-th sweep
+    bonds: Optional[Sequence] = None   # per spec: None (linear chain) or an (n_bonds, 2) array of monomer pairs
     scheme: int = 0             # 0: independent sets (Code 2); 1: molecule-parallel random picks (Code 1)
     ext_field: Optional[np.ndarray] = None    # (n_types, n_cells) float32 static field added to omega
     forbidden: Optional[np.ndarray] = None    # (n_cells,) uint8, 1 = no particle may enter the cell
@@ -224,6 +229,19 @@ class OracleSystem:
         s.set_order = int(self.set_order)
         s.field_every = int(self.field_every)
         s.scheme = int(self.scheme)
+        if self.bonds is not None:
+            per = [np.zeros((0, 2), np.uint32) if b is None else np.ascontiguousarray(b, dtype=np.uint32).reshape(-1, 2)
+                   for b in self.bonds]
+            assert len(per) == len(self.specs)
+            self._nbonds = np.array([len(b) for b in per], dtype=np.uint32)
+            self._bonds = np.ascontiguousarray(np.concatenate(per).reshape(-1), dtype=np.uint32)
+            if self._bonds.size == 0:
+                self._bonds = np.zeros(2, np.uint32)
+            s.spec_n_bonds = self._nbonds.ctypes.data_as(C.POINTER(C.c_uint32))
+            s.bonds = self._bonds.ctypes.data_as(C.POINTER(C.c_uint32))
+        else:
+            s.spec_n_bonds = C.POINTER(C.c_uint32)()
+            s.bonds = C.POINTER(C.c_uint32)()
         if self.ext_field is not None:
             self._ext = np.ascontiguousarray(self.ext_field, dtype=np.float32).reshape(self.n_types, -1)
             s.ext_field = self._ext.ctypes.data_as(C.POINTER(C.c_float))
@@ -307,6 +325,12 @@ class OracleSystem:
         """One MC sweep in place (omega frozen). Returns the number of accepted moves."""
         return int(lib().soma_oracle_sweep(self.ref, _fp(x), _fp(y), _fp(z), _fp(omega), sweep,
                                            move_kind, _u8p(decisions)))
+
+    def sets(self, spec: int) -> np.ndarray:
+        """Independent set of every monomer of architecture ``spec`` (greedy first fit, reading R25)."""
+        out = np.zeros(len(self.specs[spec][1]), dtype=np.uint32)
+        lib().soma_oracle_sets(self.ref, spec, _u32p(out))
+        return out
 
     def pick(self, attempt_id: int, sweep: int, N: int) -> int:
         """Particle chosen by attempt ``attempt_id`` (= first bead + k) of a chain of N beads (Code 1)."""

@@ -62,6 +62,8 @@ typedef struct {
     uint32_t        field_every;   /* omega refreshed after every field_every-th sweep (R22); 0, 1: every sweep */
     int32_t         scheme;        /* 0: independent sets (Code 2); 1: molecule-parallel, N random picks */
                                    /*    per molecule and sweep (Code 1; R24)           */
+    const uint32_t *spec_n_bonds;  /* nullable; [n_specs] bonds of each architecture, 0 = linear chain   */
+    const uint32_t *bonds;         /* concatenated (i, j) monomer pairs of the architectures with bonds  */
     const float    *ext_field;     /* nullable, [n_types][cells]: static external field added to omega   */
     const uint8_t  *forbidden;     /* nullable, [cells]: 1 = no particle may enter this cell             */
 } oracle_system;
@@ -258,18 +260,31 @@ void soma_oracle_local_proposal(const oracle_system *s, uint64_t bead, uint64_t 
  * fp32 operation order below).  Non-bonded (Eq. 15): dE_nb = omega_k(c') - omega_k(c),
  * with c' the cell of the stored trial position r' = fl32(r + d); exactly 0 when c' == c.
  * has_l / has_r say whether the chain neighbours at bead-1 / bead+1 exist. */
+/* The same with the bond sum s = sum_nb (r - r_nb) and the number of bonded neighbours m handed in
+ * (any molecular architecture). */
+static void local_delta_e_core(const oracle_system *s, const float *x, const float *y, const float *z,
+                               const float *omega, uint64_t bead, float sx, float sy, float sz, float mf,
+                               uint32_t type, const float d[3], float *dE_b, float *dE_nb, float r_new[3]);
+
 void soma_oracle_local_delta_e(const oracle_system *s, const float *x, const float *y, const float *z,
                                const float *omega, uint64_t bead, int has_l, int has_r, uint32_t type,
                                const float d[3], float *dE_b, float *dE_nb, float r_new[3])
 {
-    const float hk = (float)(1.5 * ((double)s->N_ref - 1.0)); /* k_0 / 2 with R_e0 = 1 */
     const float rx = x[bead], ry = y[bead], rz = z[bead];
     /* s = sum over existing neighbours of (r - r_nb); an absent neighbour contributes exactly 0 */
     const float blx = has_l ? rx - x[bead - 1] : 0.0f, brx = has_r ? rx - x[bead + 1] : 0.0f;
     const float bly = has_l ? ry - y[bead - 1] : 0.0f, bry = has_r ? ry - y[bead + 1] : 0.0f;
     const float blz = has_l ? rz - z[bead - 1] : 0.0f, brz = has_r ? rz - z[bead + 1] : 0.0f;
-    const float sx = blx + brx, sy = bly + bry, sz = blz + brz;
     const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
+    local_delta_e_core(s, x, y, z, omega, bead, blx + brx, bly + bry, blz + brz, mf, type, d, dE_b, dE_nb, r_new);
+}
+
+static void local_delta_e_core(const oracle_system *s, const float *x, const float *y, const float *z,
+                               const float *omega, uint64_t bead, float sx, float sy, float sz, float mf,
+                               uint32_t type, const float d[3], float *dE_b, float *dE_nb, float r_new[3])
+{
+    const float hk = (float)(1.5 * ((double)s->N_ref - 1.0)); /* k_0 / 2 with R_e0 = 1 */
+    const float rx = x[bead], ry = y[bead], rz = z[bead];
     const float ds = fmaf(d[2], sz, fmaf(d[1], sy, d[0] * sx));
     const float dd = fmaf(d[2], d[2], fmaf(d[1], d[1], d[0] * d[0]));
     *dE_b = hk * fmaf(2.0f, ds, mf * dd);
@@ -336,19 +351,30 @@ void soma_oracle_smc_proposal(const oracle_system *s, uint64_t bead, uint64_t sw
     *u = soma_oracle_u23(v[0]) - 1.0f;
 }
 
+static void smc_delta_core(const oracle_system *s, const float *x, const float *y, const float *z,
+                           const float *omega, uint64_t bead, float sx, float sy, float sz, float mf, uint32_t type,
+                           const float g[3], float d[3], float *dE, float *log_ratio, float r_new[3]);
+
 void soma_oracle_smc_delta(const oracle_system *s, const float *x, const float *y, const float *z,
                            const float *omega, uint64_t bead, int has_l, int has_r, uint32_t type,
+                           const float g[3], float d[3], float *dE, float *log_ratio, float r_new[3])
+{
+    const float rx = x[bead], ry = y[bead], rz = z[bead];
+    const float blx = has_l ? rx - x[bead - 1] : 0.0f, brx = has_r ? rx - x[bead + 1] : 0.0f;
+    const float bly = has_l ? ry - y[bead - 1] : 0.0f, bry = has_r ? ry - y[bead + 1] : 0.0f;
+    const float blz = has_l ? rz - z[bead - 1] : 0.0f, brz = has_r ? rz - z[bead + 1] : 0.0f;
+    const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
+    smc_delta_core(s, x, y, z, omega, bead, blx + brx, bly + bry, blz + brz, mf, type, g, d, dE, log_ratio, r_new);
+}
+
+static void smc_delta_core(const oracle_system *s, const float *x, const float *y, const float *z,
+                           const float *omega, uint64_t bead, float sx, float sy, float sz, float mf, uint32_t type,
                            const float g[3], float d[3], float *dE, float *log_ratio, float r_new[3])
 {
     const float k0 = (float)(3.0 * ((double)s->N_ref - 1.0));
     const float a_s = s->smc_step;
     const float noise = sqrtf(2.0f * a_s);
     const float rx = x[bead], ry = y[bead], rz = z[bead];
-    const float blx = has_l ? rx - x[bead - 1] : 0.0f, brx = has_r ? rx - x[bead + 1] : 0.0f;
-    const float bly = has_l ? ry - y[bead - 1] : 0.0f, bry = has_r ? ry - y[bead + 1] : 0.0f;
-    const float blz = has_l ? rz - z[bead - 1] : 0.0f, brz = has_r ? rz - z[bead + 1] : 0.0f;
-    const float sx = blx + brx, sy = bly + bry, sz = blz + brz;
-    const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
     const float F[3] = { -k0 * sx, -k0 * sy, -k0 * sz };
     for (int a = 0; a < 3; ++a) d[a] = fmaf(a_s, F[a], noise * g[a]);
     const float ds = fmaf(d[2], sz, fmaf(d[1], sy, d[0] * sx));
@@ -391,6 +417,113 @@ static int mc_smc(const oracle_system *s, float *x, float *y, float *z, const fl
     return 1;
 }
 
+/* ------------------------------------------------------------------------------------------ */
+/* General molecular architectures ("almost arbitrary architectures", 292,     */
+/* 344-354).  An architecture with spec_n_bonds > 0 is given by its bond list; every bond is the  */
+/* harmonic spring of Eq. 2 with the same k_0.  Reading R25:                                       */
+/*  - neighbour lists in ascending monomer index; the bond sum s = sum_nb (r - r_nb) of Eq. 2 is   */
+/*    accumulated in that order in fp32 (a linear chain given as bonds (j, j+1) then reproduces    */
+/*    the chain code above bit for bit);                                                           */
+/*  - independent sets ("a simple heuristics ... aiming for the minimal number of sets",            */
+/*    PAPER.md:292): greedy first fit in monomer order -- monomer j joins the lowest-numbered set   */
+/*    that holds none of its bonded neighbours; for a linear chain that is even / odd (Fig. 1);     */
+/*  - the sets are worked through in the order 0, 1, ... (R11), their members in monomer order.     */
+/* ------------------------------------------------------------------------------------------ */
+static const uint32_t *spec_bonds(const oracle_system *s, uint32_t spec)
+{
+    const uint32_t *b = s->bonds;
+    for (uint32_t a = 0; a < spec; ++a) b += 2u * s->spec_n_bonds[a];
+    return b;
+}
+
+/* adjacency of one architecture: nbr_off[N+1], nbr[2 n_bonds] (ascending within a monomer) */
+static void build_adjacency(uint32_t N, uint32_t n_bonds, const uint32_t *bonds, uint32_t *nbr_off, uint32_t *nbr)
+{
+    for (uint32_t j = 0; j <= N; ++j) nbr_off[j] = 0;
+    for (uint32_t b = 0; b < n_bonds; ++b) { nbr_off[bonds[2 * b] + 1]++; nbr_off[bonds[2 * b + 1] + 1]++; }
+    for (uint32_t j = 0; j < N; ++j) nbr_off[j + 1] += nbr_off[j];
+    uint32_t *fill = (uint32_t *)calloc(N, sizeof(uint32_t));
+    for (uint32_t b = 0; b < n_bonds; ++b) {
+        const uint32_t i = bonds[2 * b], j = bonds[2 * b + 1];
+        nbr[nbr_off[i] + fill[i]++] = j;
+        nbr[nbr_off[j] + fill[j]++] = i;
+    }
+    free(fill);
+    for (uint32_t j = 0; j < N; ++j)          /* insertion sort of each (short) list */
+        for (uint32_t a = nbr_off[j] + 1; a < nbr_off[j + 1]; ++a) {
+            const uint32_t v = nbr[a];
+            uint32_t c = a;
+            while (c > nbr_off[j] && nbr[c - 1] > v) { nbr[c] = nbr[c - 1]; --c; }
+            nbr[c] = v;
+        }
+}
+
+/* set_of[j] = independent set of monomer j of architecture `spec`; returns the number of sets */
+uint32_t soma_oracle_sets(const oracle_system *s, uint32_t spec, uint32_t *set_of)
+{
+    const uint32_t N = s->spec_n_beads[spec];
+    const uint32_t nb = s->spec_n_bonds ? s->spec_n_bonds[spec] : 0u;
+    if (nb == 0) {                                   /* linear chain: even / odd (Fig. 1) */
+        for (uint32_t j = 0; j < N; ++j) set_of[j] = j & 1u;
+        return N > 1 ? 2u : 1u;
+    }
+    uint32_t *off = (uint32_t *)malloc(sizeof(uint32_t) * (N + 1)), *nbr = (uint32_t *)malloc(sizeof(uint32_t) * 2 * nb);
+    build_adjacency(N, nb, spec_bonds(s, spec), off, nbr);
+    uint32_t n_sets = 0;
+    for (uint32_t j = 0; j < N; ++j) {
+        uint32_t c = 0;
+        for (;;) {                                   /* lowest set without a bonded neighbour (only j' < j are placed) */
+            int clash = 0;
+            for (uint32_t a = off[j]; a < off[j + 1]; ++a)
+                if (nbr[a] < j && set_of[nbr[a]] == c) clash = 1;
+            if (!clash) break;
+            ++c;
+        }
+        set_of[j] = c;
+        if (c + 1 > n_sets) n_sets = c + 1;
+    }
+    free(off); free(nbr);
+    return n_sets;
+}
+
+/* one molecule of a general architecture, all sets in order */
+static uint64_t sweep_general_molecule(const oracle_system *s, float *x, float *y, float *z, const float *omega,
+                                       uint64_t first, uint32_t N, const uint8_t *types, const uint32_t *off,
+                                       const uint32_t *nbr, const uint32_t *set_of, uint32_t n_sets,
+                                       uint64_t sweep, int move_kind, uint8_t *decisions)
+{
+    uint64_t accepted = 0;
+    for (uint32_t i_set = 0; i_set < n_sets; ++i_set)
+        for (uint32_t ip = 0; ip < N; ++ip) {
+            if (set_of[ip] != i_set) continue;
+            const uint64_t bead = first + ip;
+            float sx = 0.0f, sy = 0.0f, sz = 0.0f;
+            const uint32_t m = off[ip + 1] - off[ip];
+            for (uint32_t a = off[ip]; a < off[ip + 1]; ++a) {
+                const uint64_t nb = first + nbr[a];
+                const float bx = x[bead] - x[nb], by = y[bead] - y[nb], bz = z[bead] - z[nb];
+                if (a == off[ip]) { sx = bx; sy = by; sz = bz; } else { sx = sx + bx; sy = sy + by; sz = sz + bz; }
+            }
+            float r_new[3], u, dE;
+            if (move_kind == 2) {
+                float g[3], d[3], lr;
+                soma_oracle_smc_proposal(s, bead, sweep, g, &u);
+                smc_delta_core(s, x, y, z, omega, bead, sx, sy, sz, (float)m, types[ip], g, d, &dE, &lr, r_new);
+                dE = dE + lr;
+            } else {
+                float d[3], eb, enb;
+                soma_oracle_local_proposal(s, bead, sweep, d, &u);
+                local_delta_e_core(s, x, y, z, omega, bead, sx, sy, sz, (float)m, types[ip], d, &eb, &enb, r_new);
+                dE = eb + enb;
+            }
+            const int acc = soma_oracle_metropolis(dE, u);
+            if (acc) { x[bead] = r_new[0]; y[bead] = r_new[1]; z[bead] = r_new[2]; }
+            accepted += (uint64_t)acc;
+            if (decisions) decisions[bead] = (uint8_t)acc;
+        }
+    return accepted;
+}
+
 /* "Generate random permutation of the sets" (Code 2; "a pre-defined random order",
  * PAPER.md:294).  A linear chain has two sets, so the permutation is one fair bit per molecule and
  * sweep.  Reading R21: bit 31 of word 0 of Philox(counter = (global index of the molecule's first
@@ -421,6 +554,24 @@ uint64_t soma_oracle_sweep(const oracle_system *s, float *x, float *y, float *z,
     for (uint32_t a = 0; a < s->n_specs; ++a) {
         const uint32_t N = s->spec_n_beads[a];
         const int64_t n_mol = (int64_t)s->spec_n_chains[a];
+        if (s->spec_n_bonds && s->spec_n_bonds[a] > 0) {        /* general architecture (R25) */
+            const uint32_t nb = s->spec_n_bonds[a];
+            uint32_t *off = (uint32_t *)malloc(sizeof(uint32_t) * (N + 1));
+            uint32_t *nbr = (uint32_t *)malloc(sizeof(uint32_t) * 2 * nb);
+            uint32_t *set_of = (uint32_t *)malloc(sizeof(uint32_t) * N);
+            build_adjacency(N, nb, spec_bonds(s, a), off, nbr);
+            const uint32_t n_sets = soma_oracle_sets(s, a, set_of);
+#ifdef _OPENMP
+#pragma omp parallel for schedule(static) reduction(+ : accepted)
+#endif
+            for (int64_t mol = 0; mol < n_mol; ++mol)
+                accepted += sweep_general_molecule(s, x, y, z, omega, spec_first_bead + (uint64_t)mol * N, N, types,
+                                                   off, nbr, set_of, n_sets, sweep, move_kind, decisions);
+            free(off); free(nbr); free(set_of);
+            spec_first_bead += (uint64_t)n_mol * N;
+            types += N;
+            continue;
+        }
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static) reduction(+ : accepted)
 #endif

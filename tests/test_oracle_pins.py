@@ -153,7 +153,7 @@ def _total_H(pos, chains, types, omega, k0, box, grid):
     return H
 
 
-def _tiny_system(seed, specs, N_ref, box, grid, A=0.1, **kw):
+def _tiny_system(seed, specs, N_ref, box, grid, A=0.1, **kw):  # kw: set_order, bonds, ...
     s = OracleSystem(specs=specs, N_ref=N_ref, n_types=2, box=box, grid=grid, chiN=0.0, kappaN=0.0,
                      A=A, seed=seed, **kw)
     rng = np.random.default_rng(seed)
@@ -813,3 +813,133 @@ def test_molecule_scheme_relaxes_ideal_chains():
     b2 = (b**2).sum(-1)
     assert abs(b2.mean() * (N - 1) - 1) < 0.012
     assert abs(re2.mean() - 1.0) < 5 * math.sqrt(2 / 3 / n)
+
+
+# ----------------------------------------------------------------------------------------------
+# P15  general molecular architectures: bond lists, independent sets
+# ----------------------------------------------------------------------------------------------
+def _star(arms, arm_len):
+    """Bonds of a star: monomer 0 is the centre, arm a holds monomers 1 + a*arm_len ... in order."""
+    bonds = []
+    for a in range(arms):
+        prev = 0
+        for k in range(arm_len):
+            j = 1 + a * arm_len + k
+            bonds.append((prev, j))
+            prev = j
+    return np.array(bonds, np.uint32)
+
+
+def test_independent_sets_are_greedy_first_fit_and_valid():
+    star, ring5 = _star(3, 4), np.array([(0, 1), (1, 2), (2, 3), (3, 4), (4, 0)], np.uint32)
+    lin = np.array([(j, j + 1) for j in range(6)], np.uint32)
+    s = OracleSystem(specs=[(1, np.zeros(13, np.uint8)), (1, np.zeros(5, np.uint8)), (1, np.zeros(7, np.uint8)),
+                            (1, np.zeros(7, np.uint8))], N_ref=8, n_types=1, box=(1.0,) * 3, grid=(2, 2, 2),
+                     bonds=[star, ring5, lin, None])
+    for spec, bonds, N in [(0, star, 13), (1, ring5, 5), (2, lin, 7)]:
+        sets = s.sets(spec)
+        nbrs = [[] for _ in range(N)]
+        for i, j in bonds:
+            nbrs[i].append(j); nbrs[j].append(i)
+        for j in range(N):
+            earlier = {int(sets[k]) for k in nbrs[j] if k < j}
+            assert sets[j] == min(c for c in range(N) if c not in earlier)     # first fit in monomer order
+            assert all(sets[k] != sets[j] for k in nbrs[j])                    # members are not bonded
+    assert list(s.sets(1)) == [0, 1, 0, 1, 2]                                  # odd ring needs a third set
+    assert list(s.sets(2)) == [0, 1, 0, 1, 0, 1, 0] == list(s.sets(3))         # linear chain: even / odd (Fig. 1)
+    assert s.sets(0)[0] == 0 and set(s.sets(0)[[1, 5, 9]]) == {1}              # star: centre, then first arm beads
+
+
+@pytest.mark.parametrize("move,kw", [(MOVE_LOCAL, {}), (MOVE_SMC, {"smc_step": 0.004})])
+def test_linear_chain_given_as_bonds_reproduces_the_chain_code(move, kw):
+    N, n = 9, 40
+    types = np.array([0, 0, 0, 1, 1, 1, 1, 0, 0], np.uint8)
+    lin = np.array([(j + 1, j) if j % 2 else (j, j + 1) for j in range(N - 1)][::-1], np.uint32)   # shuffled on purpose
+    common = dict(specs=[(n, types)], N_ref=N, n_types=2, box=(2.0,) * 3, grid=(4, 4, 4), A=0.3, seed=5, **kw)
+    a, b = OracleSystem(**common), OracleSystem(bonds=[lin], **common)
+    rng = np.random.default_rng(3)
+    P = np.cumsum(rng.standard_normal((n, N, 3)) * 0.2 + (rng.random((n, 1, 3)) * 2) * (np.arange(N)[None, :, None] == 0), 1)
+    xa = [np.ascontiguousarray(P.reshape(-1, 3)[:, c], dtype=np.float32) for c in range(3)]
+    xb = [v.copy() for v in xa]
+    omega = rng.normal(0, 1, (2, 64)).astype(np.float32)
+    for sweep in range(6):
+        da, db = np.zeros(n * N, np.uint8), np.zeros(n * N, np.uint8)
+        assert a.sweep(*xa, omega, sweep, move, da) == b.sweep(*xb, omega, sweep, move, db)
+        assert np.array_equal(da, db) and all(np.array_equal(u, v) for u, v in zip(xa, xb))
+
+
+def _total_H_bonds(pos, mols, bond_lists, types, omega, k0, box, grid):
+    H = 0.0
+    for (first, N), bonds in zip(mols, bond_lists):
+        for i, j in bonds:
+            b = pos[first + i] - pos[first + j]
+            H += 0.5 * k0 * float(b @ b)
+        for j in range(N):
+            H += float(omega[types[first + j], _cell_f64(pos[first + j], box, grid)])
+    return H
+
+
+def test_general_architecture_sweep_replayed_by_brute_force():
+    """Star and ring molecules: replay of a sweep set by set (sets from the test above), members in
+    monomer order, with the total Hamiltonian (all bonds + field) recomputed in float64."""
+    star, ring = _star(3, 2), np.array([(0, 1), (1, 2), (2, 3), (3, 4), (4, 0)], np.uint32)
+    specs = [(3, np.array([0, 1, 1, 0, 0, 1, 1], np.uint8)), (2, np.array([0, 0, 1, 1, 1], np.uint8))]
+    box, grid = (2.0, 2.0, 2.0), (4, 4, 4)
+    s, mols, pos, omega = _tiny_system(41, specs, 8, box, grid, A=0.3, bonds=[star, ring])
+    bond_lists = [star] * 3 + [ring] * 2
+    set_lists = [s.sets(0)] * 3 + [s.sets(1)] * 2
+    types = s.bead_types()
+    k0 = 3.0 * (s.N_ref - 1)
+    compared = 0
+    for sweep in range(8):
+        x, y, z = (np.ascontiguousarray(pos[:, a]) for a in range(3))
+        dec = np.zeros(len(pos), np.uint8)
+        s.sweep(x, y, z, omega, sweep, MOVE_LOCAL, dec)
+        ref, ref_dec, fragile = pos.copy(), np.zeros(len(pos), np.uint8), False
+        for (first, N), sets in zip(mols, set_lists):
+            for i_set in range(int(sets.max()) + 1):
+                for j in range(N):
+                    if sets[j] != i_set:
+                        continue
+                    g = first + j
+                    d, u = s.local_proposal(g, sweep)
+                    rn = ref[g] + d
+                    p64 = ref.astype(np.float64)
+                    H0 = _total_H_bonds(p64, mols, bond_lists, types, omega, k0, box, grid)
+                    p64[g] = rn
+                    dE = _total_H_bonds(p64, mols, bond_lists, types, omega, k0, box, grid) - H0
+                    thr = math.exp(-dE) if dE > 0 else 2.0
+                    if abs(u - thr) < 1e-5 or abs(dE) < 1e-6:
+                        fragile = True
+                    if dE <= 0 or u < thr:
+                        ref[g] = rn
+                        ref_dec[g] = 1
+        if not fragile:
+            compared += 1
+            assert np.array_equal(dec, ref_dec)
+            assert np.array_equal(np.stack([x, y, z], 1), ref)
+        pos = np.stack([x, y, z], 1)
+    assert compared >= 3
+
+
+def test_ideal_star_polymers_relax_to_gaussian_tree_statistics():
+    """Every bond is the spring of Eq. 2, so in an ideal branched molecule the mean-square distance of
+    two monomers p bonds apart along the tree is p / (N_ref - 1) R_e0^2."""
+    arms, arm_len, n, N_ref = 3, 4, 8000, 9
+    N = 1 + arms * arm_len
+    s = OracleSystem(specs=[(n, np.zeros(N, np.uint8))], N_ref=N_ref, n_types=1, box=(8.0,) * 3, grid=(8, 8, 8),
+                     A=0.2, seed=12, bonds=[_star(arms, arm_len)])
+    rng = np.random.default_rng(2)
+    P = (rng.random((n, 1, 3)) * 8 + rng.standard_normal((n, N, 3)) * 0.05)      # collapsed start: must swell
+    x, y, z = (np.ascontiguousarray(P.reshape(-1, 3)[:, a], dtype=np.float32) for a in range(3))
+    omega = np.zeros((1, s.n_cells), np.float32)
+    for sweep in range(500):
+        s.sweep(x, y, z, omega, sweep, MOVE_LOCAL)
+    Q = np.stack([x, y, z], -1).astype(np.float64).reshape(n, N, 3)
+    def msd(i, j):
+        return ((Q[:, i] - Q[:, j]) ** 2).sum(-1).mean()
+    b2 = 1.0 / (N_ref - 1)
+    tip = [a * arm_len + arm_len for a in range(arms)]
+    for (i, j, p) in [(0, 1, 1), (0, tip[0], arm_len), (tip[0], tip[1], 2 * arm_len), (tip[1], tip[2], 2 * arm_len),
+                      (2, 3, 1), (1, 5, 2)]:
+        assert abs(msd(i, j) / (p * b2) - 1) < 0.03 + 4 * math.sqrt(2 / 3 / n), (i, j, p, msd(i, j))
