@@ -84,12 +84,20 @@ enum { SOMA_K_MOVE = 0, SOMA_K_DENSITY = 1, SOMA_K_FIELD = 2, SOMA_K_LAYOUT = 3,
 
 typedef struct soma_ctx soma_ctx; /* opaque */
 
-/* One molecular architecture: n_chains linear chains of n_beads monomers with the given bead
- * types (architecture stored once per molecule type). */
+/* One molecular architecture: n_chains molecules of n_beads monomers with the given bead types
+ * (architecture stored once per molecule type).  n_bonds = 0: a linear chain
+ * (monomer j bonded to j + 1).  n_bonds > 0: any architecture (stars, rings, ...) given by its bond
+ * list; every bond is the harmonic spring of Eq. 2.  The library then builds the independent sets
+ * by greedy first fit in monomer order -- monomer j joins the lowest-numbered set that
+ * holds none of its bonded neighbours -- works through them in the order 0, 1, ..., and sums the
+ * bonds of a monomer in ascending order of the neighbour's index (R25).  Architectures
+ * with a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only. */
 typedef struct {
-    uint64_t       n_chains;
-    uint32_t       n_beads;
-    const uint8_t *types; /* host, [n_beads], each < n_types; read during soma_init only */
+    uint64_t        n_chains;
+    uint32_t        n_beads;
+    const uint8_t  *types;   /* host, [n_beads], each < n_types; read during soma_init only          */
+    uint32_t        n_bonds; /* 0: linear chain                                                       */
+    const uint32_t *bonds;   /* host, [2 * n_bonds] monomer pairs (i, j), i != j, each pair once; or NULL */
 } soma_chain_spec;
 
 /* Create a system and run stage 1 (densities, fields) on its initial configuration.

@@ -12,7 +12,8 @@ from ._build import build  # noqa: F401
 
 def from_workload(w, xyz0=None, stream=None) -> "Soma":
     """Create a system from a ``workloads.Workload`` description (marshalling only)."""
-    s = Soma([(n, t) for n, t in w.specs], w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A,
+    bonds = getattr(w, "bonds", None) or [None] * len(w.specs)
+    s = Soma([(n, t, b) for (n, t), b in zip(w.specs, bonds)], w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A,
              w.seed, xyz0=xyz0, stream=stream)
     if getattr(w, "move", "local") == "smc":
         s.set_option(OPT_SMC_STEP, w.smc_step)

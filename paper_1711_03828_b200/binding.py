@@ -38,7 +38,8 @@ class SomaError(RuntimeError):
 
 
 class _ChainSpec(C.Structure):
-    _fields_ = [("n_chains", C.c_uint64), ("n_beads", C.c_uint32), ("types", C.POINTER(C.c_uint8))]
+    _fields_ = [("n_chains", C.c_uint64), ("n_beads", C.c_uint32), ("types", C.POINTER(C.c_uint8)),
+                ("n_bonds", C.c_uint32), ("bonds", C.POINTER(C.c_uint32))]
 
 
 _lib = None
@@ -104,12 +105,17 @@ class Soma:
         L = load()
         self._L = L
         self._h = C.c_void_p()
-        keep = [np.ascontiguousarray(t, dtype=np.uint8) for _, t in specs]
+        # a spec is (n_chains, types) for a linear chain or (n_chains, types, bonds) with an (n_bonds, 2) bond list
+        keep = [np.ascontiguousarray(sp[1], dtype=np.uint8) for sp in specs]
+        keep_b = [np.ascontiguousarray(sp[2], dtype=np.uint32).reshape(-1, 2) if len(sp) > 2 and sp[2] is not None
+                  else None for sp in specs]
         arr = (_ChainSpec * len(specs))()
-        for i, ((n, _), t) in enumerate(zip(specs, keep)):
-            arr[i].n_chains = int(n)
+        for i, (sp, t, bd) in enumerate(zip(specs, keep, keep_b)):
+            arr[i].n_chains = int(sp[0])
             arr[i].n_beads = len(t)
             arr[i].types = t.ctypes.data_as(C.POINTER(C.c_uint8))
+            arr[i].n_bonds = 0 if bd is None else len(bd)
+            arr[i].bonds = C.POINTER(C.c_uint32)() if bd is None else bd.ctypes.data_as(C.POINTER(C.c_uint32))
         cbox = (C.c_float * 3)(*[float(v) for v in box])
         cgrid = (C.c_int * 3)(*[int(v) for v in grid])
         if stream is None:

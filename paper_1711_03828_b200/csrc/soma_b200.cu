@@ -61,6 +61,11 @@ struct Spec {
     uint32_t log2N = 0;     // fused_ok only
     uint64_t chain_off = 0; // offset into orig[]
     uint32_t n_tiles = 0;   // full 128-bead tiles (fused_ok only)
+    // general architecture (bond list): device words nbr_off[N+1] | nbr[2 n_bonds] | members[N] at arch_off
+    bool general = false;
+    uint32_t n_bonds = 0;
+    uint64_t arch_off = 0;
+    std::vector<uint32_t> set_off;   // [n_sets + 1] offsets into members[]
 };
 
 constexpr int kEventPool = 2048;
@@ -81,6 +86,7 @@ struct soma_ctx {
     uint32_t* counts = nullptr;
     float* omega = nullptr;
     uint32_t* toff = nullptr;
+    uint32_t* arch = nullptr;        // architectures given by bond lists (Spec::arch_off)
     float* ext = nullptr;            // [n_types][cells] static external field, or null
     uint8_t* forbidden = nullptr;    // [cells] 1 = no particle may enter, or null
     uint64_t n_forbidden = 0;
@@ -261,6 +267,22 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
 {
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
+        if (s.general) {        // bond-list architecture: the independent sets one after the other
+            const uint32_t* arch = c->arch + s.arch_off;
+            const uint32_t *nbr_off = arch, *nbr = arch + (s.N + 1), *members = nbr + 2 * (size_t)s.n_bonds;
+            for (size_t i_set = 0; i_set + 1 < s.set_off.size(); ++i_set) {
+                const uint32_t set_size = s.set_off[i_set + 1] - s.set_off[i_set];
+                const uint64_t n_items = s.n_chains * set_size;
+                const int threads = 256;
+                Timed t(c, SOMA_K_MOVE, 1);
+                soma::arch_move_kernel<kMove, kIncr, kRecord><<<(unsigned)((n_items + threads - 1) / threads), threads, 0, c->stream>>>(
+                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, nbr_off, nbr,
+                    members + s.set_off[i_set], s.N, set_size, n_items, (uint32_t)s.gid0, c->orig + s.chain_off,
+                    c->decisions, c->acc_slots);
+            }
+            CU(cudaGetLastError());
+            continue;
+        }
         if (c->scheme == 1) {   // Code 1: one thread per molecule
             const size_t per_warp = sizeof(float) * 96 * (size_t)s.N;     // 32 chains x 3 coordinates
             const int warps = (int)std::min<size_t>(4, (200 * 1024) / per_warp);
@@ -461,7 +483,7 @@ void soma_destroy(soma_ctx* c)
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
-    cudaFree(c->ext); cudaFree(c->forbidden);
+    cudaFree(c->ext); cudaFree(c->forbidden); cudaFree(c->arch);
     cudaFree(c->acc_slots);
     cudaFree(c->orig); cudaFree(c->orig_tmp); cudaFree(c->scratch); cudaFree(c->stage);
     cudaFree(c->sort_keys[0]); cudaFree(c->sort_keys[1]); cudaFree(c->sort_vals[0]); cudaFree(c->sort_vals[1]);
@@ -509,7 +531,7 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
     for (int i = 0; i < n_types; ++i)
         for (int k = 0; k < n_types; ++k) c->chiN[i][k] = i == k ? 0.0f : chiN;
 
-    std::vector<uint32_t> toff_host;
+    std::vector<uint32_t> toff_host, arch_host;
     uint64_t gid = 0, off = 0;
     for (int a = 0; a < n_specs; ++a) {
         Spec s;
@@ -523,7 +545,50 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         s.gid0 = gid;
         s.off = off;
         s.toff_off = (uint32_t)toff_host.size();
-        s.fused_ok = s.N >= 4 && s.N <= 128 && (128 % s.N) == 0;
+        s.n_bonds = chains[a].n_bonds;
+        s.general = s.n_bonds > 0;
+        if (s.general) {
+            if (!chains[a].bonds) { delete c; return fail(SOMA_EINVAL, "soma_init: spec %d: n_bonds > 0 but bonds is NULL", a); }
+            // neighbour lists in ascending order, greedy first-fit independent sets (R25)
+            std::vector<std::vector<uint32_t>> nb(s.N);
+            for (uint32_t b = 0; b < s.n_bonds; ++b) {
+                const uint32_t i = chains[a].bonds[2 * b], j = chains[a].bonds[2 * b + 1];
+                if (i >= s.N || j >= s.N || i == j) {
+                    delete c;
+                    return fail(SOMA_EINVAL, "soma_init: spec %d bond %u (%u, %u): need i != j, both < n_beads", a, b, i, j);
+                }
+                nb[i].push_back(j);
+                nb[j].push_back(i);
+            }
+            std::vector<uint32_t> set_of(s.N, 0);
+            uint32_t n_sets = 0;
+            for (uint32_t j = 0; j < s.N; ++j) {
+                std::sort(nb[j].begin(), nb[j].end());
+                if (std::adjacent_find(nb[j].begin(), nb[j].end()) != nb[j].end()) {
+                    delete c;
+                    return fail(SOMA_EINVAL, "soma_init: spec %d: a bond of monomer %u is listed twice", a, j);
+                }
+                uint32_t col = 0;
+                for (bool clash = true; clash; ) {
+                    clash = false;
+                    for (uint32_t k : nb[j]) if (k < j && set_of[k] == col) clash = true;
+                    if (clash) ++col;
+                }
+                set_of[j] = col;
+                n_sets = std::max(n_sets, col + 1);
+            }
+            s.arch_off = arch_host.size();
+            uint32_t run = 0;
+            for (uint32_t j = 0; j < s.N; ++j) { arch_host.push_back(run); run += (uint32_t)nb[j].size(); }
+            arch_host.push_back(run);
+            for (uint32_t j = 0; j < s.N; ++j) for (uint32_t k : nb[j]) arch_host.push_back(k);
+            s.set_off.assign(1, 0);
+            for (uint32_t col = 0; col < n_sets; ++col) {
+                for (uint32_t j = 0; j < s.N; ++j) if (set_of[j] == col) arch_host.push_back(j);
+                s.set_off.push_back((uint32_t)(arch_host.size() - s.arch_off - (s.N + 1) - 2 * (size_t)s.n_bonds));
+            }
+        }
+        s.fused_ok = !s.general && s.N >= 4 && s.N <= 128 && (128 % s.N) == 0;
         if (s.fused_ok) {
             while ((1u << s.log2N) < s.N) ++s.log2N;
             s.n_tiles = (uint32_t)(s.n_chains * s.N / soma::kTile);
@@ -608,6 +673,10 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
     CUI(cudaMalloc(&c->counts, sizeof(uint32_t) * cells * n_types));
     CUI(cudaMalloc(&c->omega, sizeof(float) * cells * n_types));
     CUI(cudaMalloc(&c->toff, sizeof(uint32_t) * toff_host.size()));
+    if (!arch_host.empty()) {
+        CUI(cudaMalloc(&c->arch, sizeof(uint32_t) * arch_host.size()));
+        CUI(cudaMemcpyAsync(c->arch, arch_host.data(), sizeof(uint32_t) * arch_host.size(), cudaMemcpyHostToDevice, c->stream));
+    }
     CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads + 31) / 32 + 8)));
     CUI(cudaMalloc(&c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMallocHost(&c->acc_host, sizeof(unsigned long long) * soma::kAccSlots));
@@ -656,6 +725,10 @@ int soma_step(soma_ctx* c, int n_sweeps)
     if (n_sweeps < 0) return fail(SOMA_EINVAL, "soma_step: n_sweeps must be >= 0");
     if (c->move == 2 && !(c->smc_step > 0.0f))
         return fail(SOMA_ESTATE, "soma_step: Smart-MC selected but SOMA_OPT_SMC_STEP not set");
+    if (c->scheme == 1 || c->set_order == 1)
+        for (const Spec& s : c->specs)
+            if (s.general)
+                return fail(SOMA_ESTATE, "soma_step: architectures given by a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only");
     for (int i = 0; i < n_sweeps; ++i) {
         if (c->record)
             CU(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32), c->stream));

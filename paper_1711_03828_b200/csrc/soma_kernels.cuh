@@ -6,6 +6,7 @@
 //                         (independent sets of Fig. 1 / Code 2), neighbours by
 //                         warp shuffle, each position read and written once per sweep.
 //   generic_move_kernel   a1 or a2 for any chain length: one thread per monomer of one parity.
+//   arch_move_kernel      one independent set of a general architecture (bond lists): one thread per member
 //   molecule_move_kernel  the paper's other scheme (Code 1): one thread per molecule, N random picks
 //   histogram_kernel      a3  n_i(c), Eq. 4
 //   field_kernel          a4  omega_i(c), Eq. 12
@@ -286,20 +287,17 @@ __device__ __forceinline__ void count_follow(uint32_t* __restrict__ counts, bool
     }
 }
 
-// One whole move of one bead (generic kernel).  (x,y,z) is updated in place when accepted.
-//   (xl..),(xr..)  chain neighbours; an absent neighbour is passed as the bead itself (bond 0)
+// One whole move of one bead (generic kernels).  (x,y,z) is updated in place when accepted.
+//   (sx,sy,sz)     s = sum over the bonded neighbours of (r - r_nb), Eq. 2
 //   mf             number of bonded neighbours as float
 //   toff           type * cells, offset of this bead type's plane in omega / counts
 //   gid            global bead index = Philox counter word 0
 template <int kMove, bool kIncr>
-__device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
-                                        uint32_t* __restrict__ counts, float& x, float& y, float& z,
-                                        float xl, float yl, float zl, float xr, float yr, float zr,
-                                        float mf, uint32_t toff, uint32_t gid)
+__device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restrict__ omega,
+                                          uint32_t* __restrict__ counts, float& x, float& y, float& z,
+                                          float sx, float sy, float sz, float mf, uint32_t toff, uint32_t gid)
 {
     const Draw q = draw_move<kMove>(P, gid);
-    float sx, sy, sz;
-    bond_sum(x, y, z, xl, yl, zl, xr, yr, zr, sx, sy, sz);
     float dx = q.a, dy = q.b, dz = q.c, log_ratio = 0.0f;
     if (kMove == 2) smc_proposal(P, mf, sx, sy, sz, q, dx, dy, dz, log_ratio);
     const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
@@ -315,6 +313,18 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
     z = acc ? z2 : z;
     if (kIncr) count_follow(counts, acc, i_old, i_new);
     return acc;
+}
+
+// The same for a monomer of a linear chain, from its two chain neighbours.
+template <int kMove, bool kIncr>
+__device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
+                                        uint32_t* __restrict__ counts, float& x, float& y, float& z,
+                                        float xl, float yl, float zl, float xr, float yr, float zr,
+                                        float mf, uint32_t toff, uint32_t gid)
+{
+    float sx, sy, sz;
+    bond_sum(x, y, z, xl, yl, zl, xr, yr, zr, sx, sy, sz);
+    return mc_move_s<kMove, kIncr>(P, omega, counts, x, y, z, sx, sy, sz, mf, toff, gid);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -550,6 +560,46 @@ generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y,
         const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
         const uint32_t gid = gid0 + orig[chain] * N + j;   // the chain's identity, not its slot (soma_layout.cuh)
         acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf, toff_tab[j], gid);
+        if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
+        if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
+    }
+    const uint32_t n_acc = __popc(__ballot_sync(0xFFFFFFFFu, acc));
+    if ((threadIdx.x & 31u) == 0 && n_acc)
+        atomicAdd(acc_slots + ((t >> 5) % kAccSlots), (unsigned long long)n_acc);
+}
+
+// ------------------------------------------------------------------------------------------------
+// One independent set of a general molecular architecture (DESIGN.md
+// R25): one thread per member of set `i_set` of every molecule; the host launches the sets one after the
+// other.  The architecture is stored once per molecule type (the idea of Fig. 2) as
+// 32-bit words:  nbr_off[N + 1] | nbr[2 n_bonds] (ascending per monomer) | members[N] (set by set).
+// The bond sum s of Eq. 2 runs over the neighbour list in that order.
+// ------------------------------------------------------------------------------------------------
+template <int kMove, bool kIncr, bool kRecord>
+__global__ void __launch_bounds__(256)
+arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+                 const float* __restrict__ omega, uint32_t* __restrict__ counts,
+                 const uint32_t* __restrict__ toff_tab, const uint32_t* __restrict__ nbr_off,
+                 const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ members, uint32_t N,
+                 uint32_t set_size, uint64_t n_items, uint32_t gid0, const uint32_t* __restrict__ orig,
+                 uint32_t* __restrict__ dec_words, unsigned long long* __restrict__ acc_slots)
+{
+    const uint64_t t = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    bool acc = false;
+    if (t < n_items) {
+        const uint64_t mol = t / set_size;
+        const uint32_t j = members[(uint32_t)(t - mol * set_size)];      // monomer of this set member
+        const uint64_t base = mol * N, i = base + j;
+        float px = x[i], py = y[i], pz = z[i];
+        float sx = 0.0f, sy = 0.0f, sz = 0.0f;
+        const uint32_t a0 = nbr_off[j], a1 = nbr_off[j + 1u];
+        for (uint32_t a = a0; a < a1; ++a) {                              // other sets: not written in this launch
+            const uint64_t k = base + nbr[a];
+            const float bx = px - x[k], by = py - y[k], bz = pz - z[k];
+            if (a == a0) { sx = bx; sy = by; sz = bz; } else { sx = sx + bx; sy = sy + by; sz = sz + bz; }
+        }
+        const uint32_t gid = gid0 + orig[mol] * N + j;
+        acc = mc_move_s<kMove, kIncr>(P, omega, counts, px, py, pz, sx, sy, sz, (float)(a1 - a0), toff_tab[j], gid);
         if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
         if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
     }

@@ -11,6 +11,8 @@ def oracle_system(w: Workload, **over) -> oracle.OracleSystem:
     kw = dict(specs=[(n, np.asarray(t, dtype=np.uint8)) for n, t in w.specs], N_ref=w.N_ref,
               n_types=w.n_types, box=w.box, grid=w.grid, chiN=w.chiN, kappaN=w.kappaN, A=w.A,
               seed=w.seed, hamiltonian=0, smc_step=w.smc_step)
+    if getattr(w, "bonds", None):
+        kw["bonds"] = [None if b is None else np.asarray(b, dtype=np.uint32).reshape(-1, 2) for b in w.bonds]
     kw.update(over)
     return oracle.OracleSystem(**kw)
 

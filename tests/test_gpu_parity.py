@@ -206,6 +206,77 @@ def test_field_interval(density):
 
 
 # ---------------------------------------------------------------------------------------------
+# general molecular architectures given by bond lists
+# ---------------------------------------------------------------------------------------------
+def _star_bonds(arms, arm_len):
+    bonds = []
+    for a in range(arms):
+        prev = 0
+        for k in range(arm_len):
+            j = 1 + a * arm_len + k
+            bonds.append((prev, j))
+            prev = j
+    return tuple(bonds)
+
+
+def _tree_walk(w, seed=5):
+    """Start state that respects the bond lists: every monomer one Gaussian bond away from the lowest
+    neighbour placed before it (input generation only)."""
+    rng = np.random.default_rng(seed)
+    sigma = 1.0 / np.sqrt(3.0 * (w.N_ref - 1))
+    out = []
+    bonds = w.bonds or (None,) * len(w.specs)
+    for (n, t), bl in zip(w.specs, bonds):
+        N = len(t)
+        bl = [(j, j + 1) for j in range(N - 1)] if bl is None else bl
+        parent = {}
+        for i, j in bl:
+            lo, hi = min(i, j), max(i, j)
+            parent.setdefault(hi, lo)
+        P = np.zeros((n, N, 3))
+        P[:, 0] = rng.random((n, 3)) * np.asarray(w.box)
+        for j in range(1, N):
+            P[:, j] = P[:, parent.get(j, j - 1)] + rng.standard_normal((n, 3)) * sigma
+        out.append(P.reshape(-1, 3))
+    pos = np.concatenate(out)
+    return np.stack([np.ascontiguousarray(pos[:, a], dtype=np.float32) for a in range(3)])
+
+
+def _branched_melt(move="local", smc_step=0.0):
+    star = _star_bonds(3, 5)                                                    # 16 monomers, centre = 0
+    ring = tuple((j, (j + 1) % 7) for j in range(7))                            # odd ring: three sets
+    comb = tuple([(j, j + 1) for j in range(5)] + [(1, 6), (3, 7), (4, 8), (8, 9)])   # backbone with side chains
+    return workloads.Workload("branched", ((700, (0,) + (0,) * 5 + (1,) * 10), (301, (0, 0, 0, 1, 1, 1, 1)),
+                                           (150, (1,) * 6 + (0,) * 4), (64, workloads.diblock(32, 16))),
+                              16, 2, (4.0, 4.0, 3.0), (16, 16, 12), 18.0, 40.0, 0.1, 23, move=move, smc_step=smc_step,
+                              bonds=(star, ring, comb, None))
+
+
+@pytest.mark.parametrize("move,step", [("local", 0.0), ("smc", 0.05 / 15)])
+def test_stars_rings_and_combs(move, step):
+    w = _branched_melt(move, step)
+    lockstep(w, 5, xyz0=_tree_walk(w))
+
+
+def test_linear_chain_given_as_bonds_equals_the_fused_kernel():
+    base = workloads.c1()
+    lin = tuple((j, j + 1) for j in range(31))
+    as_bonds = workloads.Workload("C1bonds", base.specs, 32, 2, base.box, base.grid, base.chiN, base.kappaN, base.A,
+                                  base.seed, bonds=(lin,))
+    xyz0 = np.stack(workloads.gaussian_walks(base))
+    a, b = P.from_workload(base, xyz0=xyz0), P.from_workload(as_bonds, xyz0=xyz0)
+    a.step(6); b.step(6)
+    assert np.array_equal(a.positions(), b.positions())
+    assert np.array_equal(a.fields()[1], b.fields()[1]) and a.stats() == b.stats()
+    b.set_option(P.OPT_SCHEME, 1)
+    with pytest.raises(P.SomaError):
+        b.step(1)
+    a.destroy(); b.destroy()
+    with pytest.raises(P.SomaError):
+        P.Soma([(4, [0, 0, 0], [(0, 3)])], 3, 1, (1.0,) * 3, (2, 2, 2), 0.0, 0.0, 0.1, 1)   # bond to a monomer that is not there
+
+
+# ---------------------------------------------------------------------------------------------
 # molecule-parallel scheme (Code 1, PAPER.md:261-286)
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[0], workloads.small_cases()[2],

@@ -34,6 +34,7 @@ class Workload:
     move: str = "local"        # "local" | "smc"
     smc_step: float = 0.0
     note: str = ""
+    bonds: Tuple = ()          # per spec: None (linear chain) or a tuple of (i, j) monomer pairs; () = all linear
 
     @property
     def n_beads(self) -> int:
