@@ -24,7 +24,7 @@ constexpr int kMaxTypes = 8;
 constexpr int kTile = 128;          // beads per warp tile in the fused kernel (4 per lane)
 constexpr int kAccSlots = 256;      // spread slots of the accepted-moves counter
 #ifndef SOMA_FUSED_THREADS
-#define SOMA_FUSED_THREADS 128       // threads per block of the fused kernel
+#define SOMA_FUSED_THREADS 640       // threads per block of the fused kernel: one block of 20 warps per SM
 #endif
 constexpr int kFusedThreads = SOMA_FUSED_THREADS;
 #ifndef SOMA_MOL_UNROLL
@@ -33,7 +33,7 @@ constexpr int kFusedThreads = SOMA_FUSED_THREADS;
 constexpr int kMolUnroll = SOMA_MOL_UNROLL;   // attempts of the staged molecule kernel unrolled together
 
 #ifndef SOMA_FUSED_MIN_BLOCKS
-#define SOMA_FUSED_MIN_BLOCKS 5      // resident blocks per SM the fused kernel is compiled for (register cap)
+#define SOMA_FUSED_MIN_BLOCKS 1      // resident blocks per SM the fused kernel is compiled for (register cap: 96)
 #endif
 
 struct GridP {
@@ -370,7 +370,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
     const uint32_t t_begin = (uint32_t)(((uint64_t)blockIdx.x * n_tiles) / gridDim.x);
     const uint32_t t_end = (uint32_t)(((uint64_t)(blockIdx.x + 1) * n_tiles) / gridDim.x);
-    uint32_t tile = t_begin + wib;
+    // The block's tiles are handed out dynamically: the first two rounds are fixed (tile = begin + warp,
+    // + kWarps), after that a warp takes the next free tile from a shared-memory counter, one tile ahead
+    // of the prefetch.  The schedulers do not serve their warps evenly; with a fixed share per warp the
+    // favoured ones finished early and the SM ran its last tiles at low occupancy.
+    __shared__ uint32_t s_next;
+    if (threadIdx.x == 0) s_next = t_begin + 2u * kWarps;
+    __syncthreads();
+    uint32_t tile = t_begin + wib, tile_n = tile + kWarps;
     float4 X, Y, Z;
     uint32_t C = 0u;                                          // the caller's index of this lane's chain
     if (tile < t_end) {
@@ -380,13 +387,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         Z = *reinterpret_cast<const float4*>(z + i0);
         C = orig[i0 >> log2N];
     }
-    for (; tile < t_end; tile += kWarps) {
+    while (tile < t_end) {
         const uint32_t i0 = tile * kTile + 4u * lane;
         const uint32_t gid = gid0 + (C << log2N) + j0;
+        uint32_t tile_nn = 0u;
+        if (lane == 0) tile_nn = atomicAdd(&s_next, 1u);      // the tile after the next one
 
         // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
-        const uint32_t tile_n = min(tile + kWarps, t_end - 1u);
-        const uint32_t i0n = tile_n * kTile + 4u * lane;
+        const uint32_t i0n = min(tile_n, t_end - 1u) * kTile + 4u * lane;
         const float4 Xn = *reinterpret_cast<const float4*>(x + i0n);
         const float4 Yn = *reinterpret_cast<const float4*>(y + i0n);
         const float4 Zn = *reinterpret_cast<const float4*>(z + i0n);
@@ -521,6 +529,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             if ((uint32_t)(bits >> 32)) atomicOr(dec_words + (gid >> 5) + 1u, (uint32_t)(bits >> 32));
         }
         X = Xn; Y = Yn; Z = Zn; C = Cn;
+        tile = tile_n;
+        tile_n = __shfl_sync(kFull, tile_nn, 0);
     }
     n_acc = __reduce_add_sync(kFull, n_acc);
     if (lane == 0 && n_acc)
