@@ -71,12 +71,15 @@ enum {
                                    /* index of the chain's first bead, bit 31 of word 0, 1 = odd set first     */
     SOMA_OPT_FIELD_INTERVAL = 14,  /* k >= 1 (default 1): omega is refreshed after sweeps number k, 2k, ...    */
                                    /* (counted from 1); the occupation numbers are current after every sweep   */
-    SOMA_OPT_SCHEME = 15           /* 0 (default): independent sets, every particle attempted exactly once per */
+    SOMA_OPT_SCHEME = 15,          /* 0 (default): independent sets, every particle attempted exactly once per */
                                    /* sweep (Code 2); 1: molecule-parallel scheme (Code 1):   */
                                    /* every molecule picks N times one of its particles at random.  Attempt k  */
                                    /* of the chain whose first bead is f uses Philox counter word f + k: kind 4 */
                                    /* word 0 picks i = floor(w N / 2^32), kinds 1 / 2 drive the move; bit f + k */
                                    /* of soma_decisions is the outcome of that attempt                          */
+    SOMA_OPT_PDL = 16              /* 1 (default): the fused move kernel and the field kernel are launched with */
+                                   /* programmatic dependent launch, so each becomes resident while its         */
+                                   /* predecessor drains (results do not depend on it); 0: ordinary launches    */
 };
 
 /* indices of soma_kernel_times */

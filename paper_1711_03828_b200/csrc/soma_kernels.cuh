@@ -32,6 +32,9 @@ constexpr int kFusedThreads = SOMA_FUSED_THREADS;
 #endif
 constexpr int kMolUnroll = SOMA_MOL_UNROLL;   // attempts of the staged molecule kernel unrolled together
 
+#ifndef SOMA_OMEGA_NC
+#define SOMA_OMEGA_NC 0
+#endif
 #ifndef SOMA_FUSED_MIN_BLOCKS
 #define SOMA_FUSED_MIN_BLOCKS 1      // resident blocks per SM the fused kernel is compiled for (register cap: 96)
 #endif
@@ -134,6 +137,13 @@ __device__ __forceinline__ uint32_t first_set_bit(uint32_t first_gid, uint32_t s
     return w[0] >> 31;
 }
 
+// Programmatic dependent launch: a kernel launched with the programmatic-serialization attribute may
+// become resident while its predecessor in the stream still runs.  pdl_trigger() lets the successor
+// start launching; pdl_wait() returns once the predecessor grid has completed and its writes are
+// visible.  Both are no-ops in a kernel launched the ordinary way.
+__device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // top 23 bits -> float in [1, 2), exact
 __device__ __forceinline__ float u23(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
 
@@ -156,20 +166,25 @@ __device__ __forceinline__ float ex2_approx(float x)
 // in range for every input (also NaN and |t| >= 2^22, which is outside the supported domain:
 // |x_a| < 2^22 L_a, R7).
 // ------------------------------------------------------------------------------------------------
+#ifndef SOMA_FLOOR_XU
+#define SOMA_FLOOR_XU 9
+#endif
+template <bool kXU = false>
 __device__ __forceinline__ uint32_t axis_cell(float x, float inv_L, float nf, uint32_t n_minus_1)
 {
     const float t = x * inv_L;
-    const float fl = __fadd_rd(t, 12582912.0f) - 12582912.0f;
+    const float fl = kXU ? floorf(t) : __fadd_rd(t, 12582912.0f) - 12582912.0f;
     const float frac = t - fl;
     const float s = __fmaf_rd(frac, nf, 8388608.0f);
     return min(__float_as_uint(s) - 0x4B000000u, n_minus_1);
 }
 
+template <int kXU = 0>   // bit a of kXU: floor of axis a on the XU pipe (FRND) instead of the FMA pipe
 __device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, float z)
 {
-    const uint32_t cx = axis_cell(x, g.inv_L[0], g.nf[0], g.nm1[0]);
-    const uint32_t cy = axis_cell(y, g.inv_L[1], g.nf[1], g.nm1[1]);
-    const uint32_t cz = axis_cell(z, g.inv_L[2], g.nf[2], g.nm1[2]);
+    const uint32_t cx = axis_cell<(kXU & 1) != 0>(x, g.inv_L[0], g.nf[0], g.nm1[0]);
+    const uint32_t cy = axis_cell<(kXU & 2) != 0>(y, g.inv_L[1], g.nf[1], g.nm1[1]);
+    const uint32_t cz = axis_cell<(kXU & 4) != 0>(z, g.inv_L[2], g.nf[2], g.nm1[2]);
     return (cx * g.n[1] + cy) * g.n[2] + cz;
 }
 
@@ -219,8 +234,15 @@ __device__ __forceinline__ float field_delta(const float* __restrict__ omega, ui
 {
     float w_new = 0.0f, w_old = 0.0f;
     if (i_new != i_old) {
+#if SOMA_OMEGA_NC
         w_new = __ldg(omega + i_new);
         w_old = __ldg(omega + i_old);
+#else
+        // ordinary loads: with programmatic dependent launch this kernel may be resident while the field
+        // kernel still writes omega, which rules out the non-coherent path (ld.global.nc)
+        asm("ld.global.f32 %0, [%1];" : "=f"(w_new) : "l"(omega + i_new));
+        asm("ld.global.f32 %0, [%1];" : "=f"(w_old) : "l"(omega + i_old));
+#endif
     }
     return w_new - w_old;
 }
@@ -360,6 +382,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const uint32_t lane = threadIdx.x & 31u;
     const uint32_t wib = threadIdx.x >> 5;
     constexpr uint32_t kWarps = kFusedThreads / 32;
+    pdl_trigger();
+    pdl_wait();                                               // omega of the preceding field kernel
     const uint32_t j0 = (4u * lane) & n_mask;                 // monomer index of slot 0
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
     const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
@@ -411,10 +435,11 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
             const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
             const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
-            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
-            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
-            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
-            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            constexpr int kXo = SOMA_FLOOR_XU & 7, kXn = (SOMA_FLOOR_XU >> 3) & 7;
+            const uint32_t o0 = toff.x + cell_of<kXo>(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of<kXn>(P.g, x0n, y0n, z0n);
+            const uint32_t o1 = toff.y + cell_of<kXo>(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of<kXn>(P.g, x1n, y1n, z1n);
+            const uint32_t o2 = toff.z + cell_of<kXo>(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of<kXn>(P.g, x2n, y2n, z2n);
+            const uint32_t o3 = toff.w + cell_of<kXo>(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of<kXn>(P.g, x3n, y3n, z3n);
             const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
                         e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 
@@ -750,18 +775,17 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
 //     + ext_i(c) if an external field is set; +inf in forbidden cells, so that Eq. 15 makes every move
 //     into such a cell cost +inf and the Metropolis rule rejects it (R23)
 // ------------------------------------------------------------------------------------------------
+// omega of one cell from its occupation numbers n[0 .. nt)
 template <int kTypes>
-__global__ void __launch_bounds__(256)
-field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
-             const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
+__device__ __forceinline__ void field_of_cell(const FieldP& F, const uint32_t (&n)[kMaxTypes], uint32_t c,
+                                              const float* __restrict__ ext, const uint8_t* __restrict__ forbidden,
+                                              float (&w_out)[kMaxTypes])
 {
-    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= F.cells) return;
     const int nt = kTypes > 0 ? kTypes : F.n_types;
     float phi[kMaxTypes];
 #pragma unroll
     for (int i = 0; i < kMaxTypes; ++i)
-        if (i < nt) phi[i] = (float)counts[(size_t)i * F.cells + c] * F.inv_nbar;
+        if (i < nt) phi[i] = (float)n[i] * F.inv_nbar;
     float sum = phi[0];
 #pragma unroll
     for (int i = 1; i < kMaxTypes; ++i)
@@ -782,8 +806,63 @@ field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restr
         // external fields: a static type-specific field; +inf where no particle may enter
         if (ext) w = w + ext[(size_t)i * F.cells + c];
         if (forbidden && forbidden[c]) w = __int_as_float(0x7F800000);
-        omega[(size_t)i * F.cells + c] = w;
+        w_out[i] = w;
     }
+}
+
+template <int kTypes>
+__global__ void __launch_bounds__(256)
+field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
+             const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
+{
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    pdl_trigger();
+    pdl_wait();                                               // counts of the preceding move kernel
+    if (c >= F.cells) return;
+    const int nt = kTypes > 0 ? kTypes : F.n_types;
+    uint32_t n[kMaxTypes];
+    float w[kMaxTypes];
+#pragma unroll
+    for (int i = 0; i < kMaxTypes; ++i)
+        if (i < nt) n[i] = counts[(size_t)i * F.cells + c];
+    field_of_cell<kTypes>(F, n, c, ext, forbidden, w);
+#pragma unroll
+    for (int i = 0; i < kMaxTypes; ++i)
+        if (i < nt) omega[(size_t)i * F.cells + c] = w[i];
+}
+
+// The same with four consecutive cells per thread (128-bit loads and stores); needs cells % 4 == 0 so
+// that every type's plane starts 16-byte aligned.  kTypes = 1 or 2.
+template <int kTypes>
+__global__ void __launch_bounds__(256)
+field_kernel_v4(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
+                const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
+{
+    const uint32_t c = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
+    pdl_trigger();
+    pdl_wait();                                               // counts of the preceding move kernel
+    if (c >= F.cells) return;
+    uint4 n4[kTypes];
+#pragma unroll
+    for (int i = 0; i < kTypes; ++i) n4[i] = *reinterpret_cast<const uint4*>(counts + (size_t)i * F.cells + c);
+    float4 w4[kTypes];
+#pragma unroll
+    for (int e = 0; e < 4; ++e) {
+        uint32_t n[kMaxTypes];
+        float w[kMaxTypes];
+#pragma unroll
+        for (int i = 0; i < kTypes; ++i) n[i] = e == 0 ? n4[i].x : e == 1 ? n4[i].y : e == 2 ? n4[i].z : n4[i].w;
+        field_of_cell<kTypes>(F, n, c + e, ext, forbidden, w);
+#pragma unroll
+        for (int i = 0; i < kTypes; ++i) {
+            if (e == 0) w4[i].x = w[i];
+            if (e == 1) w4[i].y = w[i];
+            if (e == 2) w4[i].z = w[i];
+            if (e == 3) w4[i].w = w[i];
+        }
+    }
+#pragma unroll
+    for (int i = 0; i < kTypes; ++i) *reinterpret_cast<float4*>(omega + (size_t)i * F.cells + c) = w4[i];
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -408,6 +408,29 @@ def test_set_positions_and_sweep_counter_reproduce_a_run():
     b.destroy()
 
 
+@pytest.mark.parametrize("w", [workloads.c1(), workloads.c2(kappaN=50.0), workloads.small_cases()[3]], ids=lambda w: w.name)
+def test_programmatic_dependent_launch_changes_no_result(w):
+    """SOMA_OPT_PDL: the move and field kernels of 40 sweeps launched back to back, each resident while
+    its predecessor drains, against the same sweeps launched one by one with a synchronisation after
+    each and ordinary launches.  A field kernel that read the counts early, or a move kernel that read
+    omega early (or stale, from L1), would change the trajectory."""
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    a = P.from_workload(w, xyz0=xyz0)
+    a.set_option(P.OPT_PDL, 1)
+    a.step(40)
+    b = P.from_workload(w, xyz0=xyz0)
+    b.set_option(P.OPT_PDL, 0)
+    for _ in range(40):
+        b.step(1)
+        b.sync()
+    assert np.array_equal(a.positions(), b.positions())
+    (om_a, cnt_a), (om_b, cnt_b) = a.fields(), b.fields()
+    assert np.array_equal(cnt_a, cnt_b) and np.array_equal(om_a, om_b)
+    assert a.stats() == b.stats()
+    a.destroy()
+    b.destroy()
+
+
 def test_device_buffers_and_timing_hooks():
     import torch
     w = workloads.c1()
