@@ -129,18 +129,19 @@ static int64_t n_cells(const oracle_system *s)
 
 /* ------------------------------------------------------------------------------------------ */
 /* Pi_c of Eq. 4: the cell that contains r.  Reading R7: coordinates are      */
-/* stored unwrapped; per axis the position in units of the box length, t = fl32(x * fl32(1/L)),  */
-/* is folded by taking its fractional part frac = fl32(t - floor(t)) in [0,1] (one IEEE           */
-/* subtraction), and the cell is floor(frac * n) with the product taken exactly (24 x 24 bits fit */
-/* a double), clamped to n-1 because frac may round up to 1.                                      */
+/* stored unwrapped; per axis the position in units of the box length is the fp32 number         */
+/* t = fl32(x * fl32(1/L)), and the cell is floor(t n) mod n = floor(t n) - n floor(t), both      */
+/* floors taken of the exact values (t has 24 significant bits and n < 2^24, so the product is    */
+/* exact in a double): half-open cells [i, i+1) DeltaL, periodic, no rounding after t.           */
+/* Supported domain |t n| < 2^22.                                                                 */
 /* ------------------------------------------------------------------------------------------ */
 static int32_t axis_cell(float x, float L, int32_t n)
 {
     const float inv_L = (float)(1.0 / (double)L);
     const float t = x * inv_L;
-    const float frac = t - floorf(t);
-    const int32_t i = (int32_t)floor((double)frac * (double)n);
-    return i < n - 1 ? i : n - 1;
+    const double k = floor((double)t * (double)n); /* exact product, exact floor */
+    const double m = floor((double)t);
+    return (int32_t)(k - (double)n * m);           /* in 0 .. n-1 */
 }
 
 int64_t soma_oracle_cell_index(const oracle_system *s, float x, float y, float z)

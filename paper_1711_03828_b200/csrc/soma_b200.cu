@@ -141,8 +141,11 @@ soma::GridP soma_ctx::gridp() const
         g.inv_L[a] = (float)(1.0 / (double)box[a]);
         g.nf[a] = (float)grid[a];
         g.n[a] = (uint32_t)grid[a];
-        g.nm1[a] = (uint32_t)grid[a] - 1u;
+        g.neg_n[a] = 0u - (uint32_t)grid[a];
     }
+    const uint32_t Mb = 0x4B400000u;   // bits of 1.5 * 2^23
+    const uint32_t Kx = (g.n[0] - 1u) * Mb, Ky = (g.n[1] - 1u) * Mb, Kz = (g.n[2] - 1u) * Mb;
+    g.k_tot = (Kx * g.n[1] + Ky) * g.n[2] + Kz;
     g.cells = (uint32_t)cells;
     return g;
 }

@@ -43,7 +43,8 @@ struct GridP {
     float inv_L[3];   // fl32(1 / L_a)
     float nf[3];      // (float) n_a
     uint32_t n[3];
-    uint32_t nm1[3];  // n_a - 1
+    uint32_t neg_n[3];  // -n_a (mod 2^32)
+    uint32_t k_tot;     // ((K_x n_y + K_y) n_z + K_z) mod 2^32, K_a = (n_a - 1) 0x4B400000: see cell_of()
     uint32_t cells;
 };
 
@@ -155,37 +156,32 @@ __device__ __forceinline__ float ex2_approx(float x)
 }
 
 // ------------------------------------------------------------------------------------------------
-// Pi_c of Eq. 4: the cell that contains r, periodic.  Per axis: position in
-// units of the box length t = x * (1/L), folded by its fractional part frac = t - floor(t), cell =
-// floor(frac * n) (exact product) clamped to n-1.
-// FRND and F2I run on the XU pipe (16 lanes/clk/SM, shared with MUFU) and saturated it in the first
-// version of this kernel, so floor and float->int are done on the FMA/ALU pipes instead:
-//   floor(t)       = fl_down(t + 1.5 * 2^23) - 1.5 * 2^23     exact for |t| < 2^22
-//   floor(frac n)  = mantissa of fl_down(frac * n + 2^23)      exact for frac * n < 2^23
-// FMUL, FADD.RM, FADD, FADD, FFMA.RM, IADD, VIMNMX.U32 per axis.  The unsigned min keeps the index
-// in range for every input (also NaN and |t| >= 2^22, which is outside the supported domain:
-// |x_a| < 2^22 L_a, R7).
+// Pi_c of Eq. 4: the cell that contains r, periodic (R7).  Per axis the
+// position in units of the box length is the fp32 number t = x * (1/L); the cell is
+//   floor(t n) mod n = floor(t n) - n floor(t),
+// both floors of the exact values.  Both come out of one instruction each, as the low mantissa bits of
+//   A = fl_down(t + 1.5 * 2^23)        bits(A) = 0x4B400000 + floor(t)
+//   B = fl_down(t * n + 1.5 * 2^23)    bits(B) = 0x4B400000 + floor(t n)     (FFMA: exact product)
+// exact for |t n| < 2^22 (the supported domain).  With K_a = (n_a - 1) 0x4B400000 the cell of axis a is
+// bits(B) - n_a bits(A) + K_a in 32-bit wrap-around arithmetic; the three constants are folded into one,
+//   cell = ((cx ny + cy) nz + cz) = (((Bx - nx Ax) ny + By - ny Ay) nz + Bz - nz Az) + k_tot,
+// five IMADs.  FMUL, FADD.RM, FFMA.RM per axis; no FRND / F2I (XU pipe), no fold of the fraction, no
+// per-axis clamp.  The final unsigned min keeps the index inside the grid for every input (NaN, or
+// coordinates outside the domain).
 // ------------------------------------------------------------------------------------------------
-#ifndef SOMA_FLOOR_XU
-#define SOMA_FLOOR_XU 9
-#endif
-template <bool kXU = false>
-__device__ __forceinline__ uint32_t axis_cell(float x, float inv_L, float nf, uint32_t n_minus_1)
-{
-    const float t = x * inv_L;
-    const float fl = kXU ? floorf(t) : __fadd_rd(t, 12582912.0f) - 12582912.0f;
-    const float frac = t - fl;
-    const float s = __fmaf_rd(frac, nf, 8388608.0f);
-    return min(__float_as_uint(s) - 0x4B000000u, n_minus_1);
-}
-
-template <int kXU = 0>   // bit a of kXU: floor of axis a on the XU pipe (FRND) instead of the FMA pipe
 __device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, float z)
 {
-    const uint32_t cx = axis_cell<(kXU & 1) != 0>(x, g.inv_L[0], g.nf[0], g.nm1[0]);
-    const uint32_t cy = axis_cell<(kXU & 2) != 0>(y, g.inv_L[1], g.nf[1], g.nm1[1]);
-    const uint32_t cz = axis_cell<(kXU & 4) != 0>(z, g.inv_L[2], g.nf[2], g.nm1[2]);
-    return (cx * g.n[1] + cy) * g.n[2] + cz;
+    const float M = 12582912.0f;
+    const float tx = x * g.inv_L[0], ty = y * g.inv_L[1], tz = z * g.inv_L[2];
+    const uint32_t ax = __float_as_uint(__fadd_rd(tx, M)), bx = __float_as_uint(__fmaf_rd(tx, g.nf[0], M));
+    const uint32_t ay = __float_as_uint(__fadd_rd(ty, M)), by = __float_as_uint(__fmaf_rd(ty, g.nf[1], M));
+    const uint32_t az = __float_as_uint(__fadd_rd(tz, M)), bz = __float_as_uint(__fmaf_rd(tz, g.nf[2], M));
+    uint32_t u = ax * g.neg_n[0] + bx;
+    u = u * g.n[1] + by;
+    u = ay * g.neg_n[1] + u;
+    u = u * g.n[2] + bz;
+    u = az * g.neg_n[2] + u;
+    return min(u + g.k_tot, g.cells - 1u);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -435,11 +431,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
             const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
             const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
-            constexpr int kXo = SOMA_FLOOR_XU & 7, kXn = (SOMA_FLOOR_XU >> 3) & 7;
-            const uint32_t o0 = toff.x + cell_of<kXo>(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of<kXn>(P.g, x0n, y0n, z0n);
-            const uint32_t o1 = toff.y + cell_of<kXo>(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of<kXn>(P.g, x1n, y1n, z1n);
-            const uint32_t o2 = toff.z + cell_of<kXo>(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of<kXn>(P.g, x2n, y2n, z2n);
-            const uint32_t o3 = toff.w + cell_of<kXo>(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of<kXn>(P.g, x3n, y3n, z3n);
+            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
+            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
+            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
             const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
                         e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 

@@ -145,7 +145,8 @@ def test_ragged_last_tile_of_the_fused_kernel():
 def test_unwrapped_coordinates_far_from_the_origin():
     w = workloads.c1()
     x, y, z = workloads.gaussian_walks(w)
-    xyz0 = np.stack([x - 37 * 4.0, y + 1000 * 4.0, z + 5.0e6]).astype(np.float32)   # |i_z| > 2^22: integer fold path
+    # z: t n = 4.0e6, just inside the supported domain |t n| < 2^22 (reading R7); x: negative images
+    xyz0 = np.stack([x - 37 * 4.0, y + 1000 * 4.0, z + 1.0e6]).astype(np.float32)
     lockstep(w, 3, xyz0=xyz0)
 
 

@@ -374,6 +374,37 @@ def test_histogram_sum_rules_and_brute_force():
     assert s.cell_index(float(x[0]), float(y[0]), float(z[0])) == _cell_f64(p64[0], box, grid)
 
 
+def test_cell_index_is_the_exact_floor_of_the_fp32_box_coordinate():
+    """Reading R7: per axis t = fl32(x * fl32(1/L)); cell = floor(t n) mod n in exact arithmetic.  Checked
+    with Python rationals (no floating point after t) on random coordinates over many periodic images,
+    on coordinates on and next to cell faces and box faces, on tiny negative coordinates (which belong to
+    the last cell, never to a cell 'n'), and far from the origin."""
+    from fractions import Fraction
+    box, grid = (3.0, 2.0, 2.5), (6, 5, 7)
+    s = OracleSystem(specs=[(1, np.zeros(1, np.uint8))], N_ref=1, n_types=1, box=box, grid=grid, seed=1)
+    rng = np.random.default_rng(5)
+    xs = [rng.uniform(-40.0, 40.0, 4000).astype(np.float32)]
+    faces = np.arange(-30, 31, dtype=np.float64)[:, None] * 0.5 / np.array([1.0, 2.0, 3.0, 6.0])[None, :]
+    f32 = faces.astype(np.float32).ravel()
+    xs += [f32, np.nextafter(f32, np.float32(np.inf)), np.nextafter(f32, np.float32(-np.inf))]
+    xs += [np.array([-1e-30, -1e-10, -2.0 ** -25, -0.0, 0.0, 1e-30, 2.0 ** -25], np.float32)]
+    xs += [rng.uniform(-3.0e5, 3.0e5, 2000).astype(np.float32)]
+    xs = np.concatenate(xs)
+
+    def axis(xv, L, n):
+        inv_L = np.float32(1.0 / L)
+        t = Fraction(float(np.float32(xv) * inv_L))          # the fp32 product, then exact
+        return math.floor(t * n) % n
+
+    for i, xv in enumerate(xs):
+        yv, zv = xs[(7 * i + 3) % len(xs)], xs[(13 * i + 5) % len(xs)]
+        want = (axis(xv, box[0], grid[0]) * grid[1] + axis(yv, box[1], grid[1])) * grid[2] + axis(zv, box[2], grid[2])
+        assert s.cell_index(float(xv), float(yv), float(zv)) == want, (xv, yv, zv)
+    # the two statements the definition is chosen for
+    assert s.cell_index(-1e-30, 0.0, 0.0) == (grid[0] - 1) * grid[1] * grid[2]      # just below 0: last cell
+    assert s.cell_index(0.5, 0.0, 0.0) == 1 * grid[1] * grid[2]                      # on a face: the upper cell
+
+
 def test_homogeneous_melt_mean_occupancy():
     """Mean occupancy = rho_0 DeltaL^3 = beads/cells: 16 for the C1 melt."""
     from workloads import c1, gaussian_walks
