@@ -147,6 +147,7 @@ soma::GridP soma_ctx::gridp() const
     const uint32_t Kx = (g.n[0] - 1u) * Mb, Ky = (g.n[1] - 1u) * Mb, Kz = (g.n[2] - 1u) * Mb;
     g.k_tot = (Kx * g.n[1] + Ky) * g.n[2] + Kz;
     g.cells = (uint32_t)cells;
+    g.last = (uint32_t)(cells * (size_t)n_types) - 1u;
     return g;
 }
 

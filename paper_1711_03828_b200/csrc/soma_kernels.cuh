@@ -44,8 +44,9 @@ struct GridP {
     float nf[3];      // (float) n_a
     uint32_t n[3];
     uint32_t neg_n[3];  // -n_a (mod 2^32)
-    uint32_t k_tot;     // ((K_x n_y + K_y) n_z + K_z) mod 2^32, K_a = (n_a - 1) 0x4B400000: see cell_of()
+    uint32_t k_tot;     // ((K_x n_y + K_y) n_z + K_z) mod 2^32, K_a = (n_a - 1) 0x4B400000: see cell_raw()
     uint32_t cells;
+    uint32_t last;      // n_types * cells - 1: the last valid index of omega / counts
 };
 
 struct MoveP {
@@ -166,10 +167,11 @@ __device__ __forceinline__ float ex2_approx(float x)
 // bits(B) - n_a bits(A) + K_a in 32-bit wrap-around arithmetic; the three constants are folded into one,
 //   cell = ((cx ny + cy) nz + cz) = (((Bx - nx Ax) ny + By - ny Ay) nz + Bz - nz Az) + k_tot,
 // five IMADs.  FMUL, FADD.RM, FFMA.RM per axis; no FRND / F2I (XU pipe), no fold of the fraction, no
-// per-axis clamp.  The final unsigned min keeps the index inside the grid for every input (NaN, or
-// coordinates outside the domain).
+// per-axis clamp.  cell_raw() returns the sum without k_tot; cell_at() adds k_tot and the offset of the
+// bead type's plane in omega / counts (toff = type * cells) in one go, and its unsigned min keeps the
+// index inside the arrays for every input (NaN, or coordinates outside the domain).
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, float z)
+__device__ __forceinline__ uint32_t cell_raw(const GridP& g, float x, float y, float z)
 {
     const float M = 12582912.0f;
     const float tx = x * g.inv_L[0], ty = y * g.inv_L[1], tz = z * g.inv_L[2];
@@ -181,7 +183,13 @@ __device__ __forceinline__ uint32_t cell_of(const GridP& g, float x, float y, fl
     u = ay * g.neg_n[1] + u;
     u = u * g.n[2] + bz;
     u = az * g.neg_n[2] + u;
-    return min(u + g.k_tot, g.cells - 1u);
+    return u;
+}
+
+// toff_k = toff + k_tot
+__device__ __forceinline__ uint32_t cell_at(const GridP& g, float x, float y, float z, uint32_t toff_k)
+{
+    return min(cell_raw(g, x, y, z) + toff_k, g.last);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -319,8 +327,8 @@ __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restric
     float dx = q.a, dy = q.b, dz = q.c, log_ratio = 0.0f;
     if (kMove == 2) smc_proposal(P, mf, sx, sy, sz, q, dx, dy, dz, log_ratio);
     const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
-    const uint32_t i_old = toff + cell_of(P.g, x, y, z);
-    const uint32_t i_new = toff + cell_of(P.g, x2, y2, z2);
+    const uint32_t i_old = cell_at(P.g, x, y, z, toff + P.g.k_tot);
+    const uint32_t i_new = cell_at(P.g, x2, y2, z2, toff + P.g.k_tot);
     const float e_nb = field_delta(omega, i_old, i_new);
     const float e_b = bonded_delta(kMove == 1 ? P.hk : 0.5f * P.k0, mf, dx, dy, dz, sx, sy, sz);
     float dE = e_b + e_nb;
@@ -384,6 +392,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
     const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
     const uint4 toff = *reinterpret_cast<const uint4*>(toff_tab + j0);
+    const uint4 tk = make_uint4(toff.x + P.g.k_tot, toff.y + P.g.k_tot, toff.z + P.g.k_tot, toff.w + P.g.k_tot);
     const float mf0 = has_l0 ? 2.0f : 1.0f, mf3 = has_r3 ? 2.0f : 1.0f;
     const float half_k0 = kMove == 1 ? P.hk : 0.5f * P.k0;
     uint32_t n_acc = 0;
@@ -431,10 +440,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
             const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
             const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
-            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
-            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
-            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
-            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const uint32_t o0 = cell_at(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at(P.g, x0n, y0n, z0n, tk.x);
+            const uint32_t o1 = cell_at(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at(P.g, x1n, y1n, z1n, tk.y);
+            const uint32_t o2 = cell_at(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at(P.g, x2n, y2n, z2n, tk.z);
+            const uint32_t o3 = cell_at(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at(P.g, x3n, y3n, z3n, tk.w);
             const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
                         e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 
@@ -508,8 +517,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, 2.0f, sx2, sy2, sz2, q2, dx2, dy2, dz2, lr2);
             const float x0n = X.x + dx0, y0n = Y.x + dy0, z0n = Z.x + dz0;
             const float x2n = X.z + dx2, y2n = Y.z + dy2, z2n = Z.z + dz2;
-            const uint32_t o0 = toff.x + cell_of(P.g, X.x, Y.x, Z.x), n0 = toff.x + cell_of(P.g, x0n, y0n, z0n);
-            const uint32_t o2 = toff.z + cell_of(P.g, X.z, Y.z, Z.z), n2 = toff.z + cell_of(P.g, x2n, y2n, z2n);
+            const uint32_t o0 = cell_at(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at(P.g, x0n, y0n, z0n, tk.x);
+            const uint32_t o2 = cell_at(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at(P.g, x2n, y2n, z2n, tk.z);
             const float e0 = field_delta(omega, o0, n0), e2 = field_delta(omega, o2, n2);
             a0 = metropolis((bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0) + e0) + lr0, q0.u);
             a2 = metropolis((bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2) + e2) + lr2, q2.u);
@@ -526,8 +535,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, mf3, sx3, sy3, sz3, q3, dx3, dy3, dz3, lr3);
             const float x1n = X.y + dx1, y1n = Y.y + dy1, z1n = Z.y + dz1;
             const float x3n = X.w + dx3, y3n = Y.w + dy3, z3n = Z.w + dz3;
-            const uint32_t o1 = toff.y + cell_of(P.g, X.y, Y.y, Z.y), n1 = toff.y + cell_of(P.g, x1n, y1n, z1n);
-            const uint32_t o3 = toff.w + cell_of(P.g, X.w, Y.w, Z.w), n3 = toff.w + cell_of(P.g, x3n, y3n, z3n);
+            const uint32_t o1 = cell_at(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at(P.g, x1n, y1n, z1n, tk.y);
+            const uint32_t o3 = cell_at(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at(P.g, x3n, y3n, z3n, tk.w);
             const float e1 = field_delta(omega, o1, n1), e3 = field_delta(omega, o3, n3);
             a1 = metropolis((bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1) + e1) + lr1, q1.u);
             a3 = metropolis((bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3) + e3) + lr3, q3.u);
@@ -759,7 +768,7 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
     const uint32_t stride = gridDim.x * blockDim.x;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {
         const uint32_t j = i % N;
-        atomicAdd(counts + toff_tab[j] + cell_of(g, x[i], y[i], z[i]), 1u);
+        atomicAdd(counts + cell_at(g, x[i], y[i], z[i], toff_tab[j] + g.k_tot), 1u);
     }
 }
 
