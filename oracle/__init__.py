@@ -61,6 +61,8 @@ class _System(C.Structure):
         ("bonds", C.POINTER(C.c_uint32)),
         ("ext_field", C.POINTER(C.c_float)),
         ("forbidden", C.POINTER(C.c_uint8)),
+        ("spec_first_bead", C.POINTER(C.c_uint64)),
+        ("global_n_beads", C.c_uint64),
     ]
 
 
@@ -191,6 +193,8 @@ class OracleSystem:
     scheme: int = 0             # 0: independent sets (Code 2); 1: molecule-parallel random picks (Code 1)
     ext_field: Optional[np.ndarray] = None    # (n_types, n_cells) float32 static field added to omega
     forbidden: Optional[np.ndarray] = None    # (n_cells,) uint8, 1 = no particle may enter the cell
+    spec_first_bead: Optional[Sequence[int]] = None   # this system is a part of a larger one: index in the whole system
+    global_n_beads: int = 0                            # of each architecture's first bead; beads of the whole system
     _keep: list = field(default_factory=list, repr=False)
 
     def __post_init__(self):
@@ -252,6 +256,12 @@ class OracleSystem:
             s.forbidden = self._forb.ctypes.data_as(C.POINTER(C.c_uint8))
         else:
             s.forbidden = C.POINTER(C.c_uint8)()
+        if self.spec_first_bead is not None:
+            self._first = np.ascontiguousarray(self.spec_first_bead, dtype=np.uint64)
+            s.spec_first_bead = self._first.ctypes.data_as(C.POINTER(C.c_uint64))
+        else:
+            s.spec_first_bead = C.POINTER(C.c_uint64)()
+        s.global_n_beads = int(self.global_n_beads)
 
     # -- sizes -------------------------------------------------------------------------------
     @property

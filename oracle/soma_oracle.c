@@ -66,6 +66,10 @@ typedef struct {
     const uint32_t *bonds;         /* concatenated (i, j) monomer pairs of the architectures with bonds  */
     const float    *ext_field;     /* nullable, [n_types][cells]: static external field added to omega   */
     const uint8_t  *forbidden;     /* nullable, [cells]: 1 = no particle may enter this cell             */
+    /* A part of a larger system (molecules distributed over ranks).  nullable:         */
+    const uint64_t *spec_first_bead; /* [n_specs] index in the whole system of the first bead of this part's */
+                                   /* molecules of each architecture = their Philox counter words (R3)    */
+    uint64_t        global_n_beads; /* beads of the whole system (rho_0 of Eq. 12); 0: this system is whole */
 } oracle_system;
 
 /* ------------------------------------------------------------------------------------------ */
@@ -202,7 +206,8 @@ void soma_oracle_fields(const oracle_system *s, const uint32_t *counts, float *o
     int64_t allowed = cells;
     if (s->forbidden)
         for (int64_t c = 0; c < cells; ++c) allowed -= s->forbidden[c] ? 1 : 0;
-    const float inv_nbar = (float)((double)allowed / (double)soma_oracle_n_beads(s));
+    const uint64_t beads_all = s->global_n_beads ? s->global_n_beads : soma_oracle_n_beads(s);
+    const float inv_nbar = (float)((double)allowed / (double)beads_all);
     const float kappa0 = (float)((double)s->kappaN / (double)s->N_ref);
     float chi0[ORACLE_MAX_TYPES][ORACLE_MAX_TYPES], half_chi0[ORACLE_MAX_TYPES][ORACLE_MAX_TYPES];
     for (uint32_t i = 0; i < nt; ++i)
@@ -573,20 +578,22 @@ uint64_t soma_oracle_sweep(const oracle_system *s, float *x, float *y, float *z,
             types += N;
             continue;
         }
+        /* a part of a larger system draws the numbers of its beads' indices in the whole system */
+        const uint64_t rng_shift = s->spec_first_bead ? s->spec_first_bead[a] - spec_first_bead : 0;
 #ifdef _OPENMP
 #pragma omp parallel for schedule(static) reduction(+ : accepted)
 #endif
         for (int64_t mol = 0; mol < n_mol; ++mol) {
             const uint64_t first = spec_first_bead + (uint64_t)mol * N;
-            const uint32_t first_set = soma_oracle_first_set(s, first, sweep);
+            const uint32_t first_set = soma_oracle_first_set(s, first + rng_shift, sweep);
             for (uint32_t k_set = 0; k_set < 2; ++k_set) {      /* the two sets, one after the other */
                 const uint32_t i_set = k_set ^ first_set;       /* set_permutation[k_set]            */
                 for (uint32_t ip = i_set; ip < N; ip += 2) {     /* members of the set                */
                     const uint64_t bead = first + ip;
                     const int has_l = ip > 0, has_r = ip + 1 < N;
                     const int acc = move_kind == 2
-                        ? mc_smc(s, x, y, z, omega, bead, bead, has_l, has_r, types[ip], sweep)
-                        : mc_local(s, x, y, z, omega, bead, bead, has_l, has_r, types[ip], sweep);
+                        ? mc_smc(s, x, y, z, omega, bead, bead + rng_shift, has_l, has_r, types[ip], sweep)
+                        : mc_local(s, x, y, z, omega, bead, bead + rng_shift, has_l, has_r, types[ip], sweep);
                     accepted += (uint64_t)acc;
                     if (decisions) decisions[bead] = (uint8_t)acc;
                 }
