@@ -145,6 +145,10 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", type=int, default=0)
     ap.add_argument("--density", type=int, default=0)
+    ap.add_argument("--sharded", action="store_true",
+                    help="N > 1: ONE system of N x the config's chains in a box N x as long (same density), molecules "
+                         "distributed over the ranks, one all-reduce of the occupation numbers per sweep (SURVEY 8(e)); "
+                         "default: N independent replicas")
     args = ap.parse_args()
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3   # timing rule: W >= 3
@@ -187,11 +191,36 @@ def main():
         torch.cuda.synchronize()
 
     from dataclasses import replace
-    wr = w if rank == 0 else replace(w, seed=w.seed + rank)   # independent replicas
-    sim = P.from_workload(wr, xyz0=None)       # Gaussian-walk start drawn on the device from the seed
+    if args.sharded:
+        # weak scaling of one system: world x the chains in a box world x as long along x (same density, same
+        # cell size); every rank moves 1/world of the molecules and holds the whole grid
+        from paper_1711_03828_b200.sharded import ShardedSoma
+        w = replace(w, specs=tuple((n * world, t) for n, t in w.specs), box=(w.box[0] * world, w.box[1], w.box[2]),
+                    grid=(w.grid[0] * world, w.grid[1], w.grid[2]))
+        config.update({"parallelism": f"one system over {world} GPU(s): molecules distributed, counts all-reduced every sweep",
+                       "chains": w.n_chains, "beads": w.n_beads, "grid": list(w.grid), "box": list(w.box)})
+
+        class _Sharded:                       # the calls bench makes, on this rank's part of the system
+            def __init__(self, sh):
+                self.sh, self.sim = sh, sh.sim
+
+            def step(self, n):
+                self.sh.step(n)
+
+            def set_positions(self, xyz):
+                self.sim.set_positions(xyz)
+                self.sh._exchange(advance=False)
+
+            def __getattr__(self, name):
+                return getattr(self.sim, name)
+
+        sim = _Sharded(ShardedSoma(w, dist=dist))
+    else:
+        wr = w if rank == 0 else replace(w, seed=w.seed + rank)   # independent replicas
+        sim = P.from_workload(wr, xyz0=None)       # Gaussian-walk start drawn on the device from the seed
     sim.set_option(P.OPT_KERNEL, args.kernel)
     sim.set_option(P.OPT_DENSITY, args.density)
-    nb = w.n_beads
+    nb = sim.n_beads                           # beads this rank moves
 
     # ---- device-resident throughput ------------------------------------------------------------
     sim.step(args.warmup)

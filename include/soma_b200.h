@@ -122,6 +122,39 @@ int soma_init(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_
               const float *box, const int *grid, float chiN, float kappaN, float A, uint64_t seed,
               const float *host_xyz0, void *cuda_stream);
 
+/* Several GPUs ("molecules are distributed among the MPI ranks", every rank keeps the
+ * whole grid, the densities are summed over the ranks after every MC step).  A rank
+ * creates a context from its own molecules and says where they sit in the whole system:
+ *   spec_first_bead  host, [n_specs]: index, in the whole system's bead numbering, of the first bead of
+ *                    this rank's molecules of each architecture.  It is the Philox counter word of that
+ *                    bead, so a shard draws exactly the numbers the undivided system draws for these
+ *                    molecules (and the decision bitmap is indexed by it: soma_decisions then returns
+ *                    ceil(global_n_beads / 32) words)
+ *   global_n_beads   beads of the whole system (< 2^32): rho_0 of Eq. 12 is global_n_beads / volume
+ * All other arguments as for soma_init, describing this rank's molecules only (host_xyz0: their
+ * positions, or NULL to draw them as the undivided system would).  The context comes back with its
+ * local occupation numbers (soma_fields(ctx, NULL, counts, ..)) but WITHOUT omega: sum the counts of all
+ * ranks (integers: any order, any collective) and call soma_shard_fields(.., advance = 0).  Then, per
+ * MC step: soma_shard_moves; sum the counts of all ranks; soma_shard_fields(.., advance = 1).  The
+ * positions, occupation numbers and fields equal those of the undivided system bit for bit.  soma_step
+ * returns SOMA_ESTATE on such a context; soma_set_positions / soma_set_chi / soma_set_external / the
+ * Hamiltonian option leave omega to the next soma_shard_fields. */
+int soma_init_shard(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_ref, int n_types,
+                    const float *box, const int *grid, float chiN, float kappaN, float A, uint64_t seed,
+                    const float *host_xyz0, void *cuda_stream, const uint64_t *spec_first_bead,
+                    uint64_t global_n_beads);
+
+/* The moves of one sweep (a1, a2 | a5) of this rank's molecules in the current omega; the local
+ * occupation numbers follow (a3).  Asynchronous on the context's stream. */
+int soma_shard_moves(soma_ctx *ctx);
+
+/* a4: omega from the occupation numbers of the whole system (uint32 [n_types][cells], host or device;
+ * a device array is read in place by the field kernel and must stay untouched until the stream has
+ * passed it).  advance != 0 closes the sweep begun by soma_shard_moves (sweep counter + 1, and omega is
+ * only recomputed when SOMA_OPT_FIELD_INTERVAL says so); advance = 0: stage 1 after soma_init_shard or
+ * soma_set_positions. */
+int soma_shard_fields(soma_ctx *ctx, const uint32_t *global_counts, int src_is_device, int advance);
+
 /* n_sweeps SCMF cycles: (a1, a2 | a5), a3, a4 each.  Asynchronous on the context's stream.
  * The sweep counter advances by n_sweeps. */
 int soma_step(soma_ctx *ctx, int n_sweeps);

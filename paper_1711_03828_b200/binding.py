@@ -27,7 +27,7 @@ SYMBOLS = (
     "soma_init", "soma_step", "soma_fields", "soma_positions", "soma_set_positions", "soma_set_chi",
     "soma_set_external", "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
-    "soma_version",
+    "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields",
 )
 
 
@@ -55,6 +55,9 @@ def load() -> C.CDLL:
     vp, i32, u64 = C.c_void_p, C.c_int, C.c_uint64
     L.soma_init.argtypes = [C.POINTER(vp), C.POINTER(_ChainSpec), i32, i32, i32, C.POINTER(C.c_float),
                             C.POINTER(C.c_int), C.c_float, C.c_float, C.c_float, u64, vp, vp]
+    L.soma_init_shard.argtypes = L.soma_init.argtypes + [C.POINTER(u64), u64]
+    L.soma_shard_moves.argtypes = [vp]
+    L.soma_shard_fields.argtypes = [vp, vp, i32, i32]
     L.soma_step.argtypes = [vp, i32]
     L.soma_fields.argtypes = [vp, vp, vp, i32]
     L.soma_positions.argtypes = [vp, vp, i32]
@@ -101,7 +104,8 @@ class Soma:
 
     def __init__(self, specs: Sequence[Tuple[int, Sequence[int]]], N_ref: int, n_types: int,
                  box: Sequence[float], grid: Sequence[int], chiN: float, kappaN: float, A: float,
-                 seed: int, xyz0: Optional[np.ndarray] = None, stream: Optional[int] = None):
+                 seed: int, xyz0: Optional[np.ndarray] = None, stream: Optional[int] = None,
+                 spec_first_bead: Optional[Sequence[int]] = None, global_n_beads: int = 0):
         L = load()
         self._L = L
         self._h = C.c_void_p()
@@ -128,9 +132,14 @@ class Soma:
         if xyz0 is not None:
             xyz0 = np.ascontiguousarray(xyz0, dtype=np.float32)
             p0 = xyz0.ctypes.data
-        _check(L.soma_init(C.byref(self._h), arr, len(specs), int(N_ref), int(n_types), cbox, cgrid,
-                           C.c_float(chiN), C.c_float(kappaN), C.c_float(A), C.c_uint64(int(seed)),
-                           C.c_void_p(p0), C.c_void_p(stream or None)))
+        args = (C.byref(self._h), arr, len(specs), int(N_ref), int(n_types), cbox, cgrid, C.c_float(chiN),
+                C.c_float(kappaN), C.c_float(A), C.c_uint64(int(seed)), C.c_void_p(p0), C.c_void_p(stream or None))
+        if spec_first_bead is None:
+            _check(L.soma_init(*args))
+        else:   # this rank's molecules of a system spread over several GPUs (soma_init_shard)
+            first = (C.c_uint64 * len(specs))(*[int(v) for v in spec_first_bead])
+            _check(L.soma_init_shard(*args, first, C.c_uint64(int(global_n_beads))))
+        self.n_beads_global = int(global_n_beads) if spec_first_bead is not None else None
         self.n_beads = int(L.soma_n_beads(self._h))
         self.n_cells = int(L.soma_n_cells(self._h))
         self.n_types = int(L.soma_n_types(self._h))
@@ -138,6 +147,13 @@ class Soma:
     # -- the C ABI, one method per entry point -------------------------------------------------
     def step(self, n_sweeps: int = 1) -> None:
         _check(self._L.soma_step(self._h, int(n_sweeps)))
+
+    def shard_moves(self) -> None:
+        _check(self._L.soma_shard_moves(self._h))
+
+    def shard_fields(self, global_counts, advance: bool = True) -> None:
+        p, dev = _ptr(global_counts)
+        _check(self._L.soma_shard_fields(self._h, C.c_void_p(p), int(dev), int(bool(advance))))
 
     def fields(self, omega=None, counts=None):
         """Copy omega (and counts) out. With no arguments returns new host numpy arrays."""
@@ -183,7 +199,7 @@ class Soma:
 
     def decisions(self, bits=None):
         if bits is None:
-            bits = np.empty((self.n_beads + 31) // 32, np.uint32)
+            bits = np.empty(((self.n_beads_global or self.n_beads) + 31) // 32, np.uint32)
         p, dev = _ptr(bits)
         _check(self._L.soma_decisions(self._h, C.c_void_p(p), int(dev)))
         return bits

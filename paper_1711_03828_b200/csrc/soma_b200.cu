@@ -54,6 +54,7 @@ struct Spec {
     uint64_t n_chains = 0;
     uint32_t N = 0;
     uint64_t n_beads = 0;   // n_chains * N
+    uint64_t local0 = 0;    // index of the architecture's first bead in the caller's arrays (= gid0 unless sharded)
     uint64_t gid0 = 0;      // global index of the first bead (unpadded, the API's bead index)
     uint64_t off = 0;       // offset of the segment in the padded device arrays
     uint32_t toff_off = 0;  // offset into the toff table
@@ -81,6 +82,9 @@ struct soma_ctx {
     float kappaN = 0, A = 0;
     uint64_t seed = 0;
     uint64_t n_beads = 0, n_pad = 0, cells = 0;
+    uint64_t n_beads_global = 0;     // beads of the whole system (= n_beads unless this context is a shard)
+    int sharded = 0;                 // created by soma_init_shard: soma_shard_moves / soma_shard_fields instead of soma_step
+    uint32_t* counts_global = nullptr;   // staging for soma_shard_fields from a host array (allocated on first use)
 
     float *x = nullptr, *y = nullptr, *z = nullptr;
     uint32_t* counts = nullptr;
@@ -185,7 +189,7 @@ soma::MoveP soma_ctx::movep(uint64_t sweep_no) const
 soma::FieldP soma_ctx::fieldp() const
 {
     soma::FieldP f;
-    f.inv_nbar = (float)((double)(cells - n_forbidden) / (double)n_beads);   // accessible volume (R23)
+    f.inv_nbar = (float)((double)(cells - n_forbidden) / (double)n_beads_global);   // accessible volume (R23)
     f.kappa0 = (float)((double)kappaN / (double)N_ref);
     for (int i = 0; i < soma::kMaxTypes; ++i)
         for (int k = 0; k < soma::kMaxTypes; ++k) {
@@ -400,8 +404,9 @@ int launch_histogram(soma_ctx* c)
     return SOMA_OK;
 }
 
-int launch_fields(soma_ctx* c)
+int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr)
 {
+    if (!counts_src) counts_src = c->counts;
     const soma::FieldP F = c->fieldp();
 #ifndef SOMA_FIELD_THREADS
 #define SOMA_FIELD_THREADS 256
@@ -419,23 +424,30 @@ int launch_fields(soma_ctx* c)
     if (SOMA_FIELD_V4 && !pdl && c->cells % 4 == 0 && c->n_types <= 2) {
         const unsigned blocks4 = (unsigned)((c->cells / 4 + threads - 1) / threads);
         if (c->n_types == 1)
-            CU(launch_pdl(pdl, soma::field_kernel_v4<1>, blocks4, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden));
+            CU(launch_pdl(pdl, soma::field_kernel_v4<1>, blocks4, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden));
         else
-            CU(launch_pdl(pdl, soma::field_kernel_v4<2>, blocks4, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden));
+            CU(launch_pdl(pdl, soma::field_kernel_v4<2>, blocks4, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden));
         return SOMA_OK;
     }
     switch (c->n_types) {
-        case 1: CU(launch_pdl(pdl, soma::field_kernel<1>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden)); break;
-        case 2: CU(launch_pdl(pdl, soma::field_kernel<2>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden)); break;
-        default: CU(launch_pdl(pdl, soma::field_kernel<0>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden)); break;
+        case 1: CU(launch_pdl(pdl, soma::field_kernel<1>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
+        case 2: CU(launch_pdl(pdl, soma::field_kernel<2>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
+        default: CU(launch_pdl(pdl, soma::field_kernel<0>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
     }
     return SOMA_OK;
+}
+
+// omega after a parameter change; a shard has to wait for the next soma_shard_fields (it needs every rank's counts)
+int refresh_fields(soma_ctx* c)
+{
+    return c->sharded ? (int)SOMA_OK : launch_fields(c);
 }
 
 int stage1(soma_ctx* c)
 {
     int rc = launch_histogram(c);
     if (rc) return rc;
+    if (c->sharded) return SOMA_OK;   // omega needs every rank's counts: soma_shard_fields
     return launch_fields(c);
 }
 
@@ -497,10 +509,10 @@ int copy_soa(soma_ctx* c, float* dst_user, const float* src_user, bool to_user, 
         Timed t(c, SOMA_K_LAYOUT, 1);
         if (to_user)
             soma::reorder_kernel<true><<<blocks, 256, 0, c->stream>>>(dev_user, c->n_beads, c->x + s.off, c->y + s.off,
-                                                                     c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.gid0);
+                                                                     c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.local0);
         else
             soma::reorder_kernel<false><<<blocks, 256, 0, c->stream>>>(dev_user, c->n_beads, c->x + s.off, c->y + s.off,
-                                                                      c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.gid0);
+                                                                      c->z + s.off, c->orig + s.chain_off, s.N, s.n_beads, s.local0);
     }
     CU(cudaGetLastError());
     if (!user_is_device && to_user)
@@ -524,6 +536,7 @@ void soma_destroy(soma_ctx* c)
     if (c->stream || true) cudaStreamSynchronize(c->stream);
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
+    cudaFree(c->counts_global);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
     cudaFree(c->ext); cudaFree(c->forbidden); cudaFree(c->arch);
     cudaFree(c->acc_slots);
@@ -534,9 +547,10 @@ void soma_destroy(soma_ctx* c)
     delete c;
 }
 
-int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_ref, int n_types,
-              const float* box, const int* grid, float chiN, float kappaN, float A, uint64_t seed,
-              const float* host_xyz0, void* cuda_stream)
+static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_ref, int n_types,
+                     const float* box, const int* grid, float chiN, float kappaN, float A, uint64_t seed,
+                     const float* host_xyz0, void* cuda_stream, const uint64_t* spec_first_bead,
+                     uint64_t global_n_beads)
 {
     if (!out) return fail(SOMA_EINVAL, "soma_init: out is NULL");
     *out = nullptr;
@@ -584,7 +598,14 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
             return fail(SOMA_EINVAL, "soma_init: spec %d: n_beads must be >= 1 and types non-NULL", a);
         }
         s.n_beads = s.n_chains * s.N;
-        s.gid0 = gid;
+        s.gid0 = spec_first_bead ? spec_first_bead[a] : gid;
+        s.local0 = gid;
+        if (spec_first_bead && (s.gid0 + s.n_beads > global_n_beads || global_n_beads >= (1ull << 32))) {
+            delete c;
+            return fail(SOMA_EINVAL, "soma_init_shard: spec %d does not fit into the global system (first bead %llu, "
+                        "%llu beads, %llu beads in all, which must be < 2^32)", a, (unsigned long long)s.gid0,
+                        (unsigned long long)s.n_beads, (unsigned long long)global_n_beads);
+        }
         s.off = off;
         s.toff_off = (uint32_t)toff_host.size();
         s.n_bonds = chains[a].n_bonds;
@@ -660,6 +681,8 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         c->specs.push_back(s);
     }
     c->n_beads = gid;
+    c->sharded = spec_first_bead != nullptr;
+    c->n_beads_global = c->sharded ? global_n_beads : gid;
     c->n_pad = off + 128;
     if (c->n_beads == 0) {
         delete c;
@@ -719,13 +742,13 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
         CUI(cudaMalloc(&c->arch, sizeof(uint32_t) * arch_host.size()));
         CUI(cudaMemcpyAsync(c->arch, arch_host.data(), sizeof(uint32_t) * arch_host.size(), cudaMemcpyHostToDevice, c->stream));
     }
-    CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads + 31) / 32 + 8)));
+    CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32 + 8)));
     CUI(cudaMalloc(&c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMallocHost(&c->acc_host, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_pad, c->stream));
     CUI(cudaMemsetAsync(c->y, 0, sizeof(float) * c->n_pad, c->stream));
     CUI(cudaMemsetAsync(c->z, 0, sizeof(float) * c->n_pad, c->stream));
-    CUI(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32 + 8), c->stream));
+    CUI(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32 + 8), c->stream));
     CUI(cudaMemsetAsync(c->acc_slots, 0, sizeof(unsigned long long) * soma::kAccSlots, c->stream));
     CUI(cudaMemcpyAsync(c->toff, toff_host.data(), sizeof(uint32_t) * toff_host.size(), cudaMemcpyHostToDevice, c->stream));
     CUI(cudaStreamSynchronize(c->stream));  // toff_host goes out of scope
@@ -761,31 +784,65 @@ int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_
 #undef CUI
 }
 
+int soma_init(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_ref, int n_types,
+              const float* box, const int* grid, float chiN, float kappaN, float A, uint64_t seed,
+              const float* host_xyz0, void* cuda_stream)
+{
+    return init_impl(out, chains, n_specs, N_ref, n_types, box, grid, chiN, kappaN, A, seed, host_xyz0, cuda_stream,
+                     nullptr, 0);
+}
+
+int soma_init_shard(soma_ctx** out, const soma_chain_spec* chains, int n_specs, int N_ref, int n_types,
+                    const float* box, const int* grid, float chiN, float kappaN, float A, uint64_t seed,
+                    const float* host_xyz0, void* cuda_stream, const uint64_t* spec_first_bead,
+                    uint64_t global_n_beads)
+{
+    if (!spec_first_bead) return fail(SOMA_EINVAL, "soma_init_shard: spec_first_bead is NULL");
+    return init_impl(out, chains, n_specs, N_ref, n_types, box, grid, chiN, kappaN, A, seed, host_xyz0, cuda_stream,
+                     spec_first_bead, global_n_beads);
+}
+
+// the moves of one sweep: a1, a2 (or a5) [+ a3]
+static int sweep_moves(soma_ctx* c)
+{
+    if (c->record)
+        CU(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32), c->stream));
+    if (c->layout && c->sort_interval > 0 && c->sweeps_since_sort >= (uint64_t)c->sort_interval) {
+        int rs = resort(c);                            // storage order only: no result depends on it
+        if (rs) return rs;
+    }
+    c->sweeps_since_sort += 1;
+    const soma::MoveP P = c->movep(c->sweep);
+    int rc = launch_moves(c, P);                       // a1, a2 (or a5) [+ a3 incremental]
+    if (rc) return rc;
+    if (c->density_mode == 1) {
+        rc = launch_histogram(c);                      // a3 from scratch
+        if (rc) return rc;
+    }
+    return SOMA_OK;
+}
+
+static int check_step(soma_ctx* c, const char* who)
+{
+    if (c->move == 2 && !(c->smc_step > 0.0f))
+        return fail(SOMA_ESTATE, "%s: Smart-MC selected but SOMA_OPT_SMC_STEP not set", who);
+    if (c->scheme == 1 || c->set_order == 1)
+        for (const Spec& s : c->specs)
+            if (s.general)
+                return fail(SOMA_ESTATE, "%s: architectures given by a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only", who);
+    return SOMA_OK;
+}
+
 int soma_step(soma_ctx* c, int n_sweeps)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_step: ctx is NULL");
     if (n_sweeps < 0) return fail(SOMA_EINVAL, "soma_step: n_sweeps must be >= 0");
-    if (c->move == 2 && !(c->smc_step > 0.0f))
-        return fail(SOMA_ESTATE, "soma_step: Smart-MC selected but SOMA_OPT_SMC_STEP not set");
-    if (c->scheme == 1 || c->set_order == 1)
-        for (const Spec& s : c->specs)
-            if (s.general)
-                return fail(SOMA_ESTATE, "soma_step: architectures given by a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only");
+    if (c->sharded) return fail(SOMA_ESTATE, "soma_step: this context is a shard: use soma_shard_moves / soma_shard_fields");
+    int rc = check_step(c, "soma_step");
+    if (rc) return rc;
     for (int i = 0; i < n_sweeps; ++i) {
-        if (c->record)
-            CU(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads + 31) / 32), c->stream));
-        if (c->layout && c->sort_interval > 0 && c->sweeps_since_sort >= (uint64_t)c->sort_interval) {
-            int rs = resort(c);                            // storage order only: no result depends on it
-            if (rs) return rs;
-        }
-        c->sweeps_since_sort += 1;
-        const soma::MoveP P = c->movep(c->sweep);
-        int rc = launch_moves(c, P);                       // a1, a2 (or a5) [+ a3 incremental]
+        rc = sweep_moves(c);
         if (rc) return rc;
-        if (c->density_mode == 1) {
-            rc = launch_histogram(c);                      // a3 from scratch
-            if (rc) return rc;
-        }
         if (c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
             rc = launch_fields(c);                         // a4
             if (rc) return rc;
@@ -794,6 +851,39 @@ int soma_step(soma_ctx* c, int n_sweeps)
         c->attempted += c->n_beads;
         c->decisions_valid = c->record != 0;
     }
+    return SOMA_OK;
+}
+
+int soma_shard_moves(soma_ctx* c)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_shard_moves: ctx is NULL");
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_moves: the context was not created by soma_init_shard");
+    int rc = check_step(c, "soma_shard_moves");
+    if (rc) return rc;
+    rc = sweep_moves(c);
+    if (rc) return rc;
+    c->attempted += c->n_beads;
+    c->decisions_valid = c->record != 0;
+    return SOMA_OK;
+}
+
+int soma_shard_fields(soma_ctx* c, const uint32_t* global_counts, int src_is_device, int advance)
+{
+    if (!c || !global_counts) return fail(SOMA_EINVAL, "soma_shard_fields: NULL argument");
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_fields: the context was not created by soma_init_shard");
+    const uint32_t* src = global_counts;
+    if (!src_is_device) {
+        const size_t bytes = sizeof(uint32_t) * c->cells * c->n_types;
+        if (!c->counts_global) CU(cudaMalloc(&c->counts_global, bytes));
+        CU(cudaMemcpyAsync(c->counts_global, global_counts, bytes, cudaMemcpyHostToDevice, c->stream));
+        src = c->counts_global;
+    }
+    if (!advance || c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
+        int rc = launch_fields(c, src);                    // a4 from the occupation numbers of the whole system
+        if (rc) return rc;
+    }
+    if (advance) c->sweep += 1;
+    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));   // the caller may reuse its buffer
     return SOMA_OK;
 }
 
@@ -840,7 +930,7 @@ int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
     if (i < 0 || j < 0 || i >= c->n_types || j >= c->n_types || i == j || !std::isfinite(chiN_ij))
         return fail(SOMA_EINVAL, "soma_set_chi: need 0 <= i != j < n_types and a finite value");
     c->chiN[i][j] = c->chiN[j][i] = chiN_ij;
-    return launch_fields(c);
+    return refresh_fields(c);
 }
 
 int soma_set_external(soma_ctx* c, const float* ext_field, const uint8_t* forbidden, int src_is_device)
@@ -876,7 +966,7 @@ int soma_set_external(soma_ctx* c, const float* ext_field, const uint8_t* forbid
         CU(cudaFree(c->forbidden));
         c->forbidden = nullptr;
     }
-    int rc = launch_fields(c);
+    int rc = refresh_fields(c);
     if (rc) return rc;
     if (!src_is_device) CU(cudaStreamSynchronize(c->stream));   // the caller may reuse its buffers
     return SOMA_OK;
@@ -890,7 +980,7 @@ int soma_set_option(soma_ctx* c, int key, double value)
         case SOMA_OPT_HAMILTONIAN:
             if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_HAMILTONIAN: 0 or 1");
             c->hamiltonian = iv;
-            return launch_fields(c);
+            return refresh_fields(c);
         case SOMA_OPT_MOVE:
             if (iv != 1 && iv != 2) return fail(SOMA_EINVAL, "SOMA_OPT_MOVE: 1 (local) or 2 (Smart-MC)");
             c->move = iv;
@@ -993,7 +1083,7 @@ int soma_decisions(soma_ctx* c, uint32_t* bits, int dst_is_device)
     if (!c || !bits) return fail(SOMA_EINVAL, "soma_decisions: NULL argument");
     if (!c->decisions_valid)
         return fail(SOMA_ESTATE, "soma_decisions: set SOMA_OPT_RECORD_DECISIONS=1 before the sweep");
-    CU(cudaMemcpyAsync(bits, c->decisions, sizeof(uint32_t) * ((c->n_beads + 31) / 32),
+    CU(cudaMemcpyAsync(bits, c->decisions, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32),
                        dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost, c->stream));
     if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
     return SOMA_OK;

@@ -432,6 +432,102 @@ def test_programmatic_dependent_launch_changes_no_result(w):
     b.destroy()
 
 
+# ---------------------------------------------------------------------------------------------
+# a system spread over several GPUs: soma_init_shard / soma_shard_moves / soma_shard_fields
+# ---------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("move", ["local", "smc"])
+def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move):
+    """Three shard contexts stepped one after the other on this GPU (no rank waits for another), their
+    occupation numbers added on the host in place of the all-reduce: positions, counts, omega and decisions
+    equal the undivided context bit for bit; the first sweep is also checked against the oracle's parts."""
+    from paper_1711_03828_b200.sharded import local_positions, shard_layout
+    w = workloads.Workload("shard_blend", ((300, workloads.diblock(32, 16)), (77, workloads.homopolymer(8, 1)),
+                                           (5, workloads.homopolymer(33))), 32, 2, (4.0, 4.0, 3.0), (8, 8, 6),
+                           20.0, 50.0, 0.1, 11, move=move, smc_step=0.05 / 31)
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    whole = P.from_workload(w, xyz0=xyz0)
+    whole.set_option(P.OPT_RECORD_DECISIONS, 1)
+    specs = [(n, np.asarray(t, np.uint8)) for n, t in w.specs]
+    shards = []
+    for rank in range(3):
+        local, first, n_global, slices = shard_layout(specs, rank, 3)
+        sim = P.Soma(local, w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A, w.seed,
+                     xyz0=local_positions(xyz0, slices), spec_first_bead=first, global_n_beads=n_global)
+        if move == "smc":
+            sim.set_option(P.OPT_SMC_STEP, w.smc_step)
+            sim.set_option(P.OPT_MOVE, P.MOVE_SMC)
+        sim.set_option(P.OPT_RECORD_DECISIONS, 1)
+        with pytest.raises(P.SomaError):
+            sim.step(1)                                   # a shard has no soma_step
+        shards.append((sim, slices, oracle_system(w, specs=[(n, t) for n, t in local], spec_first_bead=first,
+                                                  global_n_beads=n_global)))
+
+    def exchange(advance):
+        total = sum(sim.fields(counts=np.empty((w.n_types, w.n_cells), np.uint32))[1].astype(np.int64)
+                    for sim, _, _ in shards).astype(np.uint32)
+        for sim, _, _ in shards:
+            sim.shard_fields(total, advance=advance)
+        return total
+
+    total = exchange(False)
+    om_w, cnt_w = whole.fields()
+    assert np.array_equal(total, cnt_w)
+    for sim, _, _ in shards:
+        assert np.array_equal(sim.fields(omega=np.empty_like(om_w))[0], om_w)
+    mk = oracle.MOVE_SMC if move == "smc" else oracle.MOVE_LOCAL
+    for sweep in range(4):
+        if sweep == 0:                                    # the oracle's parts, from the same positions and omega
+            for sim, _, orc in shards:
+                q = sim.positions()
+                dec = np.zeros(q.shape[1], np.uint8)
+                orc.sweep(q[0], q[1], q[2], om_w.copy(), 0, mk, dec)
+                sim._oracle_after = (q, dec)
+        whole.step(1)
+        for sim, _, _ in shards:
+            sim.shard_moves()
+        total = exchange(True)
+        om_w, cnt_w = whole.fields()
+        dec_w = P.unpack_decisions(whole.decisions(), w.n_beads)
+        assert np.array_equal(total, cnt_w)
+        for sim, slices, _ in shards:
+            got = sim.positions()
+            assert np.array_equal(got, local_positions(whole.positions(), slices))
+            assert np.array_equal(sim.fields(omega=np.empty_like(om_w))[0], om_w)
+            dec_s = P.unpack_decisions(sim.decisions(), w.n_beads)                 # indexed by the global bead index
+            mine = np.concatenate([dec_w[a:b] for a, b in slices])
+            assert np.array_equal(np.concatenate([dec_s[a:b] for a, b in slices]), mine)
+            assert sim.stats()[2] == sweep + 1
+            if sweep == 0:
+                q, dec = sim._oracle_after
+                same = dec == mine
+                assert same.mean() >= DECISION_AGREEMENT
+                if move == "local":
+                    assert np.array_equal(got[:, same], q[:, same])
+                else:
+                    assert np.max(np.abs(got[:, same].astype(np.float64) - q[:, same])) <= POS_TOL_SMC + 1e-6
+    whole.destroy()
+    for sim, _, _ in shards:
+        sim.destroy()
+
+
+def test_sharded_driver_with_one_rank_equals_the_plain_context():
+    from paper_1711_03828_b200.sharded import ShardedSoma
+    w = workloads.c1()
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    a = P.from_workload(w, xyz0=xyz0)
+    b = ShardedSoma(w, dist=None, xyz0_global=xyz0)
+    a.step(5)
+    b.step(5)
+    assert np.array_equal(a.positions(), b.positions())
+    (om_a, cnt_a), (om_b, cnt_b) = a.fields(), b.fields()
+    assert np.array_equal(cnt_a, cnt_b) and np.array_equal(om_a, om_b)
+    c = ShardedSoma(w, dist=None)                          # start state drawn on the device from the global indices
+    d = P.from_workload(w)
+    assert np.array_equal(c.positions(), d.positions())
+    for s_ in (a, b, c, d):
+        s_.destroy()
+
+
 def test_device_buffers_and_timing_hooks():
     import torch
     w = workloads.c1()
