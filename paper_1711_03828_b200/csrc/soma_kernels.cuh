@@ -32,6 +32,9 @@ constexpr int kFusedThreads = SOMA_FUSED_THREADS;
 #endif
 constexpr int kMolUnroll = SOMA_MOL_UNROLL;   // attempts of the staged molecule kernel unrolled together
 
+#ifndef SOMA_SMC_FAST
+#define SOMA_SMC_FAST 1
+#endif
 #ifndef SOMA_OMEGA_NC
 #define SOMA_OMEGA_NC 0
 #endif
@@ -156,6 +159,13 @@ __device__ __forceinline__ float ex2_approx(float x)
     return y;
 }
 
+__device__ __forceinline__ float sqrt_approx(float x)
+{
+    float y;
+    asm("sqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
 // ------------------------------------------------------------------------------------------------
 // Pi_c of Eq. 4: the cell that contains r, periodic (R7).  Per axis the
 // position in units of the box length is the fp32 number t = x * (1/L); the cell is
@@ -220,12 +230,26 @@ __device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
         uint32_t w[4], v[4];
         philox4x32_10_head(gid, P.head[0], P.rk, w);
         philox4x32_10_head(gid, P.head[1], P.rk, v);
+#if SOMA_SMC_FAST
+        // Box-Muller with sin.approx / cos.approx (MUFU) for the angle, taken in [-pi, pi) where the
+        // approximations are best (absolute error 2^-21.4): sin(t) = -sin(t - pi), cos(t) = -cos(t - pi), and
+        // t - pi = 2 pi (U23 - 1.5) with an exact subtraction.  A Gaussian is then off by <= ~2e-6, a
+        // displacement by sqrt(2 a_s) times that: inside the parity tolerance on positions (R17).
+        // The radius keeps the accurate logf: lg2.approx has an absolute, not a relative, error near 1, where
+        // the radius sqrt(-2 ln u) is small -- measured: 1 move in 10^4 off by more than 1e-6 R_e.
+        const float ra = sqrt_approx(-2.0f * logf(2.0f - u23(w[0])));   // sqrt.approx: <= 2 ulp
+        const float rb = sqrt_approx(-2.0f * logf(2.0f - u23(w[2])));
+        const float two_pi = 6.283185307179586f;
+        const float ta = two_pi * (u23(w[1]) - 1.5f), tb = two_pi * (u23(w[3]) - 1.5f);
+        const float sa = -__sinf(ta), ca = -__cosf(ta), cb = -__cosf(tb);
+#else
         const float ra = sqrtf(-2.0f * logf(2.0f - u23(w[0])));
         const float rb = sqrtf(-2.0f * logf(2.0f - u23(w[2])));
         const float two_pi = 6.283185307179586f;
         float sa, ca, sb, cb;
         sincosf(two_pi * (u23(w[1]) - 1.0f), &sa, &ca);
         sincosf(two_pi * (u23(w[3]) - 1.0f), &sb, &cb);
+#endif
         r.a = ra * ca; r.b = ra * sa; r.c = rb * cb;
         r.u = u23(v[0]) - 1.0f;
     }
@@ -300,7 +324,7 @@ __device__ __forceinline__ void smc_proposal(const MoveP& P, float mf, float sx,
         const float ef = dz - P.a_s * Fz, er = dz + P.a_s * (Fz - km * dz);
         fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
     }
-    log_ratio = (rev - fwd) / P.four_as;
+    log_ratio = __fdividef(rev - fwd, P.four_as);   // rcp.approx + multiply: within 2 ulp of the quotient
 }
 
 // The occupation numbers follow an accepted move (+1 new cell, -1 old cell): integer arithmetic, so
