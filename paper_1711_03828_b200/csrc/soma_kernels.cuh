@@ -149,6 +149,32 @@ __device__ __forceinline__ uint32_t first_set_bit(uint32_t first_gid, uint32_t s
 __device__ __forceinline__ void pdl_trigger() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
+// Positions cross the SM once per sweep: streaming (evict-first) loads and stores, so that they do not push
+// the omega lines the gathers reuse out of L1.
+#ifndef SOMA_STREAM_POS
+#define SOMA_STREAM_POS 1
+#endif
+__device__ __forceinline__ float4 ld_stream(const float* p)
+{
+#if SOMA_STREAM_POS == 1
+    return __ldcs(reinterpret_cast<const float4*>(p));
+#elif SOMA_STREAM_POS == 2
+    float4 v;
+    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+    return v;
+#else
+    return *reinterpret_cast<const float4*>(p);
+#endif
+}
+__device__ __forceinline__ void st_stream(float* p, const float4& v)
+{
+#if SOMA_STREAM_POS >= 1
+    __stcs(reinterpret_cast<float4*>(p), v);
+#else
+    *reinterpret_cast<float4*>(p) = v;
+#endif
+}
+
 // top 23 bits -> float in [1, 2), exact
 __device__ __forceinline__ float u23(uint32_t w) { return __uint_as_float(0x3F800000u | (w >> 9)); }
 
@@ -435,9 +461,9 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     uint32_t C = 0u;                                          // the caller's index of this lane's chain
     if (tile < t_end) {
         const uint32_t i0 = tile * kTile + 4u * lane;
-        X = *reinterpret_cast<const float4*>(x + i0);
-        Y = *reinterpret_cast<const float4*>(y + i0);
-        Z = *reinterpret_cast<const float4*>(z + i0);
+        X = ld_stream(x + i0);
+        Y = ld_stream(y + i0);
+        Z = ld_stream(z + i0);
         C = orig[i0 >> log2N];
     }
     while (tile < t_end) {
@@ -448,9 +474,9 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
         // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
         const uint32_t i0n = min(tile_n, t_end - 1u) * kTile + 4u * lane;
-        const float4 Xn = *reinterpret_cast<const float4*>(x + i0n);
-        const float4 Yn = *reinterpret_cast<const float4*>(y + i0n);
-        const float4 Zn = *reinterpret_cast<const float4*>(z + i0n);
+        const float4 Xn = ld_stream(x + i0n);
+        const float4 Yn = ld_stream(y + i0n);
+        const float4 Zn = ld_stream(z + i0n);
         const uint32_t Cn = orig[i0n >> log2N];
 
         // 2. random numbers of the four moves
@@ -569,9 +595,9 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             if (kIncr) { count_follow(counts, a1, o1, n1); count_follow(counts, a3, o3, n3); }
         }
 
-        *reinterpret_cast<float4*>(x + i0) = X;
-        *reinterpret_cast<float4*>(y + i0) = Y;
-        *reinterpret_cast<float4*>(z + i0) = Z;
+        st_stream(x + i0, X);
+        st_stream(y + i0, Y);
+        st_stream(z + i0, Z);
 
         const uint32_t nib = (a0 ? 1u : 0u) | (a1 ? 2u : 0u) | (a2 ? 4u : 0u) | (a3 ? 8u : 0u);
         n_acc += __popc(nib);
