@@ -363,6 +363,20 @@ def test_c3_headline_full_size():
     assert flips <= 2 * w.n_beads * 1e-5
 
 
+def test_c4_large_melt_full_size():
+    """BASELINE config C4 (268 M beads, 8.2 M cells: omega + counts exceed L2), one lock-step sweep from the
+    device-generated start state."""
+    import psutil
+    if psutil.virtual_memory().available < 40 * 2 ** 30:
+        pytest.skip("needs ~25 GB of host memory for the oracle's copy of the configuration")
+    w = workloads.c4()
+    seedling = P.from_workload(w)                 # start state R14 drawn on the device (checked against the oracle's at C1)
+    xyz0 = seedling.positions()
+    seedling.destroy()
+    flips = lockstep(w, 1, xyz0=xyz0)
+    assert flips <= w.n_beads * 1e-5
+
+
 def test_c5_blend_full_size_smart_mc():
     w = workloads.c5(smc_step=0.05 / 63)
     lockstep(w, 1)
