@@ -63,18 +63,21 @@ __device__ __forceinline__ float box_fraction(float x, float inv_L)
 __global__ void __launch_bounds__(128)
 chain_key_kernel(const float* __restrict__ x, const float* __restrict__ y, const float* __restrict__ z,
                  uint32_t n_chains, uint32_t N, float inv_Lx, float inv_Ly, float inv_Lz, uint32_t bits,
-                 uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
+                 float side_x, float side_y, float side_z, uint32_t* __restrict__ keys, uint32_t* __restrict__ vals)
 {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= n_chains) return;
     const size_t b = (size_t)c * N;
     float sx = 0.f, sy = 0.f, sz = 0.f;
     for (uint32_t j = 0; j < N; ++j) { sx += x[b + j]; sy += y[b + j]; sz += z[b + j]; }
-    const float inv_N = 1.0f / (float)N, side = (float)(1u << bits);
+    // side_a = units of the 2^bits cube the box spans along axis a: the same length per unit along x and y
+    // (the longest axis fills the cube), a multiple of it along z, the direction in which the cells of omega
+    // and counts are contiguous in memory (see resort()).
+    const float inv_N = 1.0f / (float)N;
     const uint32_t top = (1u << bits) - 1u;
-    const uint32_t hx = min((uint32_t)(box_fraction(sx * inv_N, inv_Lx) * side), top);
-    const uint32_t hy = min((uint32_t)(box_fraction(sy * inv_N, inv_Ly) * side), top);
-    const uint32_t hz = min((uint32_t)(box_fraction(sz * inv_N, inv_Lz) * side), top);
+    const uint32_t hx = min((uint32_t)(box_fraction(sx * inv_N, inv_Lx) * side_x), top);
+    const uint32_t hy = min((uint32_t)(box_fraction(sy * inv_N, inv_Ly) * side_y), top);
+    const uint32_t hz = min((uint32_t)(box_fraction(sz * inv_N, inv_Lz) * side_z), top);
     keys[c] = hilbert3(hx, hy, hz, bits);
     vals[c] = c;
 }
