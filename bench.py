@@ -35,7 +35,7 @@ METRIC = "attempted bead moves/s (full SCMF step)"
 UNIT = "moves/s"
 MOVE_BYTES_PER_BEAD = 24.0   # fused move kernel: read 12 B + write 12 B per bead per sweep
 FIELD_BYTES_PER_CELL = 16.0  # field kernel: read n_t counts + write n_t omegas (n_t = 2), DESIGN.md
-INSTR_PER_MOVE = 152.5       # SASS warp instructions per 32 local moves of the fused kernel (profiles/r01e_README.md)
+INSTR_PER_MOVE = 152.5       # SASS warp instructions per 32 local moves of the fused kernel (profiles/r01f_README.md)
 
 
 def peaks():
@@ -259,7 +259,7 @@ def main():
                                          "field": kms[P.K_FIELD] / max(1e-12, sum(kms))},
                 "full_step_frac": (MOVE_BYTES_PER_BEAD * nb + FIELD_BYTES_PER_CELL * w.n_cells) * args.steps
                                   / (ms_total * 1e-3) / 1e9 / peak}
-    # dram bytes per launch of the move kernel from the committed ncu --set full capture (profiles/r01e_README.md)
+    # dram bytes per launch of the move kernel from the committed ncu --set full capture (profiles/r01f_README.md)
     traffic_file = ROOT / "profiles" / "traffic.json"
     if traffic_file.exists():
         try:
