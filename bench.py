@@ -145,6 +145,9 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--kernel", type=int, default=0)
     ap.add_argument("--density", type=int, default=0)
+    ap.add_argument("--aged", type=int, default=5000,
+                    help="N = 1: also time this many further sweeps in one stretch (sustained clocks under the power cap; "
+                         "the melt orders on the way, SURVEY 8(d)); 0: skip")
     ap.add_argument("--sharded", action="store_true",
                     help="N > 1: ONE system of N x the config's chains in a box N x as long (same density), molecules "
                          "distributed over the ranks, one all-reduce of the occupation numbers per sweep (SURVEY 8(e)); "
@@ -304,6 +307,29 @@ def main():
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
             "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "acceptance": acc / max(1, att)}
+    if world == 1 and args.aged > 0 and not args.sharded:
+        # The same step over a long stretch (default 5000 sweeps, ~0.5 s): the melt orders on the way
+        # (PAPER.md:497 puts domain formation at ~2500 MC steps; same access pattern, other field magnitudes),
+        # and the board reaches its power cap, so the SM clock is the sustained one, not the burst clock of the
+        # short timed region above (the kernel is bound by instruction issue, so its time follows the clock).
+        att1, acc1, _ = sim.stats()
+        barrier()
+        with ClockSampler(local_rank) as clk_s:
+            e0.record()
+            sim.step(args.aged)
+            e1.record()
+            barrier()
+        ms_aged = e0.elapsed_time(e1)
+        att2, acc2, _ = sim.stats()
+        _, cnt = sim.fields()
+        cnt = cnt.astype(np.float64)
+        tot = np.maximum(cnt.sum(0), 1.0)
+        line["sustained"] = {"sweeps": int(args.aged), "value": nb * args.aged / (ms_aged * 1e-3), "unit": UNIT,
+                             "ms_per_step": ms_aged / args.aged, "clocks": clk_s.summary(),
+                             "full_step_frac": (MOVE_BYTES_PER_BEAD * nb + FIELD_BYTES_PER_CELL * w.n_cells) * args.aged
+                                               / (ms_aged * 1e-3) / 1e9 / peak,
+                             "acceptance": (acc2 - acc1) / max(1, att2 - att1),
+                             "mean_abs_phiA_minus_phiB": float(np.mean(np.abs(cnt[0] - cnt[-1]) / tot)) if w.n_types > 1 else None}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         line["cpu_baseline"], _ = oracle_rate(w, 2, 1)
     sim.destroy()
