@@ -135,6 +135,34 @@ def aggregate_moves_per_s(n_beads: int, steps: int, world: int, ms_total_max: fl
     return world * n_beads * steps / (ms_total_max * 1e-3)
 
 
+def all_configs(P, torch):
+    """Step time of every config (profiles/*_all_configs.txt)."""
+    peak, _ = peaks()
+    cases = [("C1", workloads.c1(), {}), ("C2 kappaN=50", workloads.c2(kappaN=50.0), {}), ("C3", workloads.c3(), {}),
+             ("C3 random set order", workloads.c3(), {"order": 1}), ("C5 a_s=0.05 (literal)", workloads.c5(), {}),
+             ("C5 a_s=0.05 b0^2", workloads.c5(smc_step=0.05 / 63), {}), ("C4", workloads.c4(), {})]
+    for name, w, kw in cases:
+        sim = P.from_workload(w)
+        if "order" in kw:
+            sim.set_option(P.OPT_SET_ORDER, 1)
+        n = 200 if w.n_beads < 2e6 else (50 if w.n_beads < 1e8 else 10)
+        sim.step(5)
+        sim.sync()
+        best = float("inf")
+        for _ in range(3):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            sim.step(n)
+            e1.record()
+            sim.sync()
+            best = min(best, e0.elapsed_time(e1) / n)
+        att, acc, _ = sim.stats()
+        print(f"{name:24s} beads {w.n_beads:>10d}  {best * 1e3:9.1f} us/step  {w.n_beads / best / 1e6:8.2f} G moves/s  "
+              f"24 B/move of measured HBM peak {MOVE_BYTES_PER_BEAD * w.n_beads / (best * 1e-3) / 1e9 / peak:.3f}  "
+              f"acceptance {acc / max(1, att):.3f}", flush=True)
+        sim.destroy()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -148,6 +176,9 @@ def main():
     ap.add_argument("--aged", type=int, default=5000,
                     help="N = 1: also time this many further sweeps in one stretch (sustained clocks under the power cap; "
                          "the melt orders on the way, SURVEY 8(d)); 0: skip")
+    ap.add_argument("--all-configs", action="store_true",
+                    help="instead of the bench line: step time of every BASELINE.json config (soma_step(n) between two "
+                         "CUDA events), C3 also in random set order, C5 with both Smart-MC steps; one text line each")
     ap.add_argument("--sharded", action="store_true",
                     help="N > 1: ONE system of N x the config's chains in a box N x as long (same density), molecules "
                          "distributed over the ranks, one all-reduce of the occupation numbers per sweep (SURVEY 8(e)); "
@@ -194,6 +225,10 @@ def main():
         torch.cuda.synchronize()
 
     from dataclasses import replace
+    if args.all_configs:
+        if rank == 0:
+            all_configs(P, torch)
+        return
     if args.sharded:
         # weak scaling of one system: world x the chains in a box world x as long along x (same density, same
         # cell size); every rank moves 1/world of the molecules and holds the whole grid
