@@ -17,7 +17,10 @@
  *     index = (beads of earlier architectures) + chain * n_beads_per_chain + monomer; coordinates
  *     are unwrapped (never folded into the box).
  *   - grid arrays are [type][ix][iy][iz], iz fastest; cell (ix,iy,iz) is the half-open box
- *     [ix dLx,(ix+1) dLx) x ... that *contains* the bead (Pi_c of Eq. 4), periodic images folded.
+ *     [ix dLx,(ix+1) dLx) x ... that *contains* the bead (Pi_c of Eq. 4), periodic images folded:
+ *     per axis t = fl32(x * fl32(1/L)), cell = floor(t n) mod n in exact arithmetic (R7).
+ *     Supported coordinates: |t n| < 2^22 per axis (at least 2^22 / n box lengths from the origin in
+ *     either direction); outside of it, and for NaN, the cell is unspecified but always a valid index.
  *   - pointers named host_* are host memory, dev_* device memory; "dst_is_device" selects.
  *   - the library owns all device state of a context; callers own every buffer they pass in; input
  *     buffers are only read during the call.
