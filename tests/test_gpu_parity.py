@@ -363,6 +363,29 @@ def test_c3_headline_full_size():
     assert flips <= 2 * w.n_beads * 1e-5
 
 
+def test_c3_long_run_counts_stay_exact_through_resorts_and_dependent_launches():
+    """12,000 free-running sweeps of the headline config in one call (six periodic re-sorts of the storage
+    order, every launch a programmatic dependent launch): the incrementally updated occupation numbers
+    still equal a histogram of the final positions taken by the oracle, omega equals the oracle's fields of
+    those counts, every move was attempted, and the melt has ordered."""
+    w = workloads.c3()
+    sim = P.from_workload(w)
+    om0, cnt0 = sim.fields()
+    sim.step(12000)
+    pos = sim.positions()
+    om, cnt = sim.fields()
+    orc = oracle_system(w)
+    want = orc.histogram(pos[0].copy(), pos[1].copy(), pos[2].copy())
+    assert np.array_equal(cnt, want)
+    assert field_close(w, om, orc.fields(want)) <= FIELD_RTOL
+    att, acc, done = sim.stats()
+    assert done == 12000 and att == 12000 * w.n_beads and 0.45 < acc / att < 0.60
+    order = lambda c: float(np.mean(np.abs(c[0].astype(np.float64) - c[1]) / np.maximum(c.sum(0), 1)))
+    assert order(cnt) > 3.0 * order(cnt0)                 # lamellar domains have formed
+    assert np.isfinite(pos).all()
+    sim.destroy()
+
+
 def test_c4_large_melt_full_size():
     """BASELINE config C4 (268 M beads, 8.2 M cells: omega + counts exceed L2), one lock-step sweep from the
     device-generated start state."""
