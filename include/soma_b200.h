@@ -47,7 +47,8 @@ enum {
     SOMA_ECUDA = -2,     /* a CUDA runtime call or kernel failed              */
     SOMA_ENOMEM = -3,    /* device or host allocation failed                  */
     SOMA_ESTATE = -4,    /* call not valid in the current state of the context */
-    SOMA_ENODEVICE = -5  /* no CUDA device / wrong architecture (needs sm_100) */
+    SOMA_ENODEVICE = -5, /* no CUDA device / wrong architecture (needs sm_100) */
+    SOMA_EDOMAIN = -6    /* a coordinate handed in is NaN / infinite / outside |x n / L| < 2^22 */
 };
 
 /* keys of soma_set_option */
@@ -170,7 +171,10 @@ int soma_fields(soma_ctx *ctx, float *omega, uint32_t *counts, int dst_is_device
 /* Copy out the positions (SoA, 3*n_beads float32, unwrapped). */
 int soma_positions(soma_ctx *ctx, float *xyz, int dst_is_device);
 
-/* Replace the positions (SoA, 3*n_beads float32) and redo stage 1 (histogram + fields). */
+/* Replace the positions (SoA, 3*n_beads float32) and redo stage 1 (histogram + fields).  Synchronises.
+ * SOMA_EDOMAIN if a coordinate is not finite or outside the supported domain (the positions are then
+ * loaded all the same and the context stays usable, e.g. for another soma_set_positions); soma_init
+ * returns the same code for its host_xyz0 and creates no context. */
 int soma_set_positions(soma_ctx *ctx, const float *xyz, int src_is_device);
 
 /* Set chi_ij N = chi_ji N for one type pair (i != j) and refresh omega. */

@@ -119,6 +119,7 @@ struct soma_ctx {
 
     // options
     int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0, use_graph = 1;
+    uint32_t* n_outside = nullptr;   // device counter: beads whose coordinates are outside the supported domain
     int pdl = 1;             // programmatic dependent launch of the fused and field kernels (SOMA_OPT_PDL)
     int blocks_per_sm = 0;   // grid of the fused kernel = n_sm * blocks_per_sm; 0 = as many as are resident
     float smc_step = 0.0f;
@@ -398,7 +399,8 @@ int launch_histogram(soma_ctx* c)
         if (blocks > cap) blocks = cap;
         Timed t(c, SOMA_K_DENSITY, 1);
         soma::histogram_kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
-            g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts);
+            g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts,
+            c->n_outside);
         CU(cudaGetLastError());
     }
     return SOMA_OK;
@@ -441,6 +443,19 @@ int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr)
 int refresh_fields(soma_ctx* c)
 {
     return c->sharded ? (int)SOMA_OK : launch_fields(c);
+}
+
+// After new positions came in (soma_init, soma_set_positions): did the histogram see a coordinate outside
+// the supported domain |x_a n_a / L_a| < 2^22, or a NaN?  Synchronises.
+int check_domain(soma_ctx* c, const char* who)
+{
+    uint32_t bad = 0;
+    CU(cudaMemcpyAsync(&bad, c->n_outside, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    if (bad == 0) return SOMA_OK;
+    CU(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
+    return fail(SOMA_EDOMAIN, "%s: %u beads have a coordinate that is not finite or lies outside the supported "
+                "domain |x n / L| < 2^22 per axis", who, bad);
 }
 
 int stage1(soma_ctx* c)
@@ -545,6 +560,7 @@ void soma_destroy(soma_ctx* c)
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts_global);
+    cudaFree(c->n_outside);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
     cudaFree(c->ext); cudaFree(c->forbidden); cudaFree(c->arch);
     cudaFree(c->acc_slots);
@@ -752,6 +768,8 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     }
     CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32 + 8)));
     CUI(cudaMalloc(&c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots));
+    CUI(cudaMalloc(&c->n_outside, sizeof(uint32_t)));
+    CUI(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
     CUI(cudaMallocHost(&c->acc_host, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_pad, c->stream));
     CUI(cudaMemsetAsync(c->y, 0, sizeof(float) * c->n_pad, c->stream));
@@ -779,6 +797,7 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     }
     if (rc == SOMA_OK) rc = resort(c);
     if (rc == SOMA_OK) rc = stage1(c);
+    if (rc == SOMA_OK) rc = check_domain(c, "soma_init");
     if (rc == SOMA_OK && cudaStreamSynchronize(c->stream) != cudaSuccess)
         rc = fail(SOMA_ECUDA, "soma_init: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc != SOMA_OK) {
@@ -928,8 +947,7 @@ int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
         c->sweeps_since_sort = std::max<uint64_t>(c->sweeps_since_sort, (uint64_t)c->sort_interval - 8);
     rc = stage1(c);
     if (rc) return rc;
-    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));  // caller may reuse its buffer
-    return SOMA_OK;
+    return check_domain(c, "soma_set_positions");   // synchronises: the caller may reuse its buffer
 }
 
 int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)

@@ -813,13 +813,20 @@ molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__
 __global__ void __launch_bounds__(256)
 histogram_kernel(const GridP g, const float* __restrict__ x, const float* __restrict__ y,
                  const float* __restrict__ z, const uint32_t* __restrict__ toff_tab, uint32_t N,
-                 uint32_t n_beads, uint32_t* __restrict__ counts)
+                 uint32_t n_beads, uint32_t* __restrict__ counts, uint32_t* __restrict__ n_outside)
 {
     const uint32_t stride = gridDim.x * blockDim.x;
+    uint32_t bad = 0;
     for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {
         const uint32_t j = i % N;
-        atomicAdd(counts + cell_at(g, x[i], y[i], z[i], toff_tab[j] + g.k_tot), 1u);
+        const float xi = x[i], yi = y[i], zi = z[i];
+        atomicAdd(counts + cell_at(g, xi, yi, zi, toff_tab[j] + g.k_tot), 1u);
+        // the supported coordinates of cell_raw(): |t n| < 2^22 per axis (a NaN fails the comparison too)
+        const bool ok = fabsf(xi * g.inv_L[0] * g.nf[0]) < 4194304.0f && fabsf(yi * g.inv_L[1] * g.nf[1]) < 4194304.0f &&
+                        fabsf(zi * g.inv_L[2] * g.nf[2]) < 4194304.0f;
+        bad += ok ? 0u : 1u;
     }
+    if (bad) atomicAdd(n_outside, bad);
 }
 
 // ------------------------------------------------------------------------------------------------

@@ -565,6 +565,35 @@ def test_sharded_driver_with_one_rank_equals_the_plain_context():
         s_.destroy()
 
 
+def test_coordinates_outside_the_supported_domain_are_refused():
+    """|x n / L| < 2^22 per axis (reading R7); NaN and infinity likewise.  soma_init creates no context,
+    soma_set_positions reports the error and leaves the context usable."""
+    w = workloads.c1()
+    good = np.stack(workloads.gaussian_walks(w))
+    for bad_value in (np.nan, np.inf, 4.0 * 2.0 ** 22 / 16 * 1.01):
+        bad = good.copy()
+        bad[1, 12345] = bad_value
+        with pytest.raises(P.SomaError) as e:
+            P.from_workload(w, xyz0=bad)
+        assert e.value.code == -6 and "1 beads" in str(e.value)
+    sim = P.from_workload(w, xyz0=good)
+    bad = good.copy()
+    bad[2, :7] = -np.inf
+    with pytest.raises(P.SomaError) as e:
+        sim.set_positions(bad)
+    assert e.value.code == -6 and "7 beads" in str(e.value)
+    sim.set_positions(good)                               # the context is still usable
+    ref = P.from_workload(w, xyz0=good)
+    sim.step(3)
+    ref.step(3)
+    assert np.array_equal(sim.positions(), ref.positions())
+    edge = good.copy()
+    edge[0, 0] = np.float32(4.0 * 2.0 ** 22 / 16 * 0.999)  # just inside: accepted
+    sim.set_positions(edge)
+    sim.destroy()
+    ref.destroy()
+
+
 def test_device_buffers_and_timing_hooks():
     import torch
     w = workloads.c1()
