@@ -472,8 +472,8 @@ def test_programmatic_dependent_launch_changes_no_result(w):
 # ---------------------------------------------------------------------------------------------
 # a system spread over several GPUs: soma_init_shard / soma_shard_moves / soma_shard_fields
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("move", ["local", "smc"])
-def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move):
+@pytest.mark.parametrize("move,set_order", [("local", 0), ("local", 1), ("smc", 0)])
+def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move, set_order):
     """Three shard contexts stepped one after the other on this GPU (no rank waits for another), their
     occupation numbers added on the host in place of the all-reduce: positions, counts, omega and decisions
     equal the undivided context bit for bit; the first sweep is also checked against the oracle's parts."""
@@ -484,6 +484,7 @@ def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move)
     xyz0 = np.stack(workloads.gaussian_walks(w))
     whole = P.from_workload(w, xyz0=xyz0)
     whole.set_option(P.OPT_RECORD_DECISIONS, 1)
+    whole.set_option(P.OPT_SET_ORDER, set_order)
     specs = [(n, np.asarray(t, np.uint8)) for n, t in w.specs]
     shards = []
     for rank in range(3):
@@ -494,10 +495,11 @@ def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move)
             sim.set_option(P.OPT_SMC_STEP, w.smc_step)
             sim.set_option(P.OPT_MOVE, P.MOVE_SMC)
         sim.set_option(P.OPT_RECORD_DECISIONS, 1)
+        sim.set_option(P.OPT_SET_ORDER, set_order)
         with pytest.raises(P.SomaError):
             sim.step(1)                                   # a shard has no soma_step
         shards.append((sim, slices, oracle_system(w, specs=[(n, t) for n, t in local], spec_first_bead=first,
-                                                  global_n_beads=n_global)))
+                                                  global_n_beads=n_global, set_order=set_order)))
 
     def exchange(advance):
         total = sum(sim.fields(counts=np.empty((w.n_types, w.n_cells), np.uint32))[1].astype(np.int64)

@@ -58,8 +58,8 @@ def test_shard_layout_offsets_are_the_global_bead_indices():
     assert [l[0] for l in local] == [n for n, _ in specs] and first[0] == 0 and slices[-1][1] == w.n_beads
 
 
-def _run_whole(w, xyz0, n_sweeps, move):
-    orc = oracle_system(w)
+def _run_whole(w, xyz0, n_sweeps, move, **over):
+    orc = oracle_system(w, **over)
     x, y, z = (xyz0[a].copy() for a in range(3))
     om = orc.fields(orc.histogram(x, y, z))
     for sweep in range(n_sweeps):
@@ -69,19 +69,21 @@ def _run_whole(w, xyz0, n_sweeps, move):
     return np.stack([x, y, z]), cnt, om
 
 
-def _part(w, rank, world):
+def _part(w, rank, world, **over):
     specs = [(n, np.asarray(t, np.uint8)) for n, t in w.specs]
     local, first, n_global, slices = shard_layout(specs, rank, world)
-    return oracle_system(w, specs=[(n, t) for n, t in local], spec_first_bead=first, global_n_beads=n_global), slices
+    return oracle_system(w, specs=[(n, t) for n, t in local], spec_first_bead=first, global_n_beads=n_global, **over), slices
 
 
 def test_oracle_parts_reproduce_the_undivided_oracle():
-    """Three parts moved one after the other in one process, counts added by hand."""
+    """Three parts moved one after the other in one process, counts added by hand; local moves in fixed
+    and in random set order (the order bit is drawn for the chain's index in the whole system), Smart-MC."""
     w = _blend()
     xyz0 = np.stack(workloads.gaussian_walks(w))
-    for move in (oracle.MOVE_LOCAL,):
-        want_xyz, want_cnt, want_om = _run_whole(w, xyz0, 3, move)
-        parts = [_part(w, r, 3) for r in range(3)]
+    for move, over in ((oracle.MOVE_LOCAL, {}), (oracle.MOVE_LOCAL, {"set_order": 1}),
+                       (oracle.MOVE_SMC, {"smc_step": 0.05 / 31})):
+        want_xyz, want_cnt, want_om = _run_whole(w, xyz0, 3, move, **over)
+        parts = [_part(w, r, 3, **over) for r in range(3)]
         pos = [local_positions(xyz0, sl) for _, sl in parts]
         cnt = sum(p.histogram(*q).astype(np.int64) for (p, _), q in zip(parts, pos)).astype(np.uint32)
         om = parts[0][0].fields(cnt)
