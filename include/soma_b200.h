@@ -150,7 +150,8 @@ int soma_init_shard(soma_ctx **out, const soma_chain_spec *chains, int n_specs, 
                     uint64_t global_n_beads);
 
 /* The moves of one sweep (a1, a2 | a5) of this rank's molecules in the current omega; the local
- * occupation numbers follow (a3).  Asynchronous on the context's stream. */
+ * occupation numbers follow (a3).  Asynchronous on the context's stream.  SOMA_ESTATE for the
+ * combinations whose part-of-a-system mode has no oracle: SOMA_OPT_SCHEME 1 and bond-list architectures. */
 int soma_shard_moves(soma_ctx *ctx);
 
 /* a4: omega from the occupation numbers of the whole system (uint32 [n_types][cells], host or device;

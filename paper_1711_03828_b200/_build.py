@@ -8,9 +8,9 @@ from pathlib import Path
 
 _PKG = Path(__file__).resolve().parent
 CSRC = _PKG / "csrc"
-LIB = Path(os.environ.get("SOMA_B200_LIB", _PKG / "libsoma_b200.so"))   # override: a prebuilt variant
+LIB = _PKG / "libsoma_b200.so"
 SOURCES = [CSRC / "soma_b200.cu"]
-HEADERS = [CSRC / "soma_kernels.cuh", _PKG.parent / "include" / "soma_b200.h"]
+HEADERS = sorted(CSRC.glob("*.cuh")) + [_PKG.parent / "include" / "soma_b200.h"]
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a",
@@ -29,10 +29,6 @@ def nvcc() -> str:
 
 
 def stale() -> bool:
-    if "SOMA_B200_LIB" in os.environ:
-        if not LIB.exists():
-            raise RuntimeError(f"SOMA_B200_LIB={LIB} does not exist")
-        return False
     if not LIB.exists():
         return True
     t = LIB.stat().st_mtime

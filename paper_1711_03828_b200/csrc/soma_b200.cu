@@ -50,6 +50,21 @@ int fail(int code, const char* fmt, ...)
                         #call, cudaGetErrorString(e_), __FILE__, __LINE__);                        \
     } while (0)
 
+// Every entry point works on the device its context was created on, whatever device is current in the
+// calling thread, and leaves the caller's current device as it found it.
+struct DeviceGuard {
+    int prev = -1, want = -1;
+    explicit DeviceGuard(int device) : want(device)
+    {
+        if (cudaGetDevice(&prev) != cudaSuccess) prev = -1;
+        if (prev != want) cudaSetDevice(want);
+    }
+    ~DeviceGuard()
+    {
+        if (prev >= 0 && prev != want) cudaSetDevice(prev);
+    }
+};
+
 struct Spec {
     uint64_t n_chains = 0;
     uint32_t N = 0;
@@ -70,6 +85,7 @@ struct Spec {
 };
 
 constexpr int kEventPool = 2048;
+constexpr int kMaxDevices = 64;
 
 }  // namespace
 
@@ -277,11 +293,13 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
     auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
-    int per_sm = c->blocks_per_sm;
-    if (per_sm <= 0) {   // auto: every block resident, one wave
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, threads, 0));
-        if (per_sm < 1) per_sm = 1;
+    static int resident[kMaxDevices] = {};             // blocks per SM of this instantiation, asked once per device
+    int& res = resident[c->device % kMaxDevices];
+    if (res == 0) {
+        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res, kernel, threads, 0));
+        if (res < 1) res = 1;
     }
+    const int per_sm = c->blocks_per_sm > 0 ? c->blocks_per_sm : res;   // auto: every block resident, one wave
     int blocks = c->n_sm * per_sm;
     const int max_useful = (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
     if (blocks > max_useful) blocks = max_useful;
@@ -319,10 +337,17 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
             if (warps >= 1 && c->kernel_choice != 1) {   // chains staged in shared memory
                 auto kernel = soma::molecule_staged_kernel<kMove, kIncr, kRecord>;
                 const size_t smem = per_warp * warps;
-                if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-                int per_sm = 1;
-                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, warps * 32, smem));
-                if (per_sm < 1) per_sm = 1;
+                // shared-memory limit and resident blocks per SM: asked once per (instantiation, device, chain length)
+                static size_t asked_smem[kMaxDevices] = {};
+                static int asked_res[kMaxDevices] = {};
+                const int d = c->device % kMaxDevices;
+                if (asked_smem[d] != smem) {
+                    if (smem > 48 * 1024) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+                    CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&asked_res[d], kernel, warps * 32, smem));
+                    if (asked_res[d] < 1) asked_res[d] = 1;
+                    asked_smem[d] = smem;
+                }
+                const int per_sm = asked_res[d];
                 const uint64_t n_groups = (s.n_chains + 31) / 32;
                 const uint64_t blocks = std::min<uint64_t>((uint64_t)c->n_sm * per_sm, (n_groups + warps - 1) / warps);
                 Timed t(c, SOMA_K_MOVE, 1);
@@ -387,7 +412,9 @@ int launch_moves(soma_ctx* c, const soma::MoveP& P)
 #undef SOMA_DISPATCH
 }
 
-int launch_histogram(soma_ctx* c)
+// check_domain: also count the beads whose coordinates lie outside the supported domain (stage 1 of new
+// positions); the per-sweep histograms of SOMA_OPT_DENSITY = 1 do not -- moves cannot leave the domain
+int launch_histogram(soma_ctx* c, bool check_domain_too)
 {
     CU(cudaMemsetAsync(c->counts, 0, sizeof(uint32_t) * c->cells * c->n_types, c->stream));
     const soma::GridP g = c->gridp();
@@ -400,7 +427,7 @@ int launch_histogram(soma_ctx* c)
         Timed t(c, SOMA_K_DENSITY, 1);
         soma::histogram_kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
             g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts,
-            c->n_outside);
+            check_domain_too ? c->n_outside : nullptr);
         CU(cudaGetLastError());
     }
     return SOMA_OK;
@@ -453,14 +480,14 @@ int check_domain(soma_ctx* c, const char* who)
     CU(cudaMemcpyAsync(&bad, c->n_outside, sizeof(uint32_t), cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
     if (bad == 0) return SOMA_OK;
-    CU(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
     return fail(SOMA_EDOMAIN, "%s: %u beads have a coordinate that is not finite or lies outside the supported "
                 "domain |x n / L| < 2^22 per axis", who, bad);
 }
 
 int stage1(soma_ctx* c)
 {
-    int rc = launch_histogram(c);
+    CU(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
+    int rc = launch_histogram(c, true);
     if (rc) return rc;
     if (c->sharded) return SOMA_OK;   // omega needs every rank's counts: soma_shard_fields
     return launch_fields(c);
@@ -556,7 +583,8 @@ const char* soma_version(void) { return "soma-b200 0.1 (sm_100a)"; }
 void soma_destroy(soma_ctx* c)
 {
     if (!c) return;
-    if (c->stream || true) cudaStreamSynchronize(c->stream);
+    DeviceGuard on_device(c->device);
+    cudaStreamSynchronize(c->stream);
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts_global);
@@ -843,7 +871,7 @@ static int sweep_moves(soma_ctx* c)
     int rc = launch_moves(c, P);                       // a1, a2 (or a5) [+ a3 incremental]
     if (rc) return rc;
     if (c->density_mode == 1) {
-        rc = launch_histogram(c);                      // a3 from scratch
+        rc = launch_histogram(c, false);               // a3 from scratch
         if (rc) return rc;
     }
     return SOMA_OK;
@@ -857,12 +885,21 @@ static int check_step(soma_ctx* c, const char* who)
         for (const Spec& s : c->specs)
             if (s.general)
                 return fail(SOMA_ESTATE, "%s: architectures given by a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only", who);
+    if (c->sharded) {
+        // a part of a larger system is checked against the oracle for linear chains in the set scheme only
+        if (c->scheme == 1)
+            return fail(SOMA_ESTATE, "%s: a shard supports SOMA_OPT_SCHEME 0 only", who);
+        for (const Spec& s : c->specs)
+            if (s.general)
+                return fail(SOMA_ESTATE, "%s: a shard supports linear chains only (no bond-list architectures)", who);
+    }
     return SOMA_OK;
 }
 
 int soma_step(soma_ctx* c, int n_sweeps)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_step: ctx is NULL");
+    DeviceGuard on_device(c->device);
     if (n_sweeps < 0) return fail(SOMA_EINVAL, "soma_step: n_sweeps must be >= 0");
     if (c->sharded) return fail(SOMA_ESTATE, "soma_step: this context is a shard: use soma_shard_moves / soma_shard_fields");
     int rc = check_step(c, "soma_step");
@@ -884,6 +921,7 @@ int soma_step(soma_ctx* c, int n_sweeps)
 int soma_shard_moves(soma_ctx* c)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_shard_moves: ctx is NULL");
+    DeviceGuard on_device(c->device);
     if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_moves: the context was not created by soma_init_shard");
     int rc = check_step(c, "soma_shard_moves");
     if (rc) return rc;
@@ -897,6 +935,7 @@ int soma_shard_moves(soma_ctx* c)
 int soma_shard_fields(soma_ctx* c, const uint32_t* global_counts, int src_is_device, int advance)
 {
     if (!c || !global_counts) return fail(SOMA_EINVAL, "soma_shard_fields: NULL argument");
+    DeviceGuard on_device(c->device);
     if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_fields: the context was not created by soma_init_shard");
     const uint32_t* src = global_counts;
     if (!src_is_device) {
@@ -917,6 +956,7 @@ int soma_shard_fields(soma_ctx* c, const uint32_t* global_counts, int src_is_dev
 int soma_fields(soma_ctx* c, float* omega, uint32_t* counts, int dst_is_device)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_fields: ctx is NULL");
+    DeviceGuard on_device(c->device);
     if (!omega && !counts) return fail(SOMA_EINVAL, "soma_fields: both outputs NULL");
     const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
     const size_t n = (size_t)c->cells * c->n_types;
@@ -929,6 +969,7 @@ int soma_fields(soma_ctx* c, float* omega, uint32_t* counts, int dst_is_device)
 int soma_positions(soma_ctx* c, float* xyz, int dst_is_device)
 {
     if (!c || !xyz) return fail(SOMA_EINVAL, "soma_positions: NULL argument");
+    DeviceGuard on_device(c->device);
     int rc = copy_soa(c, xyz, nullptr, true, dst_is_device != 0);
     if (rc) return rc;
     if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
@@ -938,6 +979,7 @@ int soma_positions(soma_ctx* c, float* xyz, int dst_is_device)
 int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
 {
     if (!c || !xyz) return fail(SOMA_EINVAL, "soma_set_positions: NULL argument");
+    DeviceGuard on_device(c->device);
     int rc = copy_soa(c, nullptr, xyz, false, src_is_device != 0);
     if (rc) return rc;
     // The new positions keep the old storage order (usually they are a configuration this context
@@ -953,6 +995,7 @@ int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
 int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_set_chi: ctx is NULL");
+    DeviceGuard on_device(c->device);
     if (i < 0 || j < 0 || i >= c->n_types || j >= c->n_types || i == j || !std::isfinite(chiN_ij))
         return fail(SOMA_EINVAL, "soma_set_chi: need 0 <= i != j < n_types and a finite value");
     c->chiN[i][j] = c->chiN[j][i] = chiN_ij;
@@ -962,6 +1005,7 @@ int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
 int soma_set_external(soma_ctx* c, const float* ext_field, const uint8_t* forbidden, int src_is_device)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_set_external: ctx is NULL");
+    DeviceGuard on_device(c->device);
     const cudaMemcpyKind kind = src_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
     const size_t n = (size_t)c->cells * c->n_types;
     if (ext_field) {
@@ -1001,6 +1045,7 @@ int soma_set_external(soma_ctx* c, const float* ext_field, const uint8_t* forbid
 int soma_set_option(soma_ctx* c, int key, double value)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_set_option: ctx is NULL");
+    DeviceGuard on_device(c->device);
     const int iv = (int)value;
     switch (key) {
         case SOMA_OPT_HAMILTONIAN:
@@ -1093,6 +1138,7 @@ int soma_set_option(soma_ctx* c, int key, double value)
 int soma_stats(soma_ctx* c, uint64_t* attempted, uint64_t* accepted, uint64_t* sweeps_done)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_stats: ctx is NULL");
+    DeviceGuard on_device(c->device);
     CU(cudaMemcpyAsync(c->acc_host, c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots,
                        cudaMemcpyDeviceToHost, c->stream));
     CU(cudaStreamSynchronize(c->stream));
@@ -1107,6 +1153,7 @@ int soma_stats(soma_ctx* c, uint64_t* attempted, uint64_t* accepted, uint64_t* s
 int soma_decisions(soma_ctx* c, uint32_t* bits, int dst_is_device)
 {
     if (!c || !bits) return fail(SOMA_EINVAL, "soma_decisions: NULL argument");
+    DeviceGuard on_device(c->device);
     if (!c->decisions_valid)
         return fail(SOMA_ESTATE, "soma_decisions: set SOMA_OPT_RECORD_DECISIONS=1 before the sweep");
     CU(cudaMemcpyAsync(bits, c->decisions, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32),
@@ -1118,6 +1165,7 @@ int soma_decisions(soma_ctx* c, uint32_t* bits, int dst_is_device)
 int soma_kernel_times(soma_ctx* c, double* ms, uint64_t* launches)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_kernel_times: ctx is NULL");
+    DeviceGuard on_device(c->device);
     int rc = drain_events(c);
     if (rc) return rc;
     for (int k = 0; k < SOMA_K_COUNT; ++k) {
@@ -1137,6 +1185,7 @@ int soma_n_types(const soma_ctx* c) { return c ? c->n_types : 0; }
 int soma_sync(soma_ctx* c)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_sync: ctx is NULL");
+    DeviceGuard on_device(c->device);
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
     return SOMA_OK;

@@ -453,8 +453,9 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     // + kWarps), after that a warp takes the next free tile from a shared-memory counter, one tile ahead
     // of the prefetch.  The schedulers do not serve their warps evenly; with a fixed share per warp the
     // favoured ones finished early and the SM ran its last tiles at low occupancy.
-    __shared__ uint32_t s_next;
-    if (threadIdx.x == 0) s_next = t_begin + 2u * kWarps;
+    __shared__ uint32_t s_next[2];
+    const uint32_t zero = n_mask >> 8;                        // n_mask = N - 1 <= 127
+    if (threadIdx.x == 0) s_next[0] = t_begin + 2u * kWarps;
     __syncthreads();
     uint32_t tile = t_begin + wib, tile_n = tile + kWarps;
     float4 X, Y, Z;
@@ -469,8 +470,11 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     while (tile < t_end) {
         const uint32_t i0 = tile * kTile + 4u * lane;
         const uint32_t gid = gid0 + (C << log2N) + j0;
+        // the tile after the next one.  The counter is addressed through `warp & zero` (zero: a kernel argument
+        // bit that is never set): with a provably uniform address ptxas wraps the atomic of this single lane
+        // into its warp-aggregation sequence (vote, popc, leader election: a dozen instructions per tile)
         uint32_t tile_nn = 0u;
-        if (lane == 0) tile_nn = atomicAdd(&s_next, 1u);      // the tile after the next one
+        if (lane == 0) tile_nn = atomicAdd(s_next + (wib & zero), 1u);
 
         // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
         const uint32_t i0n = min(tile_n, t_end - 1u) * kTile + 4u * lane;
@@ -815,10 +819,10 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
                  const float* __restrict__ z, const uint32_t* __restrict__ toff_tab, uint32_t N,
                  uint32_t n_beads, uint32_t* __restrict__ counts, uint32_t* __restrict__ n_outside)
 {
-    const uint32_t stride = gridDim.x * blockDim.x;
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
     uint32_t bad = 0;
-    for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {
-        const uint32_t j = i % N;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {   // 64-bit: n_beads may be 2^32 - 1
+        const uint32_t j = (uint32_t)(i % N);
         const float xi = x[i], yi = y[i], zi = z[i];
         atomicAdd(counts + cell_at(g, xi, yi, zi, toff_tab[j] + g.k_tot), 1u);
         // the supported coordinates of cell_raw(): |t n| < 2^22 per axis (a NaN fails the comparison too)
@@ -826,7 +830,7 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
                         fabsf(zi * g.inv_L[2] * g.nf[2]) < 4194304.0f;
         bad += ok ? 0u : 1u;
     }
-    if (bad) atomicAdd(n_outside, bad);
+    if (bad && n_outside) atomicAdd(n_outside, bad);
 }
 
 // ------------------------------------------------------------------------------------------------
