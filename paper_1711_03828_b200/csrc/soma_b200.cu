@@ -293,9 +293,11 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
     auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
+    constexpr size_t kOrderSmemMax = 160 * 1024;       // shared memory for the order bits of a block's chains
     static int resident[kMaxDevices] = {};             // blocks per SM of this instantiation, asked once per device
     int& res = resident[c->device % kMaxDevices];
     if (res == 0) {
+        if (kOrder) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOrderSmemMax));
         CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res, kernel, threads, 0));
         if (res < 1) res = 1;
     }
@@ -303,8 +305,19 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     int blocks = c->n_sm * per_sm;
     const int max_useful = (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
     if (blocks > max_useful) blocks = max_useful;
+    // random set order: one byte per chain of the longest tile range a block can get; more (not all
+    // resident) blocks if that does not fit into shared memory
+    size_t order_smem = 0;
+    if (kOrder) {
+        const size_t chains_per_tile = soma::kTile / s.N;
+        for (int waves = 1;; ++waves) {
+            order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile;
+            if (order_smem <= kOrderSmemMax) break;
+            blocks = c->n_sm * per_sm * (waves + 1);
+        }
+    }
     Timed t(c, SOMA_K_MOVE, 1);
-    CU(launch_pdl(c->pdl != 0, kernel, (unsigned)blocks, (unsigned)threads, 0, c->stream,
+    CU(launch_pdl(c->pdl != 0, kernel, (unsigned)blocks, (unsigned)threads, order_smem, c->stream,
                   P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N - 1u,
                   s.n_tiles, (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots));
     return SOMA_OK;

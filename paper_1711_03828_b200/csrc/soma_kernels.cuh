@@ -423,6 +423,8 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 //   gid0        global index of the architecture's first bead
 //   orig        [n_chains] the caller's chain index of the chain in each slot (Philox counter, bitmap)
 //   dec_words   decision bitmap (whole system), or unused
+// kOrder: dynamic shared memory = one byte per chain of the block's tile range (the host keeps the ranges
+// short enough); the block draws the order bit of all its chains before it waits for its predecessor.
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord, bool kOrder>
 __global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
@@ -437,7 +439,6 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const uint32_t wib = threadIdx.x >> 5;
     constexpr uint32_t kWarps = kFusedThreads / 32;
     pdl_trigger();
-    pdl_wait();                                               // omega of the preceding field kernel
     const uint32_t j0 = (4u * lane) & n_mask;                 // monomer index of slot 0
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
     const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
@@ -456,6 +457,17 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     __shared__ uint32_t s_next[2];
     const uint32_t zero = n_mask >> 8;                        // n_mask = N - 1 <= 127
     if (threadIdx.x == 0) s_next[0] = t_begin + 2u * kWarps;
+    extern __shared__ uint8_t s_order[];                      // kOrder: order bit of the chains of this block's tiles
+    const uint32_t slot_begin = (t_begin * kTile) >> log2N;
+    if (kOrder) {
+        // "Generate random permutation of the sets" (Code 2) for every chain this block will move:
+        // needs nothing of the predecessor kernel (orig[] only changes in a re-sort), so it runs before the wait
+        const uint32_t n_slots = ((t_end - t_begin) * kTile) >> log2N;
+        for (uint32_t s = threadIdx.x; s < n_slots; s += kFusedThreads)
+            s_order[s] = (uint8_t)first_set_bit(gid0 + (orig[slot_begin + s] << log2N), P.sweep_lo, P.sweep_hi,
+                                                P.rk[0][0], P.rk[0][1]);
+    }
+    pdl_wait();                                               // omega of the preceding field kernel
     __syncthreads();
     uint32_t tile = t_begin + wib, tile_n = tile + kWarps;
     float4 X, Y, Z;
@@ -470,6 +482,8 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     while (tile < t_end) {
         const uint32_t i0 = tile * kTile + 4u * lane;
         const uint32_t gid = gid0 + (C << log2N) + j0;
+        uint32_t order_bit = 0u;
+        if (kOrder) order_bit = s_order[(i0 >> log2N) - slot_begin];
         // the tile after the next one.  The counter is addressed through `warp & zero` (zero: a kernel argument
         // bit that is never set): with a provably uniform address ptxas wraps the atomic of this single lane
         // into its warp-aggregation sequence (vote, popc, leader election: a dozen instructions per tile)
@@ -523,33 +537,41 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
                 X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
                 X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
             } else {
-                // 4'. random set order (SOMA_OPT_SET_ORDER = 1): the chain's bit says which set moves
-                // first.  Lanes of one warp hold different chains, so every slot is evaluated in both
-                // phases and takes part in the one its parity is due in.
-                const uint32_t bit = first_set_bit(gid0 + (C << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]);
-                a0 = a1 = a2 = a3 = false;
+                // 4'. random set order (SOMA_OPT_SET_ORDER = 1, "Generate random permutation of the sets", Code 2,
+                // PAPER.md:302): the chain's bit says which set moves first, and the lanes of a warp hold
+                // different chains.  Three phases: the odd monomers of the chains that start with their odd set,
+                // the even monomers of every chain, the odd monomers of the chains that start with their even
+                // set.  A chain takes part in the two phases that are its own order; every slot is evaluated
+                // where it can move (six evaluations per lane instead of four).
+                const bool odd_first = order_bit != 0u;
+                a1 = a3 = false;
+                float sx, sy, sz;
 #pragma unroll
-                for (uint32_t phase = 0; phase < 2u; ++phase) {
-                    const bool odd_now = (phase ^ bit) != 0u, even_now = !odd_now;
-                    float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
-                    float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
-                    xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
-                    xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
-                    float sx, sy, sz;
-                    bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
-                    const bool b0 = even_now && metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
-                    bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
-                    const bool b2 = even_now && metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
-                    bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
-                    const bool b1 = odd_now && metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, q1.u);
-                    bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
-                    const bool b3 = odd_now && metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, q3.u);
-                    // members of one set are not bonded to each other: all four updates at once
-                    X.x = b0 ? x0n : X.x; Y.x = b0 ? y0n : Y.x; Z.x = b0 ? z0n : Z.x;
-                    X.y = b1 ? x1n : X.y; Y.y = b1 ? y1n : Y.y; Z.y = b1 ? z1n : Z.y;
-                    X.z = b2 ? x2n : X.z; Y.z = b2 ? y2n : Y.z; Z.z = b2 ? z2n : Z.z;
-                    X.w = b3 ? x3n : X.w; Y.w = b3 ? y3n : Y.w; Z.w = b3 ? z3n : Z.w;
-                    a0 = a0 || b0; a1 = a1 || b1; a2 = a2 || b2; a3 = a3 || b3;
+                for (int phase = 0; phase < 3; ++phase) {
+                    if (phase == 1) {          // even monomers (slots 0, 2) of every chain
+                        float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+                        xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+                        bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
+                        a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
+                        bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
+                        a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
+                        X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
+                        X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
+                    } else {                   // odd monomers (slots 1, 3): phase 0 if odd_first, phase 2 if not
+                        // a chain whose turn it is not compares with u = +inf, which accepts nothing
+                        const bool due = (phase == 0) == odd_first;
+                        const float inf = __int_as_float(0x7F800000);
+                        const float u1 = due ? q1.u : inf, u3 = due ? q3.u : inf;
+                        float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+                        xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+                        bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
+                        const bool b1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, u1);
+                        bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
+                        const bool b3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, u3);
+                        X.y = b1 ? x1n : X.y; Y.y = b1 ? y1n : Y.y; Z.y = b1 ? z1n : Z.y;
+                        X.w = b3 ? x3n : X.w; Y.w = b3 ? y3n : Y.w; Z.w = b3 ? z3n : Z.w;
+                        a1 = a1 || b1; a3 = a3 || b3;
+                    }
                 }
             }
 
