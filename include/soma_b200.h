@@ -48,7 +48,13 @@ enum {
     SOMA_ENOMEM = -3,    /* device or host allocation failed                  */
     SOMA_ESTATE = -4,    /* call not valid in the current state of the context */
     SOMA_ENODEVICE = -5, /* no CUDA device / wrong architecture (needs sm_100) */
-    SOMA_EDOMAIN = -6    /* a coordinate handed in is NaN / infinite / outside |x n / L| < 2^22 */
+    SOMA_EDOMAIN = -6,   /* a coordinate handed in is NaN / infinite / outside |x n / L| < 2^22 */
+    SOMA_EOVERFLOW = -7  /* a cell holds more than 65535 beads of one type while the occupation numbers are
+                            kept as 16 + 16 bits per cell (SOMA_OPT_COUNT_BITS).  Sticky: the field kernel sets
+                            it on the device; soma_step (on entry), soma_sync, soma_stats and the calls that
+                            copy to host memory report it from then on.  Fields and trajectory are invalid
+                            from the sweep in which it happened: set SOMA_OPT_COUNT_BITS = 32 and go back to a
+                            saved configuration (soma_set_positions)                                  */
 };
 
 /* keys of soma_set_option */
@@ -82,9 +88,21 @@ enum {
                                    /* of the chain whose first bead is f uses Philox counter word f + k: kind 4 */
                                    /* word 0 picks i = floor(w N / 2^32), kinds 1 / 2 drive the move; bit f + k */
                                    /* of soma_decisions is the outcome of that attempt                          */
-    SOMA_OPT_PDL = 16              /* 1 (default): the fused move kernel and the field kernel are launched with */
+    SOMA_OPT_PDL = 16,             /* 1 (default): the fused move kernel and the field kernel are launched with */
                                    /* programmatic dependent launch, so each becomes resident while its         */
                                    /* predecessor drains (results do not depend on it); 0: ordinary launches    */
+    SOMA_OPT_COUNT_BITS = 17       /* format of the grid arrays in device memory (storage only: soma_fields     */
+                                   /* always returns [type][cell] arrays with uint32 occupation numbers).  32:  */
+                                   /* planes omega[type][cell], uint32 n[type][cell].  16 (n_types = 2 only):   */
+                                   /* one record {omega_A, omega_B} per cell and both occupation numbers in one */
+                                   /* 32-bit word, 16 bits each, as PAPER.md:243 stores them (uint16): 12       */
+                                   /* instead of 16 bytes per cell; a cell with more than 65535 beads of one    */
+                                   /* type is detected whenever the fields are computed -> SOMA_EOVERFLOW.      */
+                                   /* 0 (default): 16 if n_types = 2 and the planes would take more than 48 MB  */
+                                   /* (they no longer stay in L2 beside the positions streaming through), else  */
+                                   /* 32; soma_init and soma_set_positions fall back to 32 on their own if the  */
+                                   /* configuration handed in is too dense (an overflow during later sweeps is  */
+                                   /* reported, not repaired).  Recounts.                                        */
 };
 
 /* indices of soma_kernel_times */

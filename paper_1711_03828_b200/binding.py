@@ -17,6 +17,8 @@ OK = 0
 OPT_HAMILTONIAN, OPT_MOVE, OPT_SMC_STEP, OPT_RECORD_DECISIONS = 1, 2, 3, 4
 OPT_KERNEL, OPT_DENSITY, OPT_TIMING, OPT_SWEEP_COUNTER, OPT_GRAPH, OPT_BLOCKS_PER_SM = 5, 6, 7, 8, 9, 10
 OPT_LAYOUT, OPT_SORT_INTERVAL, OPT_SET_ORDER, OPT_FIELD_INTERVAL, OPT_SCHEME, OPT_PDL = 11, 12, 13, 14, 15, 16
+OPT_COUNT_BITS = 17
+EOVERFLOW = -7
 MOVE_LOCAL, MOVE_SMC = 1, 2
 KERNEL_AUTO, KERNEL_GENERIC, KERNEL_FUSED = 0, 1, 2
 DENSITY_INCREMENTAL, DENSITY_FULL = 0, 1

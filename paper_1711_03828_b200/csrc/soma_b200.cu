@@ -3,9 +3,13 @@
 // Device memory layout:
 //   x, y, z     three fp32 arrays, chain-major; every architecture's segment starts on a 512-byte
 //               boundary (128 floats) so that a warp tile of the fused kernel is 3 x LDG.128 per lane
-//   counts      uint32 [n_types][cells]      (L2-resident for every BASELINE config but C4)
-//   omega       float32 [n_types][cells]
-//   toff        uint32 per monomer of every architecture: type * cells
+//   omega, counts   two formats (soma_ctx::pack, SOMA_OPT_COUNT_BITS):
+//               planes   float32 omega[n_types][cells], uint32 counts[n_types][cells]
+//               records  (two types) omega[cells] = {omega_A, omega_B}; counts uint32 [cells], n_A in the low and
+//                        n_B in the high 16 bits (PAPER.md:243 stores uint16; overflow is detected by the field
+//                        kernel, SOMA_EOVERFLOW): 12 instead of 16 bytes per cell, the default once the planes
+//                        would not stay in L2.  The C ABI's [type][cell] arrays: export_grid_kernel (soma_fields)
+//   toff        uint32 per monomer of every architecture: the offset of its type in omega (type * cells, or type)
 //   decisions   1 bit per bead (only written with SOMA_OPT_RECORD_DECISIONS)
 //   acc_slots   256 spread 64-bit counters of accepted moves
 //   orig        uint32 per chain slot: the caller's index of the chain stored there (soma_layout.cuh);
@@ -103,9 +107,16 @@ struct soma_ctx {
     uint32_t* counts_global = nullptr;   // staging for soma_shard_fields from a host array (allocated on first use)
 
     float *x = nullptr, *y = nullptr, *z = nullptr;
-    uint32_t* counts = nullptr;
-    float* omega = nullptr;
-    uint32_t* toff = nullptr;
+    uint32_t* counts = nullptr;      // planes [n_types][cells], or packed [cells] (pack)
+    float* omega = nullptr;          // planes [n_types][cells], or records [cells][2] (pack)
+    int count_bits = 0;              // SOMA_OPT_COUNT_BITS: 0 auto, 16, 32
+    bool pack = false;               // occupation numbers of two types packed 16 + 16 bits per cell
+    unsigned long long* ticket_sum = nullptr;   // device: ticket and sum of the field kernel's overflow check
+    uint32_t* overflow_host = nullptr;   // pinned, mapped: sticky flag the kernels set (a packed half overflowed)
+    uint32_t* overflow_dev = nullptr;    // its device address
+    void* grid_stage = nullptr;      // [n_types][cells] floats + uint32: soma_fields to host memory (allocated on first use)
+    uint32_t* toff = nullptr;        // per monomer of every architecture: type * cells (planes) or type (records)
+    std::vector<uint32_t> types_host;    // the bead types behind toff
     uint32_t* arch = nullptr;        // architectures given by bond lists (Spec::arch_off)
     float* ext = nullptr;            // [n_types][cells] static external field, or null
     uint8_t* forbidden = nullptr;    // [cells] 1 = no particle may enter, or null
@@ -166,7 +177,7 @@ soma::GridP soma_ctx::gridp() const
     }
     const uint32_t Mb = 0x4B400000u;   // bits of 1.5 * 2^23
     const uint32_t Kx = (g.n[0] - 1u) * Mb, Ky = (g.n[1] - 1u) * Mb, Kz = (g.n[2] - 1u) * Mb;
-    g.k_tot = (Kx * g.n[1] + Ky) * g.n[2] + Kz;
+    g.k_rec = ((Kx * g.n[1] + Ky) * g.n[2] + Kz) * (pack ? 2u : 1u);
     g.cells = (uint32_t)cells;
     g.last = (uint32_t)(cells * (size_t)n_types) - 1u;
     return g;
@@ -288,10 +299,10 @@ cudaError_t launch_pdl(bool pdl, void (*kernel)(KArgs...), unsigned blocks, unsi
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-template <int kMove, bool kIncr, bool kRecord, bool kOrder>
+template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack>
 int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
-    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder>;
+    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder, kPack>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
     constexpr size_t kOrderSmemMax = 160 * 1024;       // shared memory for the order bits of a block's chains
     static int resident[kMaxDevices] = {};             // blocks per SM of this instantiation, asked once per device
@@ -323,7 +334,7 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     return SOMA_OK;
 }
 
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
 int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
 {
     for (const Spec& s : c->specs) {
@@ -336,7 +347,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const uint64_t n_items = s.n_chains * set_size;
                 const int threads = 256;
                 Timed t(c, SOMA_K_MOVE, 1);
-                soma::arch_move_kernel<kMove, kIncr, kRecord><<<(unsigned)((n_items + threads - 1) / threads), threads, 0, c->stream>>>(
+                soma::arch_move_kernel<kMove, kIncr, kRecord, kPack><<<(unsigned)((n_items + threads - 1) / threads), threads, 0, c->stream>>>(
                     P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, nbr_off, nbr,
                     members + s.set_off[i_set], s.N, set_size, n_items, (uint32_t)s.gid0, c->orig + s.chain_off,
                     c->decisions, c->acc_slots);
@@ -348,7 +359,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
             const size_t per_warp = sizeof(float) * 96 * (size_t)s.N;     // 32 chains x 3 coordinates
             const int warps = (int)std::min<size_t>(4, (200 * 1024) / per_warp);
             if (warps >= 1 && c->kernel_choice != 1) {   // chains staged in shared memory
-                auto kernel = soma::molecule_staged_kernel<kMove, kIncr, kRecord>;
+                auto kernel = soma::molecule_staged_kernel<kMove, kIncr, kRecord, kPack>;
                 const size_t smem = per_warp * warps;
                 // shared-memory limit and resident blocks per SM: asked once per (instantiation, device, chain length)
                 static size_t asked_smem[kMaxDevices] = {};
@@ -373,7 +384,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
             const int threads = 128;
             const unsigned blocks = (unsigned)((s.n_chains + threads - 1) / threads);
             Timed t(c, SOMA_K_MOVE, 1);
-            soma::molecule_move_kernel<kMove, kIncr, kRecord><<<blocks, threads, 0, c->stream>>>(
+            soma::molecule_move_kernel<kMove, kIncr, kRecord, kPack><<<blocks, threads, 0, c->stream>>>(
                 P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N,
                 s.n_chains, (uint32_t)s.gid0, c->orig + s.chain_off, c->decisions, c->acc_slots);
             CU(cudaGetLastError());
@@ -383,8 +394,8 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
         if (spec_uses_fused(c, s) && s.n_tiles > 0) {
-            int rc = (kMove == 1 && c->set_order == 1) ? launch_fused<kMove, kIncr, kRecord, kMove == 1>(c, P, s)
-                                                       : launch_fused<kMove, kIncr, kRecord, false>(c, P, s);
+            int rc = (kMove == 1 && c->set_order == 1) ? launch_fused<kMove, kIncr, kRecord, kMove == 1, kPack>(c, P, s)
+                                                       : launch_fused<kMove, kIncr, kRecord, false, kPack>(c, P, s);
             if (rc) return rc;
             done = (uint64_t)s.n_tiles * soma::kTile;
         }
@@ -396,7 +407,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const int threads = 256;
                 const uint64_t blocks = (n_items + threads - 1) / threads;
                 Timed t(c, SOMA_K_MOVE, 1);
-                soma::generic_move_kernel<kMove, kIncr, kRecord><<<(unsigned)blocks, threads, 0, c->stream>>>(
+                soma::generic_move_kernel<kMove, kIncr, kRecord, kPack><<<(unsigned)blocks, threads, 0, c->stream>>>(
                     P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity,
                     (uint32_t)c->set_order, n_items,
                     (uint32_t)s.gid0, c->orig + s.chain_off + done / s.N, c->decisions, c->acc_slots);
@@ -407,29 +418,57 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
     return SOMA_OK;
 }
 
+template <int kMove, bool kIncr, bool kRecord>
+int launch_moves_3(soma_ctx* c, const soma::MoveP& P)
+{
+    return c->pack ? launch_moves_t<kMove, kIncr, kRecord, true>(c, P) : launch_moves_t<kMove, kIncr, kRecord, false>(c, P);
+}
+template <int kMove, bool kIncr>
+int launch_moves_2(soma_ctx* c, const soma::MoveP& P)
+{
+    return c->record ? launch_moves_3<kMove, kIncr, true>(c, P) : launch_moves_3<kMove, kIncr, false>(c, P);
+}
+template <int kMove>
+int launch_moves_1(soma_ctx* c, const soma::MoveP& P)
+{
+    return c->density_mode == 0 ? launch_moves_2<kMove, true>(c, P) : launch_moves_2<kMove, false>(c, P);
+}
 int launch_moves(soma_ctx* c, const soma::MoveP& P)
 {
-    const bool incr = c->density_mode == 0;
-    const bool rec = c->record != 0;
-#define SOMA_DISPATCH(M)                                                        \
-    if (incr) {                                                                 \
-        return rec ? launch_moves_t<M, true, true>(c, P) : launch_moves_t<M, true, false>(c, P);   \
-    } else {                                                                    \
-        return rec ? launch_moves_t<M, false, true>(c, P) : launch_moves_t<M, false, false>(c, P); \
-    }
-    if (c->move == 2) {
-        SOMA_DISPATCH(2)
-    } else {
-        SOMA_DISPATCH(1)
-    }
-#undef SOMA_DISPATCH
+    return c->move == 2 ? launch_moves_1<2>(c, P) : launch_moves_1<1>(c, P);
+}
+
+// Which grid format SOMA_OPT_COUNT_BITS asks for.  Auto (0): records with packed counters for two bead types
+// once the planes (16 bytes per cell) would take more than kPackAutoBytes -- measured on a B200 (126 MB L2):
+// C3 (8 MB of planes) 100.3 us per step with planes, 104.3 with records (the packed update costs ~20
+// instructions per 128 moves in an issue-bound kernel); C4 (131 MB) 1908 against 1758.
+constexpr size_t kPackAutoBytes = 48u << 20;
+bool want_pack(const soma_ctx* c)
+{
+    if (c->n_types != 2 || c->count_bits == 32) return false;
+    return c->count_bits == 16 || 16 * (size_t)c->cells > kPackAutoBytes;
+}
+
+// toff follows the grid format: call after c->pack changed.  Synchronises (host vector goes out of scope).
+int upload_toff(soma_ctx* c)
+{
+    std::vector<uint32_t> t(c->types_host.size());
+    for (size_t i = 0; i < t.size(); ++i) t[i] = c->types_host[i] * (c->pack ? 1u : (uint32_t)c->cells);
+    CU(cudaMemcpyAsync(c->toff, t.data(), sizeof(uint32_t) * t.size(), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return SOMA_OK;
+}
+
+size_t counts_bytes(const soma_ctx* c)
+{
+    return sizeof(uint32_t) * c->cells * (c->pack ? 1 : (size_t)c->n_types);
 }
 
 // check_domain: also count the beads whose coordinates lie outside the supported domain (stage 1 of new
 // positions); the per-sweep histograms of SOMA_OPT_DENSITY = 1 do not -- moves cannot leave the domain
 int launch_histogram(soma_ctx* c, bool check_domain_too)
 {
-    CU(cudaMemsetAsync(c->counts, 0, sizeof(uint32_t) * c->cells * c->n_types, c->stream));
+    CU(cudaMemsetAsync(c->counts, 0, counts_bytes(c), c->stream));
     const soma::GridP g = c->gridp();
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
@@ -438,7 +477,8 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
         const uint64_t cap = (uint64_t)c->n_sm * 16;
         if (blocks > cap) blocks = cap;
         Timed t(c, SOMA_K_DENSITY, 1);
-        soma::histogram_kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
+        auto kernel = c->pack ? soma::histogram_kernel<true> : soma::histogram_kernel<false>;
+        kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
             g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts,
             check_domain_too ? c->n_outside : nullptr);
         CU(cudaGetLastError());
@@ -446,9 +486,11 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
     return SOMA_OK;
 }
 
-int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr)
+// counts_src: occupation numbers in the internal layout (default: this context's own), n_counted: the beads
+// they count (the packed format's overflow check, soma::CountCheck)
+int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr, uint64_t n_counted = 0)
 {
-    if (!counts_src) counts_src = c->counts;
+    if (!counts_src) { counts_src = c->counts; n_counted = c->n_beads; }
     const soma::FieldP F = c->fieldp();
 #ifndef SOMA_FIELD_THREADS
 #define SOMA_FIELD_THREADS 256
@@ -457,24 +499,17 @@ int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr)
     const unsigned blocks = (unsigned)((c->cells + threads - 1) / threads);
     Timed t(c, SOMA_K_FIELD, 1);
     const bool pdl = c->pdl != 0;
-#ifndef SOMA_FIELD_V4
-#define SOMA_FIELD_V4 1
-#endif
-    // Four cells per thread with 128-bit accesses is the faster field kernel when it starts after the move
-    // kernel has ended (4.1 -> 2.8 us at C3); with programmatic dependent launch the many small blocks of
-    // the one-cell-per-thread kernel slip in behind the draining move blocks and the step is shorter.
-    if (SOMA_FIELD_V4 && !pdl && c->cells % 4 == 0 && c->n_types <= 2) {
-        const unsigned blocks4 = (unsigned)((c->cells / 4 + threads - 1) / threads);
-        if (c->n_types == 1)
-            CU(launch_pdl(pdl, soma::field_kernel_v4<1>, blocks4, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden));
-        else
-            CU(launch_pdl(pdl, soma::field_kernel_v4<2>, blocks4, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden));
+    // One cell per thread: with programmatic dependent launch the many small blocks slip in behind the
+    // draining move blocks.
+    const unsigned long long n = n_counted;
+    if (c->pack) {
+        CU(launch_pdl(pdl, soma::field_kernel<2, true>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n));
         return SOMA_OK;
     }
     switch (c->n_types) {
-        case 1: CU(launch_pdl(pdl, soma::field_kernel<1>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
-        case 2: CU(launch_pdl(pdl, soma::field_kernel<2>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
-        default: CU(launch_pdl(pdl, soma::field_kernel<0>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden)); break;
+        case 1: CU(launch_pdl(pdl, soma::field_kernel<1, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
+        case 2: CU(launch_pdl(pdl, soma::field_kernel<2, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
+        default: CU(launch_pdl(pdl, soma::field_kernel<0, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
     }
     return SOMA_OK;
 }
@@ -497,13 +532,46 @@ int check_domain(soma_ctx* c, const char* who)
                 "domain |x n / L| < 2^22 per axis", who, bad);
 }
 
-int stage1(soma_ctx* c)
+// The sticky flag of the packed occupation numbers (soma::field_kernel): valid after a synchronisation.
+int check_overflow(soma_ctx* c, const char* who)
+{
+    if (!*(volatile uint32_t*)c->overflow_host) return SOMA_OK;
+    return fail(SOMA_EOVERFLOW, "%s: a cell holds more than 65535 beads of one type, which the packed 16-bit "
+                "occupation numbers cannot count; set SOMA_OPT_COUNT_BITS to 32 and restart from a configuration "
+                "saved before", who);
+}
+
+int stage1_once(soma_ctx* c)
 {
     CU(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
     int rc = launch_histogram(c, true);
     if (rc) return rc;
-    if (c->sharded) return SOMA_OK;   // omega needs every rank's counts: soma_shard_fields
+    // a shard's omega needs every rank's counts (soma_shard_fields); the launch here is the overflow check
+    // of its own packed counts (the field it writes is replaced before the first move)
+    if (c->sharded && !c->pack) return SOMA_OK;
     return launch_fields(c);
+}
+
+// Stage 1 on new positions (soma_init, soma_set_positions): occupation numbers, fields, and the checks of
+// the coordinate domain and of the packed counters.  Synchronises.  With SOMA_OPT_COUNT_BITS = 0 (auto) a
+// configuration too dense for 16 + 16 bits switches the context to 32-bit counters.
+int stage1(soma_ctx* c, const char* who)
+{
+    int rc = stage1_once(c);
+    if (rc) return rc;
+    rc = check_domain(c, who);
+    if (rc) return rc;
+    if (c->pack && *(volatile uint32_t*)c->overflow_host) {
+        if (c->count_bits == 16) return check_overflow(c, who);
+        *(volatile uint32_t*)c->overflow_host = 0u;
+        c->pack = false;
+        rc = upload_toff(c);
+        if (rc) return rc;
+        rc = stage1_once(c);
+        if (rc) return rc;
+        CU(cudaStreamSynchronize(c->stream));
+    }
+    return SOMA_OK;
 }
 
 // ---- layout: Hilbert order of the chains, caller order <-> device order ---------------------------
@@ -602,6 +670,9 @@ void soma_destroy(soma_ctx* c)
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
     cudaFree(c->counts_global);
     cudaFree(c->n_outside);
+    cudaFree(c->ticket_sum);
+    cudaFree(c->grid_stage);
+    if (c->overflow_host) cudaFreeHost(c->overflow_host);
     cudaFree(c->counts); cudaFree(c->omega); cudaFree(c->toff); cudaFree(c->decisions);
     cudaFree(c->ext); cudaFree(c->forbidden); cudaFree(c->arch);
     cudaFree(c->acc_slots);
@@ -734,7 +805,7 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
                 delete c;
                 return fail(SOMA_EINVAL, "soma_init: spec %d monomer %u has type %u >= n_types", a, j, (unsigned)t);
             }
-            toff_host.push_back((uint32_t)(t * cells));
+            toff_host.push_back((uint32_t)t);
         }
         while (toff_host.size() % 4) toff_host.push_back(0);  // uint4 loads of the fused kernel
         gid += s.n_beads;
@@ -810,6 +881,12 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     CUI(cudaMalloc(&c->decisions, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32 + 8)));
     CUI(cudaMalloc(&c->acc_slots, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMalloc(&c->n_outside, sizeof(uint32_t)));
+    CUI(cudaMalloc(&c->ticket_sum, sizeof(unsigned long long)));
+    CUI(cudaMemsetAsync(c->ticket_sum, 0, sizeof(unsigned long long), c->stream));
+    CUI(cudaHostAlloc(&c->overflow_host, sizeof(uint32_t), cudaHostAllocMapped));
+    *c->overflow_host = 0u;
+    CUI(cudaHostGetDevicePointer((void**)&c->overflow_dev, c->overflow_host, 0));
+    c->pack = want_pack(c);
     CUI(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
     CUI(cudaMallocHost(&c->acc_host, sizeof(unsigned long long) * soma::kAccSlots));
     CUI(cudaMemsetAsync(c->x, 0, sizeof(float) * c->n_pad, c->stream));
@@ -817,8 +894,8 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     CUI(cudaMemsetAsync(c->z, 0, sizeof(float) * c->n_pad, c->stream));
     CUI(cudaMemsetAsync(c->decisions, 0, sizeof(uint32_t) * ((c->n_beads_global + 31) / 32 + 8), c->stream));
     CUI(cudaMemsetAsync(c->acc_slots, 0, sizeof(unsigned long long) * soma::kAccSlots, c->stream));
-    CUI(cudaMemcpyAsync(c->toff, toff_host.data(), sizeof(uint32_t) * toff_host.size(), cudaMemcpyHostToDevice, c->stream));
-    CUI(cudaStreamSynchronize(c->stream));  // toff_host goes out of scope
+    c->types_host = toff_host;
+    if (upload_toff(c) != SOMA_OK) { soma_destroy(c); return SOMA_ECUDA; }
 
     int rc = SOMA_OK;
     if (host_xyz0) {
@@ -837,8 +914,7 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
         if (cudaGetLastError() != cudaSuccess) rc = fail(SOMA_ECUDA, "soma_init: init_walk_kernel launch failed");
     }
     if (rc == SOMA_OK) rc = resort(c);
-    if (rc == SOMA_OK) rc = stage1(c);
-    if (rc == SOMA_OK) rc = check_domain(c, "soma_init");
+    if (rc == SOMA_OK) rc = stage1(c, "soma_init");
     if (rc == SOMA_OK && cudaStreamSynchronize(c->stream) != cudaSuccess)
         rc = fail(SOMA_ECUDA, "soma_init: %s", cudaGetErrorString(cudaGetLastError()));
     if (rc != SOMA_OK) {
@@ -899,7 +975,7 @@ static int check_step(soma_ctx* c, const char* who)
             if (s.general)
                 return fail(SOMA_ESTATE, "%s: architectures given by a bond list support SOMA_OPT_SCHEME 0 and SOMA_OPT_SET_ORDER 0 only", who);
     if (c->sharded) {
-        // a part of a larger system is checked against the oracle for linear chains in the set scheme only
+        // a part of a larger system is parity-checked for linear chains in the set scheme only
         if (c->scheme == 1)
             return fail(SOMA_ESTATE, "%s: a shard supports SOMA_OPT_SCHEME 0 only", who);
         for (const Spec& s : c->specs)
@@ -916,6 +992,8 @@ int soma_step(soma_ctx* c, int n_sweeps)
     if (n_sweeps < 0) return fail(SOMA_EINVAL, "soma_step: n_sweeps must be >= 0");
     if (c->sharded) return fail(SOMA_ESTATE, "soma_step: this context is a shard: use soma_shard_moves / soma_shard_fields");
     int rc = check_step(c, "soma_step");
+    if (rc) return rc;
+    rc = check_overflow(c, "soma_step");                   // of the sweeps that have completed so far
     if (rc) return rc;
     for (int i = 0; i < n_sweeps; ++i) {
         rc = sweep_moves(c);
@@ -950,15 +1028,21 @@ int soma_shard_fields(soma_ctx* c, const uint32_t* global_counts, int src_is_dev
     if (!c || !global_counts) return fail(SOMA_EINVAL, "soma_shard_fields: NULL argument");
     DeviceGuard on_device(c->device);
     if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_fields: the context was not created by soma_init_shard");
+    // counts_global: 2 x [n_types][cells] words, the caller's array (if it is host memory) and its internal layout
+    const size_t n = (size_t)c->cells * c->n_types;
+    if (!c->counts_global) CU(cudaMalloc(&c->counts_global, 2 * sizeof(uint32_t) * n));
     const uint32_t* src = global_counts;
     if (!src_is_device) {
-        const size_t bytes = sizeof(uint32_t) * c->cells * c->n_types;
-        if (!c->counts_global) CU(cudaMalloc(&c->counts_global, bytes));
-        CU(cudaMemcpyAsync(c->counts_global, global_counts, bytes, cudaMemcpyHostToDevice, c->stream));
-        src = c->counts_global;
+        CU(cudaMemcpyAsync(c->counts_global + n, global_counts, sizeof(uint32_t) * n, cudaMemcpyHostToDevice, c->stream));
+        src = c->counts_global + n;
     }
     if (!advance || c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
-        int rc = launch_fields(c, src);                    // a4 from the occupation numbers of the whole system
+        const unsigned blocks = (unsigned)((c->cells + 255) / 256);
+        c->launches += 1;
+        if (c->pack) soma::import_counts_kernel<true><<<blocks, 256, 0, c->stream>>>(src, (uint32_t)c->cells, (uint32_t)c->n_types, c->counts_global, c->overflow_dev);
+        else soma::import_counts_kernel<false><<<blocks, 256, 0, c->stream>>>(src, (uint32_t)c->cells, (uint32_t)c->n_types, c->counts_global, c->overflow_dev);
+        CU(cudaGetLastError());
+        int rc = launch_fields(c, c->counts_global, c->n_beads_global);   // a4 from the occupation numbers of the whole system
         if (rc) return rc;
     }
     if (advance) c->sweep += 1;
@@ -971,11 +1055,26 @@ int soma_fields(soma_ctx* c, float* omega, uint32_t* counts, int dst_is_device)
     if (!c) return fail(SOMA_EINVAL, "soma_fields: ctx is NULL");
     DeviceGuard on_device(c->device);
     if (!omega && !counts) return fail(SOMA_EINVAL, "soma_fields: both outputs NULL");
-    const cudaMemcpyKind kind = dst_is_device ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost;
+    // internal layout (records per cell, packed occupation numbers) -> the caller's [type][cell] arrays
     const size_t n = (size_t)c->cells * c->n_types;
-    if (omega) CU(cudaMemcpyAsync(omega, c->omega, sizeof(float) * n, kind, c->stream));
-    if (counts) CU(cudaMemcpyAsync(counts, c->counts, sizeof(uint32_t) * n, kind, c->stream));
-    if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
+    float* dev_omega = omega;
+    uint32_t* dev_counts = counts;
+    if (!dst_is_device) {
+        if (!c->grid_stage) CU(cudaMalloc(&c->grid_stage, 2 * sizeof(float) * n));
+        dev_omega = omega ? (float*)c->grid_stage : nullptr;
+        dev_counts = counts ? (uint32_t*)c->grid_stage + n : nullptr;
+    }
+    const unsigned blocks = (unsigned)((n + 255) / 256);
+    c->launches += 1;
+    if (c->pack) soma::export_grid_kernel<true><<<blocks, 256, 0, c->stream>>>(c->omega, c->counts, (uint32_t)c->cells, (uint32_t)c->n_types, dev_omega, dev_counts);
+    else soma::export_grid_kernel<false><<<blocks, 256, 0, c->stream>>>(c->omega, c->counts, (uint32_t)c->cells, (uint32_t)c->n_types, dev_omega, dev_counts);
+    CU(cudaGetLastError());
+    if (!dst_is_device) {
+        if (omega) CU(cudaMemcpyAsync(omega, dev_omega, sizeof(float) * n, cudaMemcpyDeviceToHost, c->stream));
+        if (counts) CU(cudaMemcpyAsync(counts, dev_counts, sizeof(uint32_t) * n, cudaMemcpyDeviceToHost, c->stream));
+        CU(cudaStreamSynchronize(c->stream));
+        return check_overflow(c, "soma_fields");
+    }
     return SOMA_OK;
 }
 
@@ -985,7 +1084,10 @@ int soma_positions(soma_ctx* c, float* xyz, int dst_is_device)
     DeviceGuard on_device(c->device);
     int rc = copy_soa(c, xyz, nullptr, true, dst_is_device != 0);
     if (rc) return rc;
-    if (!dst_is_device) CU(cudaStreamSynchronize(c->stream));
+    if (!dst_is_device) {
+        CU(cudaStreamSynchronize(c->stream));
+        return check_overflow(c, "soma_positions");
+    }
     return SOMA_OK;
 }
 
@@ -1000,9 +1102,12 @@ int soma_set_positions(soma_ctx* c, const float* xyz, int src_is_device)
     // next periodic re-sort forward to eight sweeps from now instead of sorting on every call.
     if (c->layout && c->sort_interval > 8)
         c->sweeps_since_sort = std::max<uint64_t>(c->sweeps_since_sort, (uint64_t)c->sort_interval - 8);
-    rc = stage1(c);
-    if (rc) return rc;
-    return check_domain(c, "soma_set_positions");   // synchronises: the caller may reuse its buffer
+    if (c->pack != want_pack(c)) {   // auto: try the packed counters again if an earlier configuration was too dense
+        c->pack = want_pack(c);
+        rc = upload_toff(c);
+        if (rc) return rc;
+    }
+    return stage1(c, "soma_set_positions");   // synchronises: the caller may reuse its buffer
 }
 
 int soma_set_chi(soma_ctx* c, int i, int j, float chiN_ij)
@@ -1139,6 +1244,20 @@ int soma_set_option(soma_ctx* c, int key, double value)
             if (iv < 1) return fail(SOMA_EINVAL, "SOMA_OPT_FIELD_INTERVAL: must be >= 1");
             c->field_interval = iv;
             return SOMA_OK;
+        case SOMA_OPT_COUNT_BITS: {
+            if (iv != 0 && iv != 16 && iv != 32) return fail(SOMA_EINVAL, "SOMA_OPT_COUNT_BITS: 0 (auto), 16 or 32");
+            if (iv == 16 && c->n_types != 2) return fail(SOMA_EINVAL, "SOMA_OPT_COUNT_BITS=16: the packed format holds two bead types");
+            c->count_bits = iv;
+            const bool want = want_pack(c);
+            CU(cudaStreamSynchronize(c->stream));
+            if (want == c->pack && !*(volatile uint32_t*)c->overflow_host) return SOMA_OK;
+            // recount in the new format (the flag of an earlier overflow goes with the old counters)
+            *(volatile uint32_t*)c->overflow_host = 0u;
+            c->pack = want;
+            int rc = upload_toff(c);
+            if (rc) return rc;
+            return stage1(c, "SOMA_OPT_COUNT_BITS");
+        }
         case SOMA_OPT_SORT_INTERVAL:
             if (iv < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SORT_INTERVAL: must be >= 0");
             c->sort_interval = iv;
@@ -1160,7 +1279,7 @@ int soma_stats(soma_ctx* c, uint64_t* attempted, uint64_t* accepted, uint64_t* s
     if (attempted) *attempted = c->attempted;
     if (accepted) *accepted = acc;
     if (sweeps_done) *sweeps_done = c->sweep;
-    return SOMA_OK;
+    return check_overflow(c, "soma_stats");
 }
 
 int soma_decisions(soma_ctx* c, uint32_t* bits, int dst_is_device)
@@ -1201,7 +1320,7 @@ int soma_sync(soma_ctx* c)
     DeviceGuard on_device(c->device);
     CU(cudaStreamSynchronize(c->stream));
     CU(cudaGetLastError());
-    return SOMA_OK;
+    return check_overflow(c, "soma_sync");
 }
 
 }  // extern "C"

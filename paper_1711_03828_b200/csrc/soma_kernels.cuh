@@ -47,9 +47,10 @@ struct GridP {
     float nf[3];      // (float) n_a
     uint32_t n[3];
     uint32_t neg_n[3];  // -n_a (mod 2^32)
-    uint32_t k_tot;     // ((K_x n_y + K_y) n_z + K_z) mod 2^32, K_a = (n_a - 1) 0x4B400000: see cell_raw()
+    uint32_t k_rec;     // f * ((K_x n_y + K_y) n_z + K_z) mod 2^32, K_a = (n_a - 1) 0x4B400000 (see cell_raw()); f = 1
+                        // for planes, 2 for records per cell (see cell_at())
     uint32_t cells;
-    uint32_t last;      // n_types * cells - 1: the last valid index of omega / counts
+    uint32_t last;      // n_types * cells - 1: the last valid index of omega
 };
 
 struct MoveP {
@@ -203,9 +204,16 @@ __device__ __forceinline__ float sqrt_approx(float x)
 // bits(B) - n_a bits(A) + K_a in 32-bit wrap-around arithmetic; the three constants are folded into one,
 //   cell = ((cx ny + cy) nz + cz) = (((Bx - nx Ax) ny + By - ny Ay) nz + Bz - nz Az) + k_tot,
 // five IMADs.  FMUL, FADD.RM, FFMA.RM per axis; no FRND / F2I (XU pipe), no fold of the fraction, no
-// per-axis clamp.  cell_raw() returns the sum without k_tot; cell_at() adds k_tot and the offset of the
-// bead type's plane in omega / counts (toff = type * cells) in one go, and its unsigned min keeps the
-// index inside the arrays for every input (NaN, or coordinates outside the domain).
+// per-axis clamp.  cell_raw() returns the sum without k_tot.  cell_at() returns the index of the bead's
+// field value in omega; it adds k_tot and the type's offset in one go (tk = toff + k_rec; toff = type * cells
+// for planes, = type for records: the table the host keeps per monomer), and its
+// unsigned min keeps the index inside the array for every input (NaN, coordinates outside the domain).
+// Two grid formats:
+//   planes (kPack = false, any number of types)  omega[type][cell], counts uint32 [type][cell]; index = cell + tk
+//   records (kPack = true, two types)            omega[cell] = {omega_A, omega_B}; the occupation numbers of a
+//          cell are one 32-bit word, n_A in the low and n_B in the high 16 bits (the paper stores uint16,
+//          PAPER.md:243): 12 instead of 16 bytes of grid data per cell, which pays once the grids outgrow L2.
+//          index = 2 cell + type is one three-input add.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ uint32_t cell_raw(const GridP& g, float x, float y, float z)
 {
@@ -222,10 +230,12 @@ __device__ __forceinline__ uint32_t cell_raw(const GridP& g, float x, float y, f
     return u;
 }
 
-// toff_k = toff + k_tot
-__device__ __forceinline__ uint32_t cell_at(const GridP& g, float x, float y, float z, uint32_t toff_k)
+// tk = type + k_rec
+template <bool kPack>
+__device__ __forceinline__ uint32_t cell_at(const GridP& g, float x, float y, float z, uint32_t tk)
 {
-    return min(cell_raw(g, x, y, z) + toff_k, g.last);
+    const uint32_t u = cell_raw(g, x, y, z);
+    return min(kPack ? u + u + tk : u + tk, g.last);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -355,20 +365,30 @@ __device__ __forceinline__ void smc_proposal(const MoveP& P, float mf, float sx,
 
 // The occupation numbers follow an accepted move (+1 new cell, -1 old cell): integer arithmetic, so
 // they stay identical to a fresh histogram (a3, Eq. 4).
+// i_old, i_new: cell_at() of the old and the new position (same type).  kPack: the cell's word is index >> 1,
+// the type's half index & 1; the sums are exact modulo 2^32 whatever the order of the updates, so the word
+// always holds n_A + 65536 n_B (the field kernel checks that no half has outgrown its 16 bits).
+template <bool kPack>
 __device__ __forceinline__ void count_follow(uint32_t* __restrict__ counts, bool acc, uint32_t i_old, uint32_t i_new)
 {
     if (acc && i_new != i_old) {
-        atomicAdd(counts + i_new, 1u);
-        atomicAdd(counts + i_old, 0xFFFFFFFFu);
+        if (kPack) {
+            const uint32_t one = 1u << ((i_new & 1u) << 4);
+            atomicAdd(counts + (i_new >> 1), one);
+            atomicAdd(counts + (i_old >> 1), 0u - one);
+        } else {
+            atomicAdd(counts + i_new, 1u);
+            atomicAdd(counts + i_old, 0xFFFFFFFFu);
+        }
     }
 }
 
 // One whole move of one bead (generic kernels).  (x,y,z) is updated in place when accepted.
 //   (sx,sy,sz)     s = sum over the bonded neighbours of (r - r_nb), Eq. 2
 //   mf             number of bonded neighbours as float
-//   toff           type * cells, offset of this bead type's plane in omega / counts
+//   toff           offset of the bead type in omega: type * cells (planes) or type (records)
 //   gid            global bead index = Philox counter word 0
-template <int kMove, bool kIncr>
+template <int kMove, bool kIncr, bool kPack>
 __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restrict__ omega,
                                           uint32_t* __restrict__ counts, float& x, float& y, float& z,
                                           float sx, float sy, float sz, float mf, uint32_t toff, uint32_t gid)
@@ -377,8 +397,8 @@ __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restric
     float dx = q.a, dy = q.b, dz = q.c, log_ratio = 0.0f;
     if (kMove == 2) smc_proposal(P, mf, sx, sy, sz, q, dx, dy, dz, log_ratio);
     const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
-    const uint32_t i_old = cell_at(P.g, x, y, z, toff + P.g.k_tot);
-    const uint32_t i_new = cell_at(P.g, x2, y2, z2, toff + P.g.k_tot);
+    const uint32_t i_old = cell_at<kPack>(P.g, x, y, z, toff + P.g.k_rec);
+    const uint32_t i_new = cell_at<kPack>(P.g, x2, y2, z2, toff + P.g.k_rec);
     const float e_nb = field_delta(omega, i_old, i_new);
     const float e_b = bonded_delta(kMove == 1 ? P.hk : 0.5f * P.k0, mf, dx, dy, dz, sx, sy, sz);
     float dE = e_b + e_nb;
@@ -387,12 +407,12 @@ __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restric
     x = acc ? x2 : x;
     y = acc ? y2 : y;
     z = acc ? z2 : z;
-    if (kIncr) count_follow(counts, acc, i_old, i_new);
+    if (kIncr) count_follow<kPack>(counts, acc, i_old, i_new);
     return acc;
 }
 
 // The same for a monomer of a linear chain, from its two chain neighbours.
-template <int kMove, bool kIncr>
+template <int kMove, bool kIncr, bool kPack>
 __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict__ omega,
                                         uint32_t* __restrict__ counts, float& x, float& y, float& z,
                                         float xl, float yl, float zl, float xr, float yr, float zr,
@@ -400,7 +420,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 {
     float sx, sy, sz;
     bond_sum(x, y, z, xl, yl, zl, xr, yr, zr, sx, sy, sz);
-    return mc_move_s<kMove, kIncr>(P, omega, counts, x, y, z, sx, sy, sz, mf, toff, gid);
+    return mc_move_s<kMove, kIncr, kPack>(P, omega, counts, x, y, z, sx, sy, sz, mf, toff, gid);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -418,7 +438,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 //   5. count updates for the accepted moves, one 128-bit store per coordinate array.
 // Smart-MC proposals depend on the neighbours, so there steps 3-4 run per set.
 //   x,y,z       base of this architecture's beads (padded layout)
-//   toff_tab    [N] type * cells of every monomer of the chain
+//   toff_tab    [N] offset of every monomer's type in omega (type * cells, or type for records per cell)
 //   n_tiles     full tiles of this architecture (n_chains * N / 128)
 //   gid0        global index of the architecture's first bead
 //   orig        [n_chains] the caller's chain index of the chain in each slot (Philox counter, bitmap)
@@ -426,7 +446,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 // kOrder: dynamic shared memory = one byte per chain of the block's tile range (the host keeps the ranges
 // short enough); the block draws the order bit of all its chains before it waits for its predecessor.
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord, bool kOrder>
+template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack>
 __global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -443,7 +463,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
     const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
     const uint4 toff = *reinterpret_cast<const uint4*>(toff_tab + j0);
-    const uint4 tk = make_uint4(toff.x + P.g.k_tot, toff.y + P.g.k_tot, toff.z + P.g.k_tot, toff.w + P.g.k_tot);
+    const uint4 tk = make_uint4(toff.x + P.g.k_rec, toff.y + P.g.k_rec, toff.z + P.g.k_rec, toff.w + P.g.k_rec);
     const float mf0 = has_l0 ? 2.0f : 1.0f, mf3 = has_r3 ? 2.0f : 1.0f;
     const float half_k0 = kMove == 1 ? P.hk : 0.5f * P.k0;
     uint32_t n_acc = 0;
@@ -508,10 +528,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             const float x1n = X.y + q1.a, y1n = Y.y + q1.b, z1n = Z.y + q1.c;
             const float x2n = X.z + q2.a, y2n = Y.z + q2.b, z2n = Z.z + q2.c;
             const float x3n = X.w + q3.a, y3n = Y.w + q3.b, z3n = Z.w + q3.c;
-            const uint32_t o0 = cell_at(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at(P.g, x0n, y0n, z0n, tk.x);
-            const uint32_t o1 = cell_at(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at(P.g, x1n, y1n, z1n, tk.y);
-            const uint32_t o2 = cell_at(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at(P.g, x2n, y2n, z2n, tk.z);
-            const uint32_t o3 = cell_at(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at(P.g, x3n, y3n, z3n, tk.w);
+            const uint32_t o0 = cell_at<kPack>(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at<kPack>(P.g, x0n, y0n, z0n, tk.x);
+            const uint32_t o1 = cell_at<kPack>(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at<kPack>(P.g, x1n, y1n, z1n, tk.y);
+            const uint32_t o2 = cell_at<kPack>(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at<kPack>(P.g, x2n, y2n, z2n, tk.z);
+            const uint32_t o3 = cell_at<kPack>(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at<kPack>(P.g, x3n, y3n, z3n, tk.w);
             const float e0 = field_delta(omega, o0, n0), e1 = field_delta(omega, o1, n1),
                         e2 = field_delta(omega, o2, n2), e3 = field_delta(omega, o3, n3);
 
@@ -577,10 +597,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
             // 5. occupation numbers follow the accepted moves
             if (kIncr) {
-                count_follow(counts, a0, o0, n0);
-                count_follow(counts, a1, o1, n1);
-                count_follow(counts, a2, o2, n2);
-                count_follow(counts, a3, o3, n3);
+                count_follow<kPack>(counts, a0, o0, n0);
+                count_follow<kPack>(counts, a1, o1, n1);
+                count_follow<kPack>(counts, a2, o2, n2);
+                count_follow<kPack>(counts, a3, o3, n3);
             }
         } else {
             // Smart-MC: the proposal needs the bonded force, i.e. the neighbours as they are now
@@ -593,14 +613,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, 2.0f, sx2, sy2, sz2, q2, dx2, dy2, dz2, lr2);
             const float x0n = X.x + dx0, y0n = Y.x + dy0, z0n = Z.x + dz0;
             const float x2n = X.z + dx2, y2n = Y.z + dy2, z2n = Z.z + dz2;
-            const uint32_t o0 = cell_at(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at(P.g, x0n, y0n, z0n, tk.x);
-            const uint32_t o2 = cell_at(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at(P.g, x2n, y2n, z2n, tk.z);
+            const uint32_t o0 = cell_at<kPack>(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at<kPack>(P.g, x0n, y0n, z0n, tk.x);
+            const uint32_t o2 = cell_at<kPack>(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at<kPack>(P.g, x2n, y2n, z2n, tk.z);
             const float e0 = field_delta(omega, o0, n0), e2 = field_delta(omega, o2, n2);
             a0 = metropolis((bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0) + e0) + lr0, q0.u);
             a2 = metropolis((bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2) + e2) + lr2, q2.u);
             X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
             X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
-            if (kIncr) { count_follow(counts, a0, o0, n0); count_follow(counts, a2, o2, n2); }
+            if (kIncr) { count_follow<kPack>(counts, a0, o0, n0); count_follow<kPack>(counts, a2, o2, n2); }
 
             float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
             xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
@@ -611,14 +631,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             smc_proposal(P, mf3, sx3, sy3, sz3, q3, dx3, dy3, dz3, lr3);
             const float x1n = X.y + dx1, y1n = Y.y + dy1, z1n = Z.y + dz1;
             const float x3n = X.w + dx3, y3n = Y.w + dy3, z3n = Z.w + dz3;
-            const uint32_t o1 = cell_at(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at(P.g, x1n, y1n, z1n, tk.y);
-            const uint32_t o3 = cell_at(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at(P.g, x3n, y3n, z3n, tk.w);
+            const uint32_t o1 = cell_at<kPack>(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at<kPack>(P.g, x1n, y1n, z1n, tk.y);
+            const uint32_t o3 = cell_at<kPack>(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at<kPack>(P.g, x3n, y3n, z3n, tk.w);
             const float e1 = field_delta(omega, o1, n1), e3 = field_delta(omega, o3, n3);
             a1 = metropolis((bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1) + e1) + lr1, q1.u);
             a3 = metropolis((bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3) + e3) + lr3, q3.u);
             X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
             X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
-            if (kIncr) { count_follow(counts, a1, o1, n1); count_follow(counts, a3, o3, n3); }
+            if (kIncr) { count_follow<kPack>(counts, a1, o1, n1); count_follow<kPack>(counts, a3, o3, n3); }
         }
 
         st_stream(x + i0, X);
@@ -648,7 +668,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 //   half  = ceil(N / 2) threads per chain; n_items = n_chains * half; parity = 0, 1: first, second set
 //   set_order  0: the first set is the even monomers; 1: the chain's first_set_bit decides
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
 __global__ void __launch_bounds__(256)
 generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                     const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -674,7 +694,7 @@ generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y,
         const float xr = has_r ? x[i + 1] : px, yr = has_r ? y[i + 1] : py, zr = has_r ? z[i + 1] : pz;
         const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
         const uint32_t gid = gid0 + orig[chain] * N + j;   // the chain's identity, not its slot (soma_layout.cuh)
-        acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf, toff_tab[j], gid);
+        acc = mc_move<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf, toff_tab[j], gid);
         if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
         if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
     }
@@ -690,7 +710,7 @@ generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y,
 // 32-bit words:  nbr_off[N + 1] | nbr[2 n_bonds] (ascending per monomer) | members[N] (set by set).
 // The bond sum s of Eq. 2 runs over the neighbour list in that order.
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
 __global__ void __launch_bounds__(256)
 arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                  const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -714,7 +734,7 @@ arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, fl
             if (a == a0) { sx = bx; sy = by; sz = bz; } else { sx = sx + bx; sy = sy + by; sz = sz + bz; }
         }
         const uint32_t gid = gid0 + orig[mol] * N + j;
-        acc = mc_move_s<kMove, kIncr>(P, omega, counts, px, py, pz, sx, sy, sz, (float)(a1 - a0), toff_tab[j], gid);
+        acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, sx, sy, sz, (float)(a1 - a0), toff_tab[j], gid);
         if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
         if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
     }
@@ -733,7 +753,7 @@ arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, fl
 // thread, so they stay in L1; lanes of a warp work on 32 consecutive chains.
 //   dec_words   bit of attempt f + k (not of a bead), or unused
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
 __global__ void __launch_bounds__(128)
 molecule_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                      const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -757,7 +777,7 @@ molecule_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y
             const float xl = has_l ? x[i - 1] : px, yl = has_l ? y[i - 1] : py, zl = has_l ? z[i - 1] : pz;
             const float xr = has_r ? x[i + 1] : px, yr = has_r ? y[i + 1] : py, zr = has_r ? z[i + 1] : pz;
             const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
-            const bool acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
+            const bool acc = mc_move<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
                                                    toff_tab[j], attempt);
             if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
             if (kRecord && acc) atomicOr(dec_words + (attempt >> 5), 1u << (attempt & 31u));
@@ -774,7 +794,7 @@ molecule_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y
 // attempts of its own chain out of shared memory, and the warp writes the 32 chains back coalesced --
 // each position crosses HBM once per sweep, as in the fused kernel.  Dynamic shared memory:
 // warps_per_block * 3 * 32 N floats.
-template <int kMove, bool kIncr, bool kRecord>
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
 __global__ void __launch_bounds__(128)
 molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                        const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -813,7 +833,7 @@ molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__
                 const float xl = has_l ? sx[i - 1] : px, yl = has_l ? sy[i - 1] : py, zl = has_l ? sz[i - 1] : pz;
                 const float xr = has_r ? sx[i + 1] : px, yr = has_r ? sy[i + 1] : py, zr = has_r ? sz[i + 1] : pz;
                 const float mf = (float)((has_l ? 1 : 0) + (has_r ? 1 : 0));
-                const bool acc = mc_move<kMove, kIncr>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
+                const bool acc = mc_move<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, xl, yl, zl, xr, yr, zr, mf,
                                                        toff_tab[j], attempt);
                 if (acc) { sx[i] = px; sy[i] = py; sz[i] = pz; }
                 if (kRecord && acc) atomicOr(dec_words + (attempt >> 5), 1u << (attempt & 31u));
@@ -834,8 +854,9 @@ molecule_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__
 }
 
 // ------------------------------------------------------------------------------------------------
-// a3  occupation numbers from scratch (Eq. 4): counts[type][cell] += 1 per bead.
+// a3  occupation numbers from scratch (Eq. 4): one count per bead into the cell's record.
 // ------------------------------------------------------------------------------------------------
+template <bool kPack>
 __global__ void __launch_bounds__(256)
 histogram_kernel(const GridP g, const float* __restrict__ x, const float* __restrict__ y,
                  const float* __restrict__ z, const uint32_t* __restrict__ toff_tab, uint32_t N,
@@ -846,7 +867,9 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
     for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {   // 64-bit: n_beads may be 2^32 - 1
         const uint32_t j = (uint32_t)(i % N);
         const float xi = x[i], yi = y[i], zi = z[i];
-        atomicAdd(counts + cell_at(g, xi, yi, zi, toff_tab[j] + g.k_tot), 1u);
+        const uint32_t idx = cell_at<kPack>(g, xi, yi, zi, toff_tab[j] + g.k_rec);
+        if (kPack) atomicAdd(counts + (idx >> 1), 1u << ((idx & 1u) << 4));
+        else atomicAdd(counts + idx, 1u);
         // the supported coordinates of cell_raw(): |t n| < 2^22 per axis (a NaN fails the comparison too)
         const bool ok = fabsf(xi * g.inv_L[0] * g.nf[0]) < 4194304.0f && fabsf(yi * g.inv_L[1] * g.nf[1]) < 4194304.0f &&
                         fabsf(zi * g.inv_L[2] * g.nf[2]) < 4194304.0f;
@@ -862,7 +885,7 @@ histogram_kernel(const GridP g, const float* __restrict__ x, const float* __rest
 //     + ext_i(c) if an external field is set; +inf in forbidden cells, so that Eq. 15 makes every move
 //     into such a cell cost +inf and the Metropolis rule rejects it (R23)
 // ------------------------------------------------------------------------------------------------
-// omega of one cell from its occupation numbers n[0 .. nt)
+// omega of one cell from its occupation numbers n[0 .. nt); ext is [type][cell] (the caller's layout)
 template <int kTypes>
 __device__ __forceinline__ void field_of_cell(const FieldP& F, const uint32_t (&n)[kMaxTypes], uint32_t c,
                                               const float* __restrict__ ext, const uint8_t* __restrict__ forbidden,
@@ -897,59 +920,103 @@ __device__ __forceinline__ void field_of_cell(const FieldP& F, const uint32_t (&
     }
 }
 
-template <int kTypes>
+// Packed occupation numbers (kPack): has a 16-bit half overflowed?  The word of a cell is n_A + 65536 n_B
+// modulo 2^32 exactly, so as long as both numbers are below 65536 the halves are the numbers and the sum of
+// all halves is the number of beads counted; a number of 65536 or more lowers that sum (by 65535 per carry
+// into the upper half, by 65536 per carry out of the word) and nothing can raise it.  The field kernel
+// therefore adds up the halves it decodes anyway -- one atomic per block on *ticket_sum, block count in the
+// bits from 40 up, sum below -- and the block that draws the last ticket compares the sum with the number
+// of beads and sets the sticky flag *overflow (pinned host memory, written once if ever) if they differ.
+
+// One thread per cell.  counts and omega as planes [type][cell], or (kPack, two types) as records per cell
+// with packed counts.  kTypes = 0: any number of types (F.n_types).
+template <int kTypes, bool kPack>
 __global__ void __launch_bounds__(256)
 field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
-             const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
+             const float* __restrict__ ext, const uint8_t* __restrict__ forbidden,
+             unsigned long long* __restrict__ ticket_sum, uint32_t* __restrict__ overflow,
+             unsigned long long n_counted)
 {
+    static_assert(!kPack || kTypes == 2, "packed occupation numbers: two types");
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     pdl_trigger();
     pdl_wait();                                               // counts of the preceding move kernel
-    if (c >= F.cells) return;
-    const int nt = kTypes > 0 ? kTypes : F.n_types;
-    uint32_t n[kMaxTypes];
-    float w[kMaxTypes];
-#pragma unroll
-    for (int i = 0; i < kMaxTypes; ++i)
-        if (i < nt) n[i] = counts[(size_t)i * F.cells + c];
-    field_of_cell<kTypes>(F, n, c, ext, forbidden, w);
-#pragma unroll
-    for (int i = 0; i < kMaxTypes; ++i)
-        if (i < nt) omega[(size_t)i * F.cells + c] = w[i];
-}
-
-// The same with four consecutive cells per thread (128-bit loads and stores); needs cells % 4 == 0 so
-// that every type's plane starts 16-byte aligned.  kTypes = 1 or 2.
-template <int kTypes>
-__global__ void __launch_bounds__(256)
-field_kernel_v4(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
-                const float* __restrict__ ext, const uint8_t* __restrict__ forbidden)
-{
-    const uint32_t c = 4u * (blockIdx.x * blockDim.x + threadIdx.x);
-    pdl_trigger();
-    pdl_wait();                                               // counts of the preceding move kernel
-    if (c >= F.cells) return;
-    uint4 n4[kTypes];
-#pragma unroll
-    for (int i = 0; i < kTypes; ++i) n4[i] = *reinterpret_cast<const uint4*>(counts + (size_t)i * F.cells + c);
-    float4 w4[kTypes];
-#pragma unroll
-    for (int e = 0; e < 4; ++e) {
+    uint32_t total = 0;
+    if (c < F.cells) {
+        const int nt = kTypes > 0 ? kTypes : F.n_types;
         uint32_t n[kMaxTypes];
         float w[kMaxTypes];
+        if (kPack) {
+            const uint32_t v = counts[c];
+            n[0] = v & 0xFFFFu;
+            n[1] = v >> 16;
+            total = n[0] + n[1];
+        } else {
 #pragma unroll
-        for (int i = 0; i < kTypes; ++i) n[i] = e == 0 ? n4[i].x : e == 1 ? n4[i].y : e == 2 ? n4[i].z : n4[i].w;
-        field_of_cell<kTypes>(F, n, c + e, ext, forbidden, w);
+            for (int i = 0; i < kMaxTypes; ++i)
+                if (i < nt) n[i] = counts[(size_t)i * F.cells + c];
+        }
+        field_of_cell<kTypes>(F, n, c, ext, forbidden, w);
+        if (kPack) {
+            reinterpret_cast<float2*>(omega)[c] = make_float2(w[0], w[1]);
+        } else {
 #pragma unroll
-        for (int i = 0; i < kTypes; ++i) {
-            if (e == 0) w4[i].x = w[i];
-            if (e == 1) w4[i].y = w[i];
-            if (e == 2) w4[i].z = w[i];
-            if (e == 3) w4[i].w = w[i];
+            for (int i = 0; i < kMaxTypes; ++i)
+                if (i < nt) omega[(size_t)i * F.cells + c] = w[i];
         }
     }
-#pragma unroll
-    for (int i = 0; i < kTypes; ++i) *reinterpret_cast<float4*>(omega + (size_t)i * F.cells + c) = w4[i];
+    if (kPack) {
+        __shared__ uint32_t s_total;
+        if (threadIdx.x == 0) s_total = 0u;
+        __syncthreads();
+        total = __reduce_add_sync(0xFFFFFFFFu, total);
+        if ((threadIdx.x & 31u) == 0u && total) atomicAdd(&s_total, total);
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            const unsigned long long mine = (1ull << 40) | (unsigned long long)s_total;
+            const unsigned long long before = atomicAdd(ticket_sum, mine);
+            if ((before >> 40) == (unsigned long long)(gridDim.x - 1u)) {      // the last block of this launch
+                if (((before + mine) & ((1ull << 40) - 1ull)) != n_counted) *overflow = 1u;
+                *ticket_sum = 0ull;                                            // for the next launch
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Grid arrays between the device format (planes, or records per cell with packed occupation numbers) and
+// the caller's [type][cell] arrays of the C ABI.
+// ------------------------------------------------------------------------------------------------
+template <bool kPack>
+__global__ void __launch_bounds__(256)
+export_grid_kernel(const float* __restrict__ omega, const uint32_t* __restrict__ counts, uint32_t cells, uint32_t nt,
+                   float* __restrict__ omega_out, uint32_t* __restrict__ counts_out)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= (uint64_t)cells * nt) return;
+    const uint32_t t = (uint32_t)(i / cells), c = (uint32_t)(i - (uint64_t)t * cells);
+    if (omega_out) omega_out[i] = kPack ? omega[(size_t)c * nt + t] : omega[i];
+    if (counts_out) {
+        if (kPack) counts_out[i] = t ? counts[c] >> 16 : counts[c] & 0xFFFFu;
+        else counts_out[i] = counts[i];
+    }
+}
+
+// src: occupation numbers [type][cell] (e.g. summed over the ranks of a sharded system) -> internal layout
+template <bool kPack>
+__global__ void __launch_bounds__(256)
+import_counts_kernel(const uint32_t* __restrict__ src, uint32_t cells, uint32_t nt, uint32_t* __restrict__ dst,
+                     uint32_t* __restrict__ overflow)
+{
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= cells) return;
+    if (kPack) {
+        const uint32_t a = src[c], b = src[(size_t)cells + c];
+        if ((a | b) >> 16) *overflow = 1u;
+        dst[c] = a + (b << 16);
+    } else {
+        for (uint32_t t = 0; t < nt; ++t) dst[(size_t)t * cells + c] = src[(size_t)t * cells + c];
+    }
 }
 
 // ------------------------------------------------------------------------------------------------
