@@ -9,7 +9,14 @@ field update over every bead of the workload.  Default wo
 
 Multi-GPU: north_star runs the path on one GPU with no sharding and no collective ("replicas
 only"): --gpus N runs N independent replicas (different seeds), one process per GPU,
-value = total moves of all replicas / max-over-ranks time, scaling "weak".
+value = total moves of all replicas / max-over-ranks time, scaling "weak".  Started without
+torchrun (no WORLD_SIZE in the environment) with N > 1, bench.py starts its N ranks itself
+(python -m torch.distributed.run); the line's n_gpus is the number of ranks that ran.
+
+Numbers of the bench line: `value` = the K timed steps (one soma_step(K) call between two CUDA
+events; with the default K = 200 that is 20 ms at the burst clock), `sustained` = 5000 further
+sweeps in one stretch with the clocks sampled through NVML -- the board reaches its power cap
+after ~0.1 s, so `sustained` is the rate a production run sees and the one the documents lead with.
 
 --impl reference times the CPU oracle (oracle/soma_oracle.c, as it stands) on the host cores.
 """
@@ -35,7 +42,7 @@ METRIC = "attempted bead moves/s (full SCMF step)"
 UNIT = "moves/s"
 MOVE_BYTES_PER_BEAD = 24.0   # fused move kernel: read 12 B + write 12 B per bead per sweep
 FIELD_BYTES_PER_CELL = 16.0  # field kernel: read n_t counts + write n_t omegas (n_t = 2), DESIGN.md
-INSTR_PER_MOVE = 152.5       # SASS warp instructions per 32 local moves of the fused kernel (profiles/r01f_README.md)
+SCHEDULERS_PER_SM = 4         # warp schedulers per SM, one instruction per cycle each (B300_MICROARCH.md)
 
 
 def peaks():
@@ -49,24 +56,49 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks and throttle reasons during the timed region."""
+    """SM clock and throttle reasons during the timed region, sampled through NVML (nvidia-ml-py) every
+    millisecond from a thread of this process; nvidia-smi (~50 ms per call) as the fallback."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+    NAMES = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
 
-    def __init__(self, index: int):
-        self.index, self.samples, self.stop, self.t = index, [], threading.Event(), None
+    def __init__(self, index: int, period_s: float = 0.001):
+        self.index, self.period, self.samples, self.stop, self.t = index, period_s, [], threading.Event(), None
+        self.nvml, self.handle, self.max_mhz, self.source = None, None, None, "nvidia-smi"
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            # NVML enumerates the physical devices; honour CUDA_VISIBLE_DEVICES for a plain integer list
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+            ids = [int(v) for v in vis.split(",")] if vis and all(v.strip().isdigit() for v in vis.split(",")) else None
+            phys = ids[index] if ids and index < len(ids) else index
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
+            self.nvml, self.source = pynvml, "nvml"
+        except Exception:
+            self.nvml = None
+
+    def _once(self):
+        if self.nvml is not None:
+            n = self.nvml
+            mhz = float(n.nvmlDeviceGetClockInfo(self.handle, n.NVML_CLOCK_SM))
+            r = int(n.nvmlDeviceGetCurrentClocksEventReasons(self.handle))
+            bits = [n.nvmlClocksEventReasonHwSlowdown, n.nvmlClocksEventReasonHwThermalSlowdown,
+                    n.nvmlClocksEventReasonSwThermalSlowdown, n.nvmlClocksEventReasonSwPowerCap]
+            return [mhz, self.max_mhz] + [bool(r & b) for b in bits]
+        out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                              "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
+        f = [v.strip() for v in out.strip().split(",")]
+        return [float(f[0]), float(f[1])] + [v.lower().startswith("active") for v in f[2:6]]
 
     def _run(self):
         while not self.stop.is_set():
             try:
-                out = subprocess.run(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                      "-i", str(self.index)], capture_output=True, text=True, timeout=5).stdout
-                f = [v.strip() for v in out.strip().split(",")]
-                if len(f) >= 6:
-                    self.samples.append(f)
+                self.samples.append(self._once())
             except Exception:
-                pass
-            self.stop.wait(0.1)
+                if self.nvml is not None:      # NVML failed mid-run: fall back
+                    self.nvml, self.source = None, "nvidia-smi"
+            self.stop.wait(self.period if self.nvml is not None else 0.1)
 
     def __enter__(self):
         self.t = threading.Thread(target=self._run, daemon=True)
@@ -76,18 +108,73 @@ class ClockSampler:
     def __exit__(self, *a):
         self.stop.set()
         self.t.join(timeout=6)
+        if not self.samples:                   # a region shorter than one sample: take one now
+            try:
+                self.samples.append(self._once())
+            except Exception:
+                pass
 
     def summary(self):
         if not self.samples:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        mhz = sorted(float(s[0]) for s in self.samples)
-        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = [n for i, n in enumerate(names) if any(s[2 + i].lower().startswith("active") for s in self.samples)]
-        return {"sm_mhz": mhz[len(mhz) // 2], "sm_max_mhz": float(self.samples[0][1]), "reasons": reasons,
-                "samples": len(mhz)}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock query unavailable"]}
+        mhz = sorted(s[0] for s in self.samples)
+        reasons = [n for i, n in enumerate(self.NAMES) if any(s[2 + i] for s in self.samples)]
+        return {"sm_mhz": mhz[len(mhz) // 2], "sm_min_mhz": mhz[0], "sm_max_mhz": self.samples[0][1],
+                "reasons": reasons, "samples": len(mhz), "source": self.source}
 
 
-def oracle_rate(w, steps: int, warmup: int, budget_s: float = 20.0):
+def kernel_source_hash() -> str:
+    """Identifies the kernels a profile entry was measured on (profiles/traffic.json)."""
+    import hashlib
+    h = hashlib.sha256()
+    for f in sorted((ROOT / "paper_1711_03828_b200" / "csrc").glob("*.cu*")):
+        h.update(f.read_bytes())
+    return h.hexdigest()[:16]
+
+
+def profile_entry(name: str):
+    """dram bytes and warp instructions per launch of the move kernel from the committed ncu capture, or None
+    if there is none for this config or the kernels have changed since (a stale number is worse than none)."""
+    f = ROOT / "profiles" / "traffic.json"
+    try:
+        e = json.loads(f.read_text()).get(name)
+        if isinstance(e, dict) and e.get("kernel_hash") == kernel_source_hash():
+            return e
+    except Exception:
+        pass
+    return None
+
+
+def ingest_ncu_csv(csv_path: str, name: str):
+    """profiles/traffic.json entry from `ncu --csv --metrics dram__bytes_read.sum,dram__bytes_write.sum,
+    smsp__inst_executed.sum -k regex:fused_sweep ... python bench.py --config NAME ...` (the first launch listed)."""
+    import csv
+    vals = {}
+    with open(csv_path) as fh:
+        rows = [r for r in csv.reader(fh) if len(r) > 3]
+    hdr = next(r for r in rows if "Metric Name" in r)
+    i_name, i_unit, i_val, i_id = hdr.index("Metric Name"), hdr.index("Metric Unit"), hdr.index("Metric Value"), hdr.index("ID")
+    ids = set()
+    for r in rows[rows.index(hdr) + 1:]:               # every launch in the file: the move launches of ONE sweep
+        ids.add(r[i_id])
+        v = float(r[i_val].replace(",", ""))
+        unit = r[i_unit].lower()
+        v *= {"kbyte": 1e3, "mbyte": 1e6, "gbyte": 1e9}.get(unit, 1.0)
+        vals[r[i_name]] = vals.get(r[i_name], 0.0) + v
+    f = ROOT / "profiles" / "traffic.json"
+    d = json.loads(f.read_text()) if f.exists() else {}
+    d = {k: v for k, v in d.items() if isinstance(v, dict)}
+    d[name] = {"dram_bytes": int(vals["dram__bytes_read.sum"] + vals["dram__bytes_write.sum"]),
+               "inst_executed": int(vals["smsp__inst_executed.sum"]), "launches": len(ids),
+               "kernel_hash": kernel_source_hash(),
+               "source": f"ncu --metrics dram__bytes_read.sum,dram__bytes_write.sum,smsp__inst_executed.sum -k regex:"
+                         f"(fused_sweep|generic_move) -s <5 sweeps> -c <move launches of one sweep> python bench.py --config {name} --steps 5 --warmup 3 "
+                         f"--no-cpu-baseline --aged 0; python bench.py --ingest-ncu <csv> --config {name}"}
+    f.write_text(json.dumps(d, indent=1, sort_keys=True) + "\n")
+    print(json.dumps(d[name]))
+
+
+def oracle_rate(w, steps: int, warmup: int, budget_s: float = 20.0, one_thread_too: bool = False):
     """Time the oracle, as it stands, on the host cores: full SCMF cycles on a bounded sample."""
     sys.path.insert(0, str(ROOT / "tests"))
     import oracle
@@ -113,10 +200,27 @@ def oracle_rate(w, steps: int, warmup: int, budget_s: float = 20.0):
     t = time.perf_counter()
     s.step(x, y, z, c, om, warmup, steps)
     dt = time.perf_counter() - t
-    return {"value": sample.n_beads * steps / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{sample.n_chains} chains ({sample.n_beads} beads, {100 * sample.n_beads / w.n_beads:.1f}% of "
-                      f"{w.name}; same box, grid and chain architecture), {steps} full SCMF cycles after {warmup} "
-                      f"warm-up, OpenMP over chains"}, dt / steps * 1e3
+    out = {"value": sample.n_beads * steps / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+           "sample": f"{sample.n_chains} chains ({sample.n_beads} beads, {100 * sample.n_beads / w.n_beads:.1f}% of "
+                     f"{w.name}; same box, grid and chain architecture), {steps} full SCMF cycles after {warmup} "
+                     f"warm-up, OpenMP over chains"}
+    if one_thread_too:
+        # the oracle on one thread as well, on a sample a tenth of the budget long
+        n_all = oracle.num_threads()
+        small = w.scaled(min(1.0, 0.1 * budget_s / (per_bead * n_all * w.n_beads)), name=f"{w.name}-1thread")
+        s1 = oracle_system(small)
+        x, y, z = workloads.gaussian_walks(small)
+        c = s1.histogram(x, y, z)
+        om = s1.fields(c)
+        oracle.set_num_threads(1)
+        try:
+            t = time.perf_counter()
+            s1.step(x, y, z, c, om, 0, 1)
+            out["one_thread"] = {"value": small.n_beads / (time.perf_counter() - t), "unit": UNIT, "cores": 1,
+                                 "sample": f"{small.n_chains} chains ({small.n_beads} beads), 1 full SCMF cycle"}
+        finally:
+            oracle.set_num_threads(n_all)
+    return out, dt / steps * 1e3
 
 
 def max_over_ranks(value: float, dist, device) -> float:
@@ -183,25 +287,49 @@ def main():
                     help="N > 1: ONE system of N x the config's chains in a box N x as long (same density), molecules "
                          "distributed over the ranks, one all-reduce of the occupation numbers per sweep (SURVEY 8(e)); "
                          "default: N independent replicas")
+    ap.add_argument("--ingest-ncu", metavar="CSV",
+                    help="no run: write the profiles/traffic.json entry of --config from an ncu --csv metrics file")
     args = ap.parse_args()
+    if args.ingest_ncu:
+        ingest_ncu_csv(args.ingest_ncu, workloads.by_name(args.config).name)
+        return
     if args.warmup < 3 and args.impl == "ours":
         args.warmup = 3   # timing rule: W >= 3
+    if args.gpus < 1:
+        raise SystemExit("bench.py: --gpus must be >= 1")
+
+    if args.gpus > 1 and "WORLD_SIZE" not in os.environ:
+        # started the plain way: one process per GPU is this program's multi-GPU form, so start the ranks
+        import socket
+        with socket.socket() as sock:
+            sock.bind(("127.0.0.1", 0))
+            port = sock.getsockname()[1]
+        cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(args.gpus),
+               "--master-addr", "127.0.0.1", "--master-port", str(port), str(Path(__file__).resolve())] + sys.argv[1:]
+        raise SystemExit(subprocess.run(cmd).returncode)
 
     rank = int(os.environ.get("RANK", "0"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
+    if world != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but {world} rank(s) were started")
     w = workloads.by_name(args.config)
     config = {"workload": f"{w.name}: {w.note}", "chains": w.n_chains, "beads": w.n_beads, "grid": list(w.grid),
               "box": list(w.box), "chiN": w.chiN, "kappaN": w.kappaN, "A": w.A, "seed": w.seed, "move": w.move,
               "parallelism": "replicas only" if world > 1 else "single GPU",
-              "l2_policy": "inputs larger than L2 (positions 197 MB > 126 MB L2); no explicit flush"}
+              "timing": "W warm-up steps (the last five at most enqueued after the synchronisation, directly before the start "
+                        "event), K steps in one soma_step(K) call between two CUDA events, barrier + synchronize on both sides",
+              "l2_policy": (f"inputs larger than L2 (positions {12 * w.n_beads / 1e6:.0f} MB > 126 MB L2); no explicit flush"
+                            if 12 * w.n_beads > 126e6 else
+                            f"state fits in L2 (positions {12 * w.n_beads / 1e6:.1f} MB) and stays there from sweep to sweep, "
+                            "as in a production run of this system; no flush")}
 
     if args.impl == "reference":
         if rank != 0:
             return
         steps = min(args.steps, 3)
-        base, ms = oracle_rate(w, steps, min(args.warmup, 1))
-        line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": args.gpus,
+        base, ms = oracle_rate(w, steps, min(args.warmup, 1), one_thread_too=True)
+        line = {"impl": "reference", "metric": METRIC, "value": base["value"], "unit": UNIT, "n_gpus": world,
                 "steps": steps, "warmup": min(args.warmup, 1), "ms_per_step": ms, "higher_is_better": True,
                 "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
                 "cpu_baseline": base,
@@ -213,6 +341,8 @@ def main():
     import paper_1711_03828_b200 as P
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device; the product path has no CPU fallback")
+    if torch.cuda.device_count() < world:
+        raise SystemExit(f"bench.py: {world} ranks but only {torch.cuda.device_count()} CUDA device(s): one process per GPU")
     torch.cuda.set_device(local_rank)
     dist = None
     if world > 1:
@@ -261,14 +391,22 @@ def main():
     nb = sim.n_beads                           # beads this rank moves
 
     # ---- device-resident throughput ------------------------------------------------------------
-    sim.step(args.warmup)
+    # W warm-up steps, K timed steps between two CUDA events, barrier + synchronize on both sides.  The last (up to
+    # five) warm-up steps are enqueued after the first synchronisation, directly in front of the start event, so the
+    # timed region starts with the GPU busy (measured: after an idle period the first steps run slower, ~60 us in
+    # all, which a 20-step region of 2 ms would carry as +3 %); the events are in stream order, so exactly the K
+    # steps lie between them.
+    pre_roll = min(5, args.warmup)
+    sim.step(args.warmup - pre_roll)
     barrier()
     l0 = sim.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local_rank) as clk:
+        time.sleep(0.003)                      # the sampling thread is running before the region starts
+        sim.step(pre_roll)
+        l0 = sim.launch_count()
         e0.record()
-        for _ in range(args.steps):
-            sim.step(1)
+        sim.step(args.steps)                   # one soma_step(K) call: K x (move launch, field launch), no Python in between
         e1.record()
         barrier()
     ms_total = e0.elapsed_time(e1)
@@ -297,24 +435,24 @@ def main():
                                          "field": kms[P.K_FIELD] / max(1e-12, sum(kms))},
                 "full_step_frac": (MOVE_BYTES_PER_BEAD * nb + FIELD_BYTES_PER_CELL * w.n_cells) * args.steps
                                   / (ms_total * 1e-3) / 1e9 / peak}
-    # dram bytes per launch of the move kernel from the committed ncu --set full capture (profiles/r01f_README.md)
-    traffic_file = ROOT / "profiles" / "traffic.json"
-    if traffic_file.exists():
-        try:
-            roofline["traffic"] = json.loads(traffic_file.read_text()).get(w.name)
-        except Exception:
-            pass
-    # second roof: warp-instruction issue.  152.5 SASS warp instructions per 32 moves
-    # (ncu smsp__inst_executed.sum / launch), 4 schedulers per SM, one instruction per cycle each.
+    roofline["timing_note"] = ("ms_per_launch: CUDA events around every launch inside the library (SOMA_OPT_TIMING), which "
+                               "serialises the launches -- without the programmatic-dependent-launch overlap of the timed "
+                               "region, so it can exceed ms_per_step; full_step_frac is from the timed region itself")
+    # dram bytes and warp instructions per launch of the move kernel from the committed ncu capture of these very
+    # kernels (profiles/traffic.json; an entry measured on other kernel sources is ignored)
+    prof = profile_entry(w.name)
+    roofline["traffic"] = prof["dram_bytes"] if prof else None
+    # second roof: warp-instruction issue, one instruction per cycle and scheduler
     clocks_now = clk.summary()
-    if clocks_now.get("sm_mhz") and w.move == "local":
-        inst_per_launch = INSTR_PER_MOVE * nb / 32.0
-        peak_ips = 148 * 4 * clocks_now["sm_mhz"] * 1e6
-        roofline["issue"] = {"bound": "alu", "achieved": inst_per_launch / (move_ms * 1e-3) / 1e12,
+    if clocks_now.get("sm_mhz") and prof:
+        n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        peak_ips = n_sm * SCHEDULERS_PER_SM * clocks_now["sm_mhz"] * 1e6
+        roofline["issue"] = {"bound": "alu", "achieved": prof["inst_executed"] / (move_ms * 1e-3) / 1e12,
                              "peak": peak_ips / 1e12, "unit": "T warp-instr/s",
-                             "frac": inst_per_launch / (move_ms * 1e-3) / peak_ips,
-                             "instr_per_move": INSTR_PER_MOVE,
-                             "note": "issue slots of 148 SMs x 4 schedulers at the sampled SM clock; DESIGN.md 6.1"}
+                             "frac": prof["inst_executed"] / (move_ms * 1e-3) / peak_ips,
+                             "instr_per_32_moves": prof["inst_executed"] / (nb / 32.0),
+                             "note": f"issue slots of {n_sm} SMs x {SCHEDULERS_PER_SM} schedulers at the sampled SM clock; "
+                                     "instructions per launch from profiles/traffic.json; DESIGN.md 6.1"}
 
     # ---- end to end through the C ABI with host buffers ----------------------------------------
     n_e2e = max(3, min(args.steps, 20))
@@ -366,7 +504,7 @@ def main():
                              "acceptance": (acc2 - acc1) / max(1, att2 - att1),
                              "mean_abs_phiA_minus_phiB": float(np.mean(np.abs(cnt[0] - cnt[-1]) / tot)) if w.n_types > 1 else None}
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
-        line["cpu_baseline"], _ = oracle_rate(w, 2, 1)
+        line["cpu_baseline"], _ = oracle_rate(w, 2, 1, one_thread_too=True)
     sim.destroy()
     if dist is not None:
         dist.destroy_process_group()

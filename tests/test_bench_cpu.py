@@ -62,3 +62,38 @@ def test_reference_arm_under_torchrun_prints_one_line_from_rank_0():
     line = json.loads(lines[0])
     assert line["impl"] == "reference" and line["n_gpus"] == 2 and line["value"] > 0
     assert line["cpu_baseline"]["kind"] == "oracle" and line["e2e"]["h2d_bytes_per_step"] == 0
+
+
+def test_gpus_2_without_torchrun_starts_two_ranks():
+    """`python bench.py --gpus 2 ...` as the driver runs it (no torchrun, no WORLD_SIZE): bench.py starts its
+    two ranks itself; the reference arm's rank 0 prints the one line, which says two ranks ran."""
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK", "MASTER_ADDR", "MASTER_PORT")}
+    cmd = [sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--gpus", "2", "--steps", "1", "--warmup", "0",
+           "--config", "C1"]
+    res = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT, env=env)
+    assert res.returncode == 0, res.stderr[-2000:]
+    lines = [l for l in res.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    line = json.loads(lines[0])
+    assert line["impl"] == "reference" and line["n_gpus"] == 2
+    assert line["cpu_baseline"]["one_thread"]["cores"] == 1 and line["cpu_baseline"]["one_thread"]["value"] > 0
+
+
+def test_rank_count_must_match_gpus():
+    env = dict(os.environ, WORLD_SIZE="1", RANK="0", LOCAL_RANK="0")
+    res = subprocess.run([sys.executable, str(ROOT / "bench.py"), "--impl", "reference", "--gpus", "2", "--config", "C1"],
+                         capture_output=True, text=True, timeout=120, cwd=ROOT, env=env)
+    assert res.returncode != 0 and "rank(s) were started" in res.stderr
+
+
+def test_stale_profile_entries_are_ignored(tmp_path, monkeypatch):
+    import bench
+    monkeypatch.setattr(bench, "ROOT", tmp_path)
+    (tmp_path / "profiles").mkdir()
+    (tmp_path / "paper_1711_03828_b200" / "csrc").mkdir(parents=True)
+    (tmp_path / "paper_1711_03828_b200" / "csrc" / "k.cuh").write_text("v1")
+    (tmp_path / "profiles" / "traffic.json").write_text(json.dumps(
+        {"C3": {"dram_bytes": 5, "inst_executed": 7, "kernel_hash": bench.kernel_source_hash()}, "C1": 12345}))
+    assert bench.profile_entry("C3")["dram_bytes"] == 5 and bench.profile_entry("C1") is None
+    (tmp_path / "paper_1711_03828_b200" / "csrc" / "k.cuh").write_text("v2")      # the kernels changed
+    assert bench.profile_entry("C3") is None
