@@ -115,8 +115,10 @@ def lockstep(w, n_sweeps, xyz0=None, kernel=P.KERNEL_AUTO, density=P.DENSITY_INC
         att, acc_g, done = sim.stats()
         assert done == sweep + 1 and att == nb * (sweep + 1)
     att, acc_total, _ = sim.stats()
-    assert 0 < acc_total <= att
+    assert 0 < acc_total <= att or (w.move == "smc" and w.smc_step >= 0.05)     # the literal C5 step accepts ~nothing
     sim.destroy()
+    print(f"[lockstep] {w.name}: {n_sweeps} sweeps x {nb} moves, {total_flips} decisions differ "
+          f"({total_flips / (n_sweeps * nb):.2e} per move), acceptance {acc_total / att:.3f}")
     return total_flips
 
 
@@ -471,10 +473,21 @@ def test_walls_hold_and_external_fields_can_be_removed():
 # ---------------------------------------------------------------------------------------------
 # full-size configs in the launch configuration bench.py times
 # ---------------------------------------------------------------------------------------------
-def test_c3_headline_full_size():
+# Decisions can differ only where u (23 bits) lands within the error of exp(-dE) on either side (expf: < 1 ulp,
+# ex2.approx after an fp32 multiply by log2 e: ~2 ulp) and the move is not decided by dE <= 0 anyway.  Observed on
+# a B200: 1 of 1.6e8 moves at C3 (10 sweeps), 4 of 2.7e8 at C4, none in 5.8e7 Smart-MC moves at C5, i.e. ~1e-8 per
+# move.  The tests below hold the observed number to twenty times that -- fifty times tighter than north_star's
+# 1e-5 -- so that a regression of the acceptance arithmetic shows long before the agreement bound is reached.
+FLIPS_PER_MOVE = 2e-7
+
+
+def test_c3_headline_full_size_10_sweeps():
+    """C3 in lock-step for 10 sweeps, from the disordered Gaussian-walk start."""
     w = workloads.c3()
-    flips = lockstep(w, 2)
-    assert flips <= 2 * w.n_beads * 1e-5
+    log = []
+    flips = lockstep(w, 10, flip_log=log)
+    assert max(log) <= FLIPS_PER_MOVE * w.n_beads, log
+    assert flips <= 10 * FLIPS_PER_MOVE * w.n_beads
 
 
 def test_c3_long_run_counts_stay_exact_through_resorts_and_dependent_launches():
@@ -498,6 +511,13 @@ def test_c3_long_run_counts_stay_exact_through_resorts_and_dependent_launches():
     assert order(cnt) > 3.0 * order(cnt0)                 # lamellar domains have formed
     assert np.isfinite(pos).all()
     sim.destroy()
+    # The ordered melt is the state the paper's runs spend their time in: large |omega_A - omega_B|
+    # across the interfaces, so dE_nb decides many more moves than in the disordered start.  Two lock-step sweeps
+    # from it: decisions, accepted positions, occupation numbers and fields, as everywhere else.
+    assert float(np.abs(om[0] - om[1]).mean()) > 3.0 * float(np.abs(om0[0] - om0[1]).mean())
+    log = []
+    lockstep(w, 2, xyz0=pos, flip_log=log)
+    assert max(log) <= FLIPS_PER_MOVE * w.n_beads, log
 
 
 def test_c4_large_melt_full_size():
@@ -511,12 +531,17 @@ def test_c4_large_melt_full_size():
     xyz0 = seedling.positions()
     seedling.destroy()
     flips = lockstep(w, 1, xyz0=xyz0)
-    assert flips <= w.n_beads * 1e-5
+    assert flips <= FLIPS_PER_MOVE * w.n_beads
 
 
-def test_c5_blend_full_size_smart_mc():
-    w = workloads.c5(smc_step=0.05 / 63)
-    lockstep(w, 1)
+@pytest.mark.parametrize("smc_step", [0.05, 0.05 / 63], ids=["literal-0.05", "0.05-b0^2"])
+def test_c5_blend_full_size_smart_mc(smc_step):
+    """BASELINE config C5 at full size with the Smart-MC step as BASELINE.json states it (0.05 R_e^2: the drift
+    a_s k_0 b_0 is ten bond lengths, nothing is accepted) and with 0.05 b_0^2, which has a useful acceptance
+    (R19).  Smart-MC decisions go through logf / sincosf on both sides, hence the wider flip bound."""
+    w = workloads.c5(smc_step=smc_step)
+    flips = lockstep(w, 1)
+    assert flips <= 5 * FLIPS_PER_MOVE * w.n_beads
 
 
 # ---------------------------------------------------------------------------------------------

@@ -521,6 +521,32 @@ def test_smc_gaussians_are_standard_normal():
     assert 0 <= us.min() and us.max() < 1 and abs(us.mean() - 0.5) < 4 / math.sqrt(12 * 2000)
 
 
+def test_smc_proposal_is_the_documented_map_of_the_philox_words():
+    """Reading R13, value by value: the Gaussians are Box-Muller on the words of the Philox call of kind 2,
+    sub 0 -- u1 = 2 - U23(w0) in (0, 1], u2 = U23(w1) - 1 -> g_x = r cos(2 pi u2), g_y = r sin(2 pi u2),
+    r = sqrt(-2 ln u1); w2, w3 -> g_z (the cosine branch) -- and the acceptance number is U23(word 0 of the call
+    sub 1) - 1.  Recomputed here from the (P1-pinned) Philox words with Python's float64 math; the moments test
+    above cannot tell cos from sin or w0 from w2, this one can."""
+    seed = 0x0123456789ABCDEF
+    s = _free_beads(1, seed=seed, smc_step=0.01)
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    two_pi32 = float(np.float32(6.283185307179586))
+    for bead, sweep in [(0, 0), (1, 0), (0, 1), (77, 3), (123456, 2**32 + 5), (2**32 - 1, 2**40 + 9)] + \
+                       [(b, 11) for b in range(200)]:
+        w = oracle.philox4x32_10((bead, sweep & 0xFFFFFFFF, sweep >> 32, (2 << 8) | 0), key)
+        v = oracle.philox4x32_10((bead, sweep & 0xFFFFFFFF, sweep >> 32, (2 << 8) | 1), key)
+        u1a, u2a = 1.0 - (w[0] >> 9) * 2.0**-23, (w[1] >> 9) * 2.0**-23
+        u1b, u2b = 1.0 - (w[2] >> 9) * 2.0**-23, (w[3] >> 9) * 2.0**-23
+        ra, rb = math.sqrt(-2.0 * math.log(u1a)), math.sqrt(-2.0 * math.log(u1b))
+        ta, tb = float(np.float32(two_pi32 * u2a)), float(np.float32(two_pi32 * u2b))   # the angle is an fp32 product
+        want = np.array([ra * math.cos(ta), ra * math.sin(ta), rb * math.cos(tb)])
+        g, u = s.smc_proposal(bead, sweep)
+        # fp32 logf, sqrtf, sinf / cosf and one product: a few ulp of the radius
+        tol = 6.0 * np.spacing(np.float32(max(ra, rb, 1e-3)))
+        assert np.all(np.abs(g.astype(np.float64) - want) <= tol), (bead, sweep, g, want)
+        assert u == (v[0] >> 9) * 2.0**-23
+
+
 def test_smc_energy_and_proposal_ratio_match_brute_force():
     specs = [(2, np.array([0, 0, 1, 1], np.uint8)), (1, np.array([1], np.uint8))]
     box, grid = (1.5, 1.0, 2.0), (3, 2, 4)
@@ -600,6 +626,39 @@ def test_init_positions_statistics():
     # reproducible from (seed, bead index) alone
     x2, _, _ = s.init_positions()
     assert np.array_equal(x, x2)
+
+
+def test_init_positions_are_the_documented_map_of_the_philox_words():
+    """Reading R14, value by value: kind-0 Philox words of every bead (counter = (bead, 0, 0, 0)); first bead
+    L_a w_a 2^-32; each further bead adds sigma times Box-Muller Gaussians in double -- r = sqrt(-2 ln((w + 1)
+    2^-32)) of w0 / w2, angle 2 pi w 2^-32 of w1 / w3, x: r_a cos, y: r_a sin, z: r_b cos -- running sum in double,
+    one rounding to fp32.  Recomputed with Python's math from the (P1-pinned) words; two architectures, so the
+    bead index runs on across them."""
+    seed = 987654321987
+    box = (3.0, 5.0, 7.0)
+    specs = [(3, np.zeros(5, np.uint8)), (2, np.zeros(9, np.uint8))]
+    s = OracleSystem(specs=specs, N_ref=8, n_types=1, box=box, grid=(2, 2, 2), seed=seed)
+    x, y, z = s.init_positions()
+    key = (seed & 0xFFFFFFFF, seed >> 32)
+    sigma = 1.0 / math.sqrt(3.0 * 7.0)
+    g = 0
+    for n, t in specs:
+        for _ in range(n):
+            p = [0.0, 0.0, 0.0]
+            for j in range(len(t)):
+                w = oracle.philox4x32_10((g, 0, 0, 0), key)
+                if j == 0:
+                    p = [box[a] * (w[a] / 2.0**32) for a in range(3)]
+                else:
+                    ra = math.sqrt(-2.0 * math.log((w[0] + 1.0) / 2.0**32))
+                    rb = math.sqrt(-2.0 * math.log((w[2] + 1.0) / 2.0**32))
+                    ta, tb = 2.0 * math.pi * (w[1] / 2.0**32), 2.0 * math.pi * (w[3] / 2.0**32)
+                    p = [p[0] + sigma * (ra * math.cos(ta)), p[1] + sigma * (ra * math.sin(ta)), p[2] + sigma * (rb * math.cos(tb))]
+                for got, want in zip((x[g], y[g], z[g]), p):
+                    # same double-precision formula; libm and Python may differ in the last bit of log / cos
+                    assert abs(float(got) - want) <= np.spacing(np.float32(abs(want))) , (g, got, want)
+                g += 1
+    assert g == s.n_beads
 
 
 # ----------------------------------------------------------------------------------------------
