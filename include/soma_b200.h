@@ -69,8 +69,7 @@ enum {
                                    /* 1: clear + full histogram kernel after every sweep                      */
     SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */
     SOMA_OPT_SWEEP_COUNTER = 8,    /* set the sweep counter (the "time step" word of the Philox counter)      */
-    SOMA_OPT_GRAPH = 9,            /* reserved, accepted and ignored: the sweep counter is a kernel argument,  */
-                                   /* so every sweep is launched afresh (launch overlap: SOMA_OPT_PDL)          */
+                                   /* (key 9 is not used: see DESIGN.md 6.7 for the one-launch variants measured) */
     SOMA_OPT_BLOCKS_PER_SM = 10,   /* tuning: grid of the fused kernel = SMs x this many blocks; 0 = resident max */
     SOMA_OPT_LAYOUT = 11,          /* 0: chains stay in the caller's order in device memory; 1 (default): the  */
                                    /* library keeps them in Hilbert order of their centres of mass.  Storage   */

@@ -145,7 +145,7 @@ struct soma_ctx {
     int device = 0, n_sm = 0;
 
     // options
-    int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0, use_graph = 1;
+    int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0;
     uint32_t* n_outside = nullptr;   // device counter: beads whose coordinates are outside the supported domain
     int pdl = 1;             // programmatic dependent launch of the fused and field kernels (SOMA_OPT_PDL)
     int blocks_per_sm = 0;   // grid of the fused kernel = n_sm * blocks_per_sm; 0 = as many as are resident
@@ -1200,9 +1200,6 @@ int soma_set_option(soma_ctx* c, int key, double value)
         case SOMA_OPT_SWEEP_COUNTER:
             if (value < 0) return fail(SOMA_EINVAL, "SOMA_OPT_SWEEP_COUNTER: must be >= 0");
             c->sweep = (uint64_t)value;
-            return SOMA_OK;
-        case SOMA_OPT_GRAPH:
-            c->use_graph = iv != 0;
             return SOMA_OK;
         case SOMA_OPT_PDL:
             if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_PDL: 0 or 1");
