@@ -249,6 +249,24 @@ struct Draw {            // what one move takes from Philox
     float u;             // acceptance uniform in [0, 1)
 };
 
+// -2 ln(u1) for the Box-Muller radius, u1 = 2 - U23(w) = 1 - delta in (0, 1], delta = k 2^-23 exact.
+// lg2.approx has an absolute error of 2^-22, which is a relative one only while |ln u1| is not small; near
+// u1 = 1 (delta < 1/16) the series -ln(1 - delta) = delta + delta^2/2 + ... + delta^5/5 takes over (truncation
+// 1.6e-7 relative).  Relative error of the result <= 2.6e-6 (at the switch), of the radius half that: a Gaussian
+// is off by < 5e-7.  13 instructions instead of the ~28 of logf with its special cases.
+__device__ __forceinline__ float neg2ln_u1(uint32_t w)
+{
+    const float delta = u23(w) - 1.0f, u1 = 1.0f - delta;              // both exact
+    float l2;
+    asm("lg2.approx.ftz.f32 %0, %1;" : "=f"(l2) : "f"(u1));
+    const float far = l2 * -1.3862943611198906f;                        // -2 ln 2 lg2(u1)
+    float p = fmaf(delta, 0.4f, 0.5f);
+    p = fmaf(delta, p, 0.6666666666666666f);
+    p = fmaf(delta, p, 1.0f);
+    p = fmaf(delta, p, 2.0f);
+    return delta < 0.0625f ? delta * p : far;
+}
+
 // kMove 1: d uniform in (-A,A)^3, 2^23 equidistant values per axis.
 // kMove 2: g ~ N(0,1)^3 by Box-Muller on the words of call sub=0, u from call sub=1.
 template <int kMove>
@@ -271,10 +289,9 @@ __device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
         // approximations are best (absolute error 2^-21.4): sin(t) = -sin(t - pi), cos(t) = -cos(t - pi), and
         // t - pi = 2 pi (U23 - 1.5) with an exact subtraction.  A Gaussian is then off by <= ~2e-6, a
         // displacement by sqrt(2 a_s) times that: inside the parity tolerance on positions (R17).
-        // The radius keeps the accurate logf: lg2.approx has an absolute, not a relative, error near 1, where
-        // the radius sqrt(-2 ln u) is small -- measured: 1 move in 10^4 off by more than 1e-6 R_e.
-        const float ra = sqrt_approx(-2.0f * logf(2.0f - u23(w[0])));   // sqrt.approx: <= 2 ulp
-        const float rb = sqrt_approx(-2.0f * logf(2.0f - u23(w[2])));
+        // Radius: see neg2ln_u1().
+        const float ra = sqrt_approx(neg2ln_u1(w[0]));                  // sqrt.approx: <= 2 ulp
+        const float rb = sqrt_approx(neg2ln_u1(w[2]));
         const float two_pi = 6.283185307179586f;
         const float ta = two_pi * (u23(w[1]) - 1.5f), tb = two_pi * (u23(w[3]) - 1.5f);
         const float sa = -__sinf(ta), ca = -__cosf(ta), cb = -__cosf(tb);
@@ -336,31 +353,26 @@ __device__ __forceinline__ bool metropolis(float dE, float u)
     return u < ex2_approx(dE * -1.4426950408889634f);
 }
 
-// Smart-MC proposal from the bonded force F = -k_0 s (refs [28,29]):
-//   d = a_s F + sqrt(2 a_s) g,   ln T(r->r') - ln T(r'->r) = (|d + a_s F'|^2 - |d - a_s F|^2) / (4 a_s),
-//   F' = F - k_0 m d
-__device__ __forceinline__ void smc_proposal(const MoveP& P, float mf, float sx, float sy, float sz,
-                                             const Draw& g, float& dx, float& dy, float& dz, float& log_ratio)
+// Smart-MC proposal from the bonded force F = -k_0 s (refs [28,29]; R13):
+//   d = a_s F + sqrt(2 a_s) g,   accept iff u < exp(-(dE_b + dE_nb + L)),
+//   L = ln T(r->r') - ln T(r'->r) = (|d + a_s F'|^2 - |d - a_s F|^2) / (4 a_s),   F' = F - k_0 m d.
+// With e_r - e_f = 2 a_s F - a_s k_0 m d and e_r + e_f = (2 - a_s k_0 m) d for e_f = d - a_s F, e_r = d + a_s F',
+//   L = (2 - a_s k_0 m)/4 (2 F.d - k_0 m |d|^2) = -(1 - a_s k_0 m / 2) dE_b,      dE_b = k_0/2 (2 d.s + m |d|^2),
+// so the exponent is dE_nb + (a_s k_0 m / 2) dE_b: one fused multiply-add instead of the two squared norms and
+// their difference (which also loses digits to cancellation; the closed form is the more accurate of the two).
+__device__ __forceinline__ void smc_proposal(const MoveP& P, float sx, float sy, float sz, const Draw& g,
+                                             float& dx, float& dy, float& dz)
 {
     const float Fx = -P.k0 * sx, Fy = -P.k0 * sy, Fz = -P.k0 * sz;
     dx = fmaf(P.a_s, Fx, P.noise * g.a);
     dy = fmaf(P.a_s, Fy, P.noise * g.b);
     dz = fmaf(P.a_s, Fz, P.noise * g.c);
-    const float km = P.k0 * mf;
-    float fwd = 0.0f, rev = 0.0f;
-    {
-        const float ef = dx - P.a_s * Fx, er = dx + P.a_s * (Fx - km * dx);
-        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-    }
-    {
-        const float ef = dy - P.a_s * Fy, er = dy + P.a_s * (Fy - km * dy);
-        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-    }
-    {
-        const float ef = dz - P.a_s * Fz, er = dz + P.a_s * (Fz - km * dz);
-        fwd = fmaf(ef, ef, fwd); rev = fmaf(er, er, rev);
-    }
-    log_ratio = __fdividef(rev - fwd, P.four_as);   // rcp.approx + multiply: within 2 ulp of the quotient
+}
+
+// exponent of the Smart-MC acceptance: dE_nb + (a_s k_0 m / 2) dE_b;  half_as_k0 = a_s k_0 / 2
+__device__ __forceinline__ float smc_exponent(float half_as_k0, float mf, float e_b, float e_nb)
+{
+    return fmaf(half_as_k0 * mf, e_b, e_nb);
 }
 
 // The occupation numbers follow an accepted move (+1 new cell, -1 old cell): integer arithmetic, so
@@ -394,15 +406,14 @@ __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restric
                                           float sx, float sy, float sz, float mf, uint32_t toff, uint32_t gid)
 {
     const Draw q = draw_move<kMove>(P, gid);
-    float dx = q.a, dy = q.b, dz = q.c, log_ratio = 0.0f;
-    if (kMove == 2) smc_proposal(P, mf, sx, sy, sz, q, dx, dy, dz, log_ratio);
+    float dx = q.a, dy = q.b, dz = q.c;
+    if (kMove == 2) smc_proposal(P, sx, sy, sz, q, dx, dy, dz);
     const float x2 = x + dx, y2 = y + dy, z2 = z + dz;   // r' = fl32(r + d)
     const uint32_t i_old = cell_at<kPack>(P.g, x, y, z, toff + P.g.k_rec);
     const uint32_t i_new = cell_at<kPack>(P.g, x2, y2, z2, toff + P.g.k_rec);
     const float e_nb = field_delta(omega, i_old, i_new);
     const float e_b = bonded_delta(kMove == 1 ? P.hk : 0.5f * P.k0, mf, dx, dy, dz, sx, sy, sz);
-    float dE = e_b + e_nb;
-    if (kMove == 2) dE = dE + log_ratio;
+    const float dE = kMove == 2 ? smc_exponent(P.four_as * 0.125f * P.k0, mf, e_b, e_nb) : e_b + e_nb;
     const bool acc = metropolis(dE, q.u);
     x = acc ? x2 : x;
     y = acc ? y2 : y;
@@ -606,36 +617,37 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             // Smart-MC: the proposal needs the bonded force, i.e. the neighbours as they are now
             float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
             xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
-            float sx0, sy0, sz0, sx2, sy2, sz2, dx0, dy0, dz0, dx2, dy2, dz2, lr0, lr2;
+            const float hak = P.four_as * 0.125f * P.k0;          // a_s k_0 / 2
+            float sx0, sy0, sz0, sx2, sy2, sz2, dx0, dy0, dz0, dx2, dy2, dz2;
             bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx0, sy0, sz0);
             bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx2, sy2, sz2);
-            smc_proposal(P, mf0, sx0, sy0, sz0, q0, dx0, dy0, dz0, lr0);
-            smc_proposal(P, 2.0f, sx2, sy2, sz2, q2, dx2, dy2, dz2, lr2);
+            smc_proposal(P, sx0, sy0, sz0, q0, dx0, dy0, dz0);
+            smc_proposal(P, sx2, sy2, sz2, q2, dx2, dy2, dz2);
             const float x0n = X.x + dx0, y0n = Y.x + dy0, z0n = Z.x + dz0;
             const float x2n = X.z + dx2, y2n = Y.z + dy2, z2n = Z.z + dz2;
             const uint32_t o0 = cell_at<kPack>(P.g, X.x, Y.x, Z.x, tk.x), n0 = cell_at<kPack>(P.g, x0n, y0n, z0n, tk.x);
             const uint32_t o2 = cell_at<kPack>(P.g, X.z, Y.z, Z.z, tk.z), n2 = cell_at<kPack>(P.g, x2n, y2n, z2n, tk.z);
             const float e0 = field_delta(omega, o0, n0), e2 = field_delta(omega, o2, n2);
-            a0 = metropolis((bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0) + e0) + lr0, q0.u);
-            a2 = metropolis((bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2) + e2) + lr2, q2.u);
+            a0 = metropolis(smc_exponent(hak, mf0, bonded_delta(half_k0, mf0, dx0, dy0, dz0, sx0, sy0, sz0), e0), q0.u);
+            a2 = metropolis(smc_exponent(hak, 2.0f, bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2), e2), q2.u);
             X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
             X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
             if (kIncr) { count_follow<kPack>(counts, a0, o0, n0); count_follow<kPack>(counts, a2, o2, n2); }
 
             float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
             xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
-            float sx1, sy1, sz1, sx3, sy3, sz3, dx1, dy1, dz1, dx3, dy3, dz3, lr1, lr3;
+            float sx1, sy1, sz1, sx3, sy3, sz3, dx1, dy1, dz1, dx3, dy3, dz3;
             bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx1, sy1, sz1);
             bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx3, sy3, sz3);
-            smc_proposal(P, 2.0f, sx1, sy1, sz1, q1, dx1, dy1, dz1, lr1);
-            smc_proposal(P, mf3, sx3, sy3, sz3, q3, dx3, dy3, dz3, lr3);
+            smc_proposal(P, sx1, sy1, sz1, q1, dx1, dy1, dz1);
+            smc_proposal(P, sx3, sy3, sz3, q3, dx3, dy3, dz3);
             const float x1n = X.y + dx1, y1n = Y.y + dy1, z1n = Z.y + dz1;
             const float x3n = X.w + dx3, y3n = Y.w + dy3, z3n = Z.w + dz3;
             const uint32_t o1 = cell_at<kPack>(P.g, X.y, Y.y, Z.y, tk.y), n1 = cell_at<kPack>(P.g, x1n, y1n, z1n, tk.y);
             const uint32_t o3 = cell_at<kPack>(P.g, X.w, Y.w, Z.w, tk.w), n3 = cell_at<kPack>(P.g, x3n, y3n, z3n, tk.w);
             const float e1 = field_delta(omega, o1, n1), e3 = field_delta(omega, o3, n3);
-            a1 = metropolis((bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1) + e1) + lr1, q1.u);
-            a3 = metropolis((bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3) + e3) + lr3, q3.u);
+            a1 = metropolis(smc_exponent(hak, 2.0f, bonded_delta(half_k0, 2.0f, dx1, dy1, dz1, sx1, sy1, sz1), e1), q1.u);
+            a3 = metropolis(smc_exponent(hak, mf3, bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3), e3), q3.u);
             X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
             X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
             if (kIncr) { count_follow<kPack>(counts, a1, o1, n1); count_follow<kPack>(counts, a3, o3, n3); }
