@@ -154,13 +154,20 @@ int soma_init(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_
  *                    ceil(global_n_beads / 32) words)
  *   global_n_beads   beads of the whole system (< 2^32): rho_0 of Eq. 12 is global_n_beads / volume
  * All other arguments as for soma_init, describing this rank's molecules only (host_xyz0: their
- * positions, or NULL to draw them as the undivided system would).  The context comes back with its
- * local occupation numbers (soma_fields(ctx, NULL, counts, ..)) but WITHOUT omega: sum the counts of all
- * ranks (integers: any order, any collective) and call soma_shard_fields(.., advance = 0).  Then, per
- * MC step: soma_shard_moves; sum the counts of all ranks; soma_shard_fields(.., advance = 1).  The
+ * positions, or NULL to draw them as the undivided system would).
+ *
+ * The exchange array.  A shard keeps two arrays of occupation numbers in the grid format of the context
+ * (SOMA_OPT_COUNT_BITS): its copy of the WHOLE system's numbers (what soma_fields returns), and the exchange
+ * array, into which its own kernels count -- the histogram of its molecules after soma_init_shard /
+ * soma_set_positions, the +1 / -1 of its accepted moves after soma_shard_moves.  The caller sums the exchange
+ * arrays of all ranks element-wise as uint32 (modulo 2^32; in place, any collective: NCCL all-reduce on the
+ * device address soma_shard_exchange returns) and calls soma_shard_fields, whose kernel adds the sum to the
+ * whole system's numbers, clears the exchange array for the next sweep and computes omega.  So per MC step:
+ *     soma_shard_moves;  all-reduce (sum) of the exchange array;  soma_shard_fields(ctx, 1)
+ * and once after soma_init_shard (or after every rank's soma_set_positions): all-reduce; soma_shard_fields(ctx, 0).
+ * No copy and no conversion lies between the move kernel, the collective and the field kernel.  The
  * positions, occupation numbers and fields equal those of the undivided system bit for bit.  soma_step
- * returns SOMA_ESTATE on such a context; soma_set_positions / soma_set_chi / soma_set_external / the
- * Hamiltonian option leave omega to the next soma_shard_fields. */
+ * returns SOMA_ESTATE on such a context. */
 int soma_init_shard(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_ref, int n_types,
                     const float *box, const int *grid, float chiN, float kappaN, float A, uint64_t seed,
                     const float *host_xyz0, void *cuda_stream, const uint64_t *spec_first_bead,
@@ -171,12 +178,20 @@ int soma_init_shard(soma_ctx **out, const soma_chain_spec *chains, int n_specs, 
  * combinations whose part-of-a-system mode has no oracle: SOMA_OPT_SCHEME 1 and bond-list architectures. */
 int soma_shard_moves(soma_ctx *ctx);
 
-/* a4: omega from the occupation numbers of the whole system (uint32 [n_types][cells], host or device;
- * a device array is read in place by the field kernel and must stay untouched until the stream has
- * passed it).  advance != 0 closes the sweep begun by soma_shard_moves (sweep counter + 1, and omega is
- * only recomputed when SOMA_OPT_FIELD_INTERVAL says so); advance = 0: stage 1 after soma_init_shard or
- * soma_set_positions. */
-int soma_shard_fields(soma_ctx *ctx, const uint32_t *global_counts, int src_is_device, int advance);
+/* Device address and length (uint32 words) of the exchange array: n_types * cells words for planes, cells
+ * words for the packed records.  Valid for the life of the context unless SOMA_OPT_COUNT_BITS is changed. */
+int soma_shard_exchange(soma_ctx *ctx, void **dev_words, uint64_t *n_words);
+
+/* The same array through host memory, for callers that sum on the host: to_host != 0 copies it out,
+ * to_host = 0 copies host_words in.  Synchronises. */
+int soma_shard_exchange_copy(soma_ctx *ctx, uint32_t *host_words, int to_host);
+
+/* a4: folds the (summed) exchange array into the whole system's occupation numbers, clears it, and computes
+ * omega.  advance != 0 closes the sweep begun by soma_shard_moves (sweep counter + 1; omega is only
+ * recomputed when SOMA_OPT_FIELD_INTERVAL says so, the numbers are folded in any case); advance = 0: stage 1
+ * after soma_init_shard or soma_set_positions.  Launched with programmatic dependent launch (SOMA_OPT_PDL)
+ * behind whatever precedes it in the stream. */
+int soma_shard_fields(soma_ctx *ctx, int advance);
 
 /* n_sweeps SCMF cycles: (a1, a2 | a5), a3, a4 each.  Asynchronous on the context's stream.
  * The sweep counter advances by n_sweeps. */

@@ -29,7 +29,8 @@ SYMBOLS = (
     "soma_init", "soma_step", "soma_fields", "soma_positions", "soma_set_positions", "soma_set_chi",
     "soma_set_external", "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
-    "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields",
+    "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields", "soma_shard_exchange",
+    "soma_shard_exchange_copy",
 )
 
 
@@ -59,7 +60,9 @@ def load() -> C.CDLL:
                             C.POINTER(C.c_int), C.c_float, C.c_float, C.c_float, u64, vp, vp]
     L.soma_init_shard.argtypes = L.soma_init.argtypes + [C.POINTER(u64), u64]
     L.soma_shard_moves.argtypes = [vp]
-    L.soma_shard_fields.argtypes = [vp, vp, i32, i32]
+    L.soma_shard_fields.argtypes = [vp, i32]
+    L.soma_shard_exchange.argtypes = [vp, C.POINTER(vp), C.POINTER(u64)]
+    L.soma_shard_exchange_copy.argtypes = [vp, vp, i32]
     L.soma_step.argtypes = [vp, i32]
     L.soma_fields.argtypes = [vp, vp, vp, i32]
     L.soma_positions.argtypes = [vp, vp, i32]
@@ -153,9 +156,34 @@ class Soma:
     def shard_moves(self) -> None:
         _check(self._L.soma_shard_moves(self._h))
 
-    def shard_fields(self, global_counts, advance: bool = True) -> None:
-        p, dev = _ptr(global_counts)
-        _check(self._L.soma_shard_fields(self._h, C.c_void_p(p), int(dev), int(bool(advance))))
+    def shard_fields(self, advance: bool = True) -> None:
+        _check(self._L.soma_shard_fields(self._h, int(bool(advance))))
+
+    def shard_exchange(self) -> Tuple[int, int]:
+        """(device address, uint32 words) of the exchange array of a shard."""
+        p, n = C.c_void_p(), C.c_uint64()
+        _check(self._L.soma_shard_exchange(self._h, C.byref(p), C.byref(n)))
+        return int(p.value), int(n.value)
+
+    def shard_exchange_tensor(self):
+        """The exchange array as a torch int32 tensor on the device (no copy): what the all-reduce runs on."""
+        import torch
+        addr, n = self.shard_exchange()
+
+        class _View:                                   # the CUDA array interface is all torch needs to wrap the memory
+            __cuda_array_interface__ = {"shape": (n,), "typestr": "<i4", "data": (addr, False), "version": 3, "strides": None}
+
+        return torch.as_tensor(_View(), device="cuda")
+
+    def shard_exchange_get(self) -> np.ndarray:
+        out = np.empty(self.shard_exchange()[1], np.uint32)
+        _check(self._L.soma_shard_exchange_copy(self._h, C.c_void_p(out.ctypes.data), 1))
+        return out
+
+    def shard_exchange_put(self, words: np.ndarray) -> None:
+        words = np.ascontiguousarray(words, np.uint32)
+        assert words.size == self.shard_exchange()[1]
+        _check(self._L.soma_shard_exchange_copy(self._h, C.c_void_p(words.ctypes.data), 0))
 
     def fields(self, omega=None, counts=None):
         """Copy omega (and counts) out. With no arguments returns new host numpy arrays."""

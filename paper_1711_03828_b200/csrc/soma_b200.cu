@@ -104,7 +104,8 @@ struct soma_ctx {
     uint64_t n_beads = 0, n_pad = 0, cells = 0;
     uint64_t n_beads_global = 0;     // beads of the whole system (= n_beads unless this context is a shard)
     int sharded = 0;                 // created by soma_init_shard: soma_shard_moves / soma_shard_fields instead of soma_step
-    uint32_t* counts_global = nullptr;   // staging for soma_shard_fields from a host array (allocated on first use)
+    uint32_t* exchange = nullptr;    // shard: what this rank's move kernels count into; summed over the ranks by the caller,
+                                     // folded into counts (the whole system's numbers) by the field kernel, which clears it
 
     float *x = nullptr, *y = nullptr, *z = nullptr;
     uint32_t* counts = nullptr;      // planes [n_types][cells], or packed [cells] (pack)
@@ -271,6 +272,9 @@ struct Timed {
 };
 
 // ---- launches -----------------------------------------------------------------------------------
+// where the move and histogram kernels count: a shard counts its contribution into the exchange array
+inline uint32_t* count_target(const soma_ctx* c) { return c->sharded ? c->exchange : c->counts; }
+
 bool spec_uses_fused(const soma_ctx* c, const Spec& s)
 {
     if (c->kernel_choice == 1) return false;
@@ -329,7 +333,7 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     }
     Timed t(c, SOMA_K_MOVE, 1);
     CU(launch_pdl(c->pdl != 0, kernel, (unsigned)blocks, (unsigned)threads, order_smem, c->stream,
-                  P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N - 1u,
+                  P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, s.N - 1u,
                   s.n_tiles, (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots));
     return SOMA_OK;
 }
@@ -348,7 +352,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const int threads = 256;
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::arch_move_kernel<kMove, kIncr, kRecord, kPack><<<(unsigned)((n_items + threads - 1) / threads), threads, 0, c->stream>>>(
-                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, nbr_off, nbr,
+                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, nbr_off, nbr,
                     members + s.set_off[i_set], s.N, set_size, n_items, (uint32_t)s.gid0, c->orig + s.chain_off,
                     c->decisions, c->acc_slots);
             }
@@ -376,7 +380,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const uint64_t blocks = std::min<uint64_t>((uint64_t)c->n_sm * per_sm, (n_groups + warps - 1) / warps);
                 Timed t(c, SOMA_K_MOVE, 1);
                 kernel<<<(unsigned)blocks, warps * 32, smem, c->stream>>>(
-                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N,
+                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, s.N,
                     s.n_chains, (uint32_t)s.gid0, c->orig + s.chain_off, c->decisions, c->acc_slots);
                 CU(cudaGetLastError());
                 continue;
@@ -385,7 +389,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
             const unsigned blocks = (unsigned)((s.n_chains + threads - 1) / threads);
             Timed t(c, SOMA_K_MOVE, 1);
             soma::molecule_move_kernel<kMove, kIncr, kRecord, kPack><<<blocks, threads, 0, c->stream>>>(
-                P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, c->counts, c->toff + s.toff_off, s.N,
+                P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, s.N,
                 s.n_chains, (uint32_t)s.gid0, c->orig + s.chain_off, c->decisions, c->acc_slots);
             CU(cudaGetLastError());
             continue;
@@ -408,7 +412,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const uint64_t blocks = (n_items + threads - 1) / threads;
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::generic_move_kernel<kMove, kIncr, kRecord, kPack><<<(unsigned)blocks, threads, 0, c->stream>>>(
-                    P, x + done, y + done, z + done, c->omega, c->counts, toff, s.N, half, parity,
+                    P, x + done, y + done, z + done, c->omega, count_target(c), toff, s.N, half, parity,
                     (uint32_t)c->set_order, n_items,
                     (uint32_t)s.gid0, c->orig + s.chain_off + done / s.N, c->decisions, c->acc_slots);
             }
@@ -469,6 +473,7 @@ size_t counts_bytes(const soma_ctx* c)
 int launch_histogram(soma_ctx* c, bool check_domain_too)
 {
     CU(cudaMemsetAsync(c->counts, 0, counts_bytes(c), c->stream));
+    if (c->sharded) CU(cudaMemsetAsync(c->exchange, 0, counts_bytes(c), c->stream));   // counts = 0 + sum of the ranks' histograms
     const soma::GridP g = c->gridp();
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
@@ -479,18 +484,17 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
         Timed t(c, SOMA_K_DENSITY, 1);
         auto kernel = c->pack ? soma::histogram_kernel<true> : soma::histogram_kernel<false>;
         kernel<<<(unsigned)blocks, threads, 0, c->stream>>>(
-            g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, c->counts,
+            g, c->x + s.off, c->y + s.off, c->z + s.off, c->toff + s.toff_off, s.N, (uint32_t)s.n_beads, count_target(c),
             check_domain_too ? c->n_outside : nullptr);
         CU(cudaGetLastError());
     }
     return SOMA_OK;
 }
 
-// counts_src: occupation numbers in the internal layout (default: this context's own), n_counted: the beads
-// they count (the packed format's overflow check, soma::CountCheck)
-int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr, uint64_t n_counted = 0)
+// a4.  A shard folds the exchange array (summed over the ranks by now) into its copy of the whole system's
+// occupation numbers on the way.
+int launch_fields(soma_ctx* c, bool fold_exchange = false)
 {
-    if (!counts_src) { counts_src = c->counts; n_counted = c->n_beads; }
     const soma::FieldP F = c->fieldp();
 #ifndef SOMA_FIELD_THREADS
 #define SOMA_FIELD_THREADS 256
@@ -501,23 +505,24 @@ int launch_fields(soma_ctx* c, const uint32_t* counts_src = nullptr, uint64_t n_
     const bool pdl = c->pdl != 0;
     // One cell per thread: with programmatic dependent launch the many small blocks slip in behind the
     // draining move blocks.
-    const unsigned long long n = n_counted;
+    const unsigned long long n = c->n_beads_global;        // the beads counts holds (the packed format's overflow check)
+    uint32_t* ex = fold_exchange ? c->exchange : nullptr;
     if (c->pack) {
-        CU(launch_pdl(pdl, soma::field_kernel<2, true>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n));
+        CU(launch_pdl(pdl, soma::field_kernel<2, true>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex));
         return SOMA_OK;
     }
     switch (c->n_types) {
-        case 1: CU(launch_pdl(pdl, soma::field_kernel<1, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
-        case 2: CU(launch_pdl(pdl, soma::field_kernel<2, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
-        default: CU(launch_pdl(pdl, soma::field_kernel<0, false>, blocks, threads, 0, c->stream, F, counts_src, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n)); break;
+        case 1: CU(launch_pdl(pdl, soma::field_kernel<1, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
+        case 2: CU(launch_pdl(pdl, soma::field_kernel<2, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
+        default: CU(launch_pdl(pdl, soma::field_kernel<0, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
     }
     return SOMA_OK;
 }
 
-// omega after a parameter change; a shard has to wait for the next soma_shard_fields (it needs every rank's counts)
+// omega after a parameter change (a shard holds the whole system's occupation numbers too)
 int refresh_fields(soma_ctx* c)
 {
-    return c->sharded ? (int)SOMA_OK : launch_fields(c);
+    return launch_fields(c);
 }
 
 // After new positions came in (soma_init, soma_set_positions): did the histogram see a coordinate outside
@@ -546,9 +551,7 @@ int stage1_once(soma_ctx* c)
     CU(cudaMemsetAsync(c->n_outside, 0, sizeof(uint32_t), c->stream));
     int rc = launch_histogram(c, true);
     if (rc) return rc;
-    // a shard's omega needs every rank's counts (soma_shard_fields); the launch here is the overflow check
-    // of its own packed counts (the field it writes is replaced before the first move)
-    if (c->sharded && !c->pack) return SOMA_OK;
+    if (c->sharded) return SOMA_OK;   // omega needs every rank's contribution: soma_shard_fields
     return launch_fields(c);
 }
 
@@ -668,7 +671,7 @@ void soma_destroy(soma_ctx* c)
     cudaStreamSynchronize(c->stream);
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
-    cudaFree(c->counts_global);
+    cudaFree(c->exchange);
     cudaFree(c->n_outside);
     cudaFree(c->ticket_sum);
     cudaFree(c->grid_stage);
@@ -872,6 +875,7 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     CUI(cudaMalloc(&c->y, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->z, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->counts, sizeof(uint32_t) * cells * n_types));
+    if (c->sharded) CUI(cudaMalloc(&c->exchange, sizeof(uint32_t) * cells * n_types));
     CUI(cudaMalloc(&c->omega, sizeof(float) * cells * n_types));
     CUI(cudaMalloc(&c->toff, sizeof(uint32_t) * toff_host.size()));
     if (!arch_host.empty()) {
@@ -1023,30 +1027,41 @@ int soma_shard_moves(soma_ctx* c)
     return SOMA_OK;
 }
 
-int soma_shard_fields(soma_ctx* c, const uint32_t* global_counts, int src_is_device, int advance)
+int soma_shard_exchange(soma_ctx* c, void** dev_words, uint64_t* n_words)
 {
-    if (!c || !global_counts) return fail(SOMA_EINVAL, "soma_shard_fields: NULL argument");
+    if (!c || !dev_words || !n_words) return fail(SOMA_EINVAL, "soma_shard_exchange: NULL argument");
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_exchange: the context was not created by soma_init_shard");
+    *dev_words = c->exchange;
+    *n_words = counts_bytes(c) / sizeof(uint32_t);
+    return SOMA_OK;
+}
+
+int soma_shard_exchange_copy(soma_ctx* c, uint32_t* host_words, int to_host)
+{
+    if (!c || !host_words) return fail(SOMA_EINVAL, "soma_shard_exchange_copy: NULL argument");
+    DeviceGuard on_device(c->device);
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_exchange_copy: the context was not created by soma_init_shard");
+    if (to_host) CU(cudaMemcpyAsync(host_words, c->exchange, counts_bytes(c), cudaMemcpyDeviceToHost, c->stream));
+    else CU(cudaMemcpyAsync(c->exchange, host_words, counts_bytes(c), cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    return SOMA_OK;
+}
+
+int soma_shard_fields(soma_ctx* c, int advance)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_shard_fields: ctx is NULL");
     DeviceGuard on_device(c->device);
     if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_fields: the context was not created by soma_init_shard");
-    // counts_global: 2 x [n_types][cells] words, the caller's array (if it is host memory) and its internal layout
-    const size_t n = (size_t)c->cells * c->n_types;
-    if (!c->counts_global) CU(cudaMalloc(&c->counts_global, 2 * sizeof(uint32_t) * n));
-    const uint32_t* src = global_counts;
-    if (!src_is_device) {
-        CU(cudaMemcpyAsync(c->counts_global + n, global_counts, sizeof(uint32_t) * n, cudaMemcpyHostToDevice, c->stream));
-        src = c->counts_global + n;
-    }
     if (!advance || c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
-        const unsigned blocks = (unsigned)((c->cells + 255) / 256);
-        c->launches += 1;
-        if (c->pack) soma::import_counts_kernel<true><<<blocks, 256, 0, c->stream>>>(src, (uint32_t)c->cells, (uint32_t)c->n_types, c->counts_global, c->overflow_dev);
-        else soma::import_counts_kernel<false><<<blocks, 256, 0, c->stream>>>(src, (uint32_t)c->cells, (uint32_t)c->n_types, c->counts_global, c->overflow_dev);
-        CU(cudaGetLastError());
-        int rc = launch_fields(c, c->counts_global, c->n_beads_global);   // a4 from the occupation numbers of the whole system
+        int rc = launch_fields(c, true);                   // a4 from the occupation numbers of the whole system
         if (rc) return rc;
+    } else {                                               // the counts stay current; omega is not due
+        const uint64_t n = counts_bytes(c) / sizeof(uint32_t);
+        c->launches += 1;
+        soma::fold_exchange_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->counts, c->exchange, n);
+        CU(cudaGetLastError());
     }
     if (advance) c->sweep += 1;
-    if (!src_is_device) CU(cudaStreamSynchronize(c->stream));   // the caller may reuse its buffer
     return SOMA_OK;
 }
 

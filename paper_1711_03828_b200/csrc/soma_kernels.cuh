@@ -942,12 +942,16 @@ __device__ __forceinline__ void field_of_cell(const FieldP& F, const uint32_t (&
 
 // One thread per cell.  counts and omega as planes [type][cell], or (kPack, two types) as records per cell
 // with packed counts.  kTypes = 0: any number of types (F.n_types).
+//   exchange   NULL, or (a part of a system spread over several GPUs) the array the move
+//              kernels of this rank counted into, summed over all ranks by the caller: the change of the whole
+//              system's occupation numbers since the last call, in the format of counts.  It is added to counts
+//              and cleared for the next sweep.  Sums of words are exact modulo 2^32, packed or not.
 template <int kTypes, bool kPack>
 __global__ void __launch_bounds__(256)
-field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restrict__ omega,
+field_kernel(const FieldP F, uint32_t* __restrict__ counts, float* __restrict__ omega,
              const float* __restrict__ ext, const uint8_t* __restrict__ forbidden,
              unsigned long long* __restrict__ ticket_sum, uint32_t* __restrict__ overflow,
-             unsigned long long n_counted)
+             unsigned long long n_counted, uint32_t* __restrict__ exchange)
 {
     static_assert(!kPack || kTypes == 2, "packed occupation numbers: two types");
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -959,14 +963,27 @@ field_kernel(const FieldP F, const uint32_t* __restrict__ counts, float* __restr
         uint32_t n[kMaxTypes];
         float w[kMaxTypes];
         if (kPack) {
-            const uint32_t v = counts[c];
+            uint32_t v = counts[c];
+            if (exchange) {
+                v += exchange[c];
+                counts[c] = v;
+                exchange[c] = 0u;
+            }
             n[0] = v & 0xFFFFu;
             n[1] = v >> 16;
             total = n[0] + n[1];
         } else {
 #pragma unroll
-            for (int i = 0; i < kMaxTypes; ++i)
-                if (i < nt) n[i] = counts[(size_t)i * F.cells + c];
+            for (int i = 0; i < kMaxTypes; ++i) {
+                if (i >= nt) continue;
+                const size_t at = (size_t)i * F.cells + c;
+                n[i] = counts[at];
+                if (exchange) {
+                    n[i] += exchange[at];
+                    counts[at] = n[i];
+                    exchange[at] = 0u;
+                }
+            }
         }
         field_of_cell<kTypes>(F, n, c, ext, forbidden, w);
         if (kPack) {
@@ -1065,6 +1082,16 @@ init_walk_kernel(float* __restrict__ x, float* __restrict__ y, float* __restrict
         }
         x[i] = (float)px; y[i] = (float)py; z[i] = (float)pz;
     }
+}
+
+// counts += exchange, exchange = 0: a sweep of a shard after which omega is not refreshed (SOMA_OPT_FIELD_INTERVAL)
+__global__ void __launch_bounds__(256)
+fold_exchange_kernel(uint32_t* __restrict__ counts, uint32_t* __restrict__ exchange, uint64_t n_words)
+{
+    const uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_words) return;
+    counts[i] += exchange[i];
+    exchange[i] = 0u;
 }
 
 }  // namespace soma

@@ -3,10 +3,11 @@
 The paper's parallelisation: "molecules are distributed among the MPI ranks", every rank keeps the
 whole grid, and after every MC step the densities of all ranks are summed (one all-reduce of the integer
 occupation numbers); every rank then computes omega redundantly.  Here a rank is a
-process with one B200, the all-reduce is ``torch.distributed.all_reduce`` (NCCL over NVLink on GPUs) on
-a device tensor the library writes its local occupation numbers into and reads the summed ones from --
-the only exchange step of the path.  Everything else is the single-GPU library: ``soma_init_shard``,
-``soma_shard_moves``, ``soma_shard_fields`` (include/soma_b200.h).
+process with one B200, the all-reduce is ``torch.distributed.all_reduce`` (NCCL over NVLink on GPUs) run
+in place on the library's exchange array -- the array this rank's move kernel counts into and the field
+kernel reads the sum from (no copy, no conversion in between) -- the only exchange step of the path.
+Everything else is the single-GPU library: ``soma_init_shard``, ``soma_shard_moves``,
+``soma_shard_exchange``, ``soma_shard_fields`` (include/soma_b200.h).
 
 Because the Philox counter of a bead is its index in the whole system and integer sums commute, the
 trajectory does not depend on the number of ranks: positions, occupation numbers and fields equal
@@ -71,15 +72,15 @@ class ShardedSoma:
             self.sim.set_option(B.OPT_SMC_STEP, w.smc_step)
             self.sim.set_option(B.OPT_MOVE, B.MOVE_SMC)
         self.n_beads_global = n_global
-        # the exchange buffer: local occupation numbers in, summed ones out (uint32 bits in an int32 tensor)
-        self.counts = torch.empty((w.n_types, self.sim.n_cells), dtype=torch.int32, device="cuda")
+        self.n_types = w.n_types
+        # the library's exchange array as a tensor (uint32 bits in int32: sums are exact modulo 2^32)
+        self.exchange = self.sim.shard_exchange_tensor()
         self._exchange(advance=False)
 
     def _exchange(self, advance: bool) -> None:
-        self.sim.fields(counts=self.counts)                       # a3: this rank's n_i(c)
         if self.dist is not None and self.world > 1:
-            self.dist.all_reduce(self.counts)                     # the only collective of the path (sum)
-        self.sim.shard_fields(self.counts, advance=advance)       # a4 from the whole system's n_i(c)
+            self.dist.all_reduce(self.exchange)                   # the only collective of the path (sum), in place
+        self.sim.shard_fields(advance=advance)                    # a4 from the whole system's n_i(c)
 
     def step(self, n_sweeps: int = 1) -> None:
         for _ in range(int(n_sweeps)):
@@ -92,8 +93,7 @@ class ShardedSoma:
 
     def fields(self):
         """(omega, occupation numbers of the whole system), host arrays."""
-        omega, _ = self.sim.fields(omega=np.empty((self.counts.shape[0], self.sim.n_cells), np.float32))
-        return omega, self.counts.cpu().numpy().view(np.uint32)
+        return self.sim.fields()
 
     def sync(self) -> None:
         self.sim.sync()

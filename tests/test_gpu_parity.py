@@ -611,8 +611,8 @@ def test_programmatic_dependent_launch_changes_no_result(w):
 # ---------------------------------------------------------------------------------------------
 # a system spread over several GPUs: soma_init_shard / soma_shard_moves / soma_shard_fields
 # ---------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("move,set_order", [("local", 0), ("local", 1), ("smc", 0)])
-def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move, set_order):
+@pytest.mark.parametrize("move,set_order,count_bits", [("local", 0, 0), ("local", 1, 0), ("smc", 0, 0), ("local", 0, 16)])
+def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move, set_order, count_bits):
     """Three shard contexts stepped one after the other on this GPU (no rank waits for another), their
     occupation numbers added on the host in place of the all-reduce: positions, counts, omega and decisions
     equal the undivided context bit for bit; the first sweep is also checked against the oracle's parts."""
@@ -635,23 +635,28 @@ def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move,
             sim.set_option(P.OPT_MOVE, P.MOVE_SMC)
         sim.set_option(P.OPT_RECORD_DECISIONS, 1)
         sim.set_option(P.OPT_SET_ORDER, set_order)
+        sim.set_option(P.OPT_COUNT_BITS, count_bits)      # packed words sum over the ranks like any others
         with pytest.raises(P.SomaError):
             sim.step(1)                                   # a shard has no soma_step
         shards.append((sim, slices, oracle_system(w, specs=[(n, t) for n, t in local], spec_first_bead=first,
                                                   global_n_beads=n_global, set_order=set_order)))
 
     def exchange(advance):
-        total = sum(sim.fields(counts=np.empty((w.n_types, w.n_cells), np.uint32))[1].astype(np.int64)
-                    for sim, _, _ in shards).astype(np.uint32)
+        # in place of the all-reduce: the ranks' exchange arrays added modulo 2^32 on the host
+        total = np.zeros(shards[0][0].shard_exchange()[1], np.uint32)
         for sim, _, _ in shards:
-            sim.shard_fields(total, advance=advance)
-        return total
+            total = total + sim.shard_exchange_get()
+        for sim, _, _ in shards:
+            sim.shard_exchange_put(total)
+            sim.shard_fields(advance=advance)
+        return shards[0][0].fields()[1]                   # the whole system's occupation numbers, as every shard holds them
 
     total = exchange(False)
     om_w, cnt_w = whole.fields()
     assert np.array_equal(total, cnt_w)
     for sim, _, _ in shards:
-        assert np.array_equal(sim.fields(omega=np.empty_like(om_w))[0], om_w)
+        om_s, cnt_s = sim.fields()
+        assert np.array_equal(om_s, om_w) and np.array_equal(cnt_s, cnt_w)
     mk = oracle.MOVE_SMC if move == "smc" else oracle.MOVE_LOCAL
     for sweep in range(4):
         if sweep == 0:                                    # the oracle's parts, from the same positions and omega
