@@ -320,13 +320,13 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     int blocks = c->n_sm * per_sm;
     const int max_useful = (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
     if (blocks > max_useful) blocks = max_useful;
-    // random set order: one byte per chain of the longest tile range a block can get; more (not all
-    // resident) blocks if that does not fit into shared memory
+    // random set order: four bytes per chain of the longest tile range a block can get (the chains grouped by
+    // their order bit); more (not all resident) blocks if that does not fit into shared memory
     size_t order_smem = 0;
     if (kOrder) {
         const size_t chains_per_tile = soma::kTile / s.N;
         for (int waves = 1;; ++waves) {
-            order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile;
+            order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile * 4 + 16;
             if (order_smem <= kOrderSmemMax) break;
             blocks = c->n_sm * per_sm * (waves + 1);
         }

@@ -454,7 +454,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 //   gid0        global index of the architecture's first bead
 //   orig        [n_chains] the caller's chain index of the chain in each slot (Philox counter, bitmap)
 //   dec_words   decision bitmap (whole system), or unused
-// kOrder: dynamic shared memory = one byte per chain of the block's tile range (the host keeps the ranges
+// kOrder: dynamic shared memory = four bytes per chain of the block's tile range (the host keeps the ranges
 // short enough); the block draws the order bit of all its chains before it waits for its predecessor.
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack>
@@ -488,33 +488,57 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     __shared__ uint32_t s_next[2];
     const uint32_t zero = n_mask >> 8;                        // n_mask = N - 1 <= 127
     if (threadIdx.x == 0) s_next[0] = t_begin + 2u * kWarps;
-    extern __shared__ uint8_t s_order[];                      // kOrder: order bit of the chains of this block's tiles
+    // kOrder: the chains of this block's tile range, regrouped (entry = index of the chain's first bead in this
+    // architecture's arrays, bit 0 = odd set first)
+    extern __shared__ __align__(16) uint32_t s_perm[];
     const uint32_t slot_begin = (t_begin * kTile) >> log2N;
+    const uint32_t n_slots = ((t_end - t_begin) * kTile) >> log2N;
+    const uint32_t cpt_shift = 7u - log2N, ci = (4u * lane) >> log2N;   // chains per tile = 128 / N; this lane's chain in its tile
     if (kOrder) {
         // "Generate random permutation of the sets" (Code 2) for every chain this block will move:
-        // needs nothing of the predecessor kernel (orig[] only changes in a re-sort), so it runs before the wait
-        const uint32_t n_slots = ((t_end - t_begin) * kTile) >> log2N;
-        for (uint32_t s = threadIdx.x; s < n_slots; s += kFusedThreads)
-            s_order[s] = (uint8_t)first_set_bit(gid0 + (orig[slot_begin + s] << log2N), P.sweep_lo, P.sweep_hi,
-                                                P.rk[0][0], P.rk[0][1]);
+        // needs nothing of the predecessor kernel (orig[] only changes in a re-sort), so it runs before the wait.
+        // The lanes of a warp hold different chains, and a warp whose chains all start with the same set does
+        // four evaluations per lane like the fixed order, a mixed one six (three phases); so the chains are
+        // regrouped by their bit within groups of 32 consecutive chains -- tiles are made of 128 / N consecutive
+        // entries of the list -- and (N = 32) at most one tile in eight is mixed, while a tile's chains stay
+        // neighbours in the storage order.  A stable partition per group: a warp per group, a lane per chain.
+        for (uint32_t lo0 = wib * 32u; lo0 < n_slots; lo0 += 8u * kWarps * 32u) {
+            uint32_t first[8];                                // eight groups' loads in flight
+#pragma unroll
+            for (uint32_t k = 0; k < 8u; ++k) {
+                const uint32_t s = lo0 + k * kWarps * 32u + lane;
+                first[k] = s < n_slots ? orig[slot_begin + s] : 0u;
+            }
+#pragma unroll
+            for (uint32_t k = 0; k < 8u; ++k) {
+                const uint32_t lo = lo0 + k * kWarps * 32u, s = lo + lane;
+                if (lo >= n_slots) break;
+                const uint32_t b = s < n_slots ? first_set_bit(gid0 + (first[k] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
+                const uint32_t in = __ballot_sync(kFull, s < n_slots), ones = __ballot_sync(kFull, b != 0u);
+                const uint32_t below = (1u << lane) - 1u;
+                const uint32_t n_zero = __popc(in & ~ones);
+                const uint32_t pos = b ? n_zero + __popc(ones & below) : __popc(in & ~ones & below);
+                if (s < n_slots) s_perm[lo + pos] = ((slot_begin + s) << log2N) | b;   // N >= 4: the low bits are free
+            }
+        }
     }
     pdl_wait();                                               // omega of the preceding field kernel
     __syncthreads();
     uint32_t tile = t_begin + wib, tile_n = tile + kWarps;
     float4 X, Y, Z;
     uint32_t C = 0u;                                          // the caller's index of this lane's chain
+    uint32_t E = 0u;                                          // kOrder: this lane's entry of the list
     if (tile < t_end) {
-        const uint32_t i0 = tile * kTile + 4u * lane;
+        if (kOrder) E = s_perm[((tile - t_begin) << cpt_shift) + ci];
+        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * kTile + 4u * lane;
         X = ld_stream(x + i0);
         Y = ld_stream(y + i0);
         Z = ld_stream(z + i0);
         C = orig[i0 >> log2N];
     }
     while (tile < t_end) {
-        const uint32_t i0 = tile * kTile + 4u * lane;
+        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * kTile + 4u * lane;
         const uint32_t gid = gid0 + (C << log2N) + j0;
-        uint32_t order_bit = 0u;
-        if (kOrder) order_bit = s_order[(i0 >> log2N) - slot_begin];
         // the tile after the next one.  The counter is addressed through `warp & zero` (zero: a kernel argument
         // bit that is never set): with a provably uniform address ptxas wraps the atomic of this single lane
         // into its warp-aggregation sequence (vote, popc, leader election: a dozen instructions per tile)
@@ -522,7 +546,9 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         if (lane == 0) tile_nn = atomicAdd(s_next + (wib & zero), 1u);
 
         // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
-        const uint32_t i0n = min(tile_n, t_end - 1u) * kTile + 4u * lane;
+        uint32_t En = 0u;
+        if (kOrder) En = s_perm[((min(tile_n, t_end - 1u) - t_begin) << cpt_shift) + ci];
+        const uint32_t i0n = kOrder ? (En & ~1u) + j0 : min(tile_n, t_end - 1u) * kTile + 4u * lane;
         const float4 Xn = ld_stream(x + i0n);
         const float4 Yn = ld_stream(y + i0n);
         const float4 Zn = ld_stream(z + i0n);
@@ -572,37 +598,46 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
                 // PAPER.md:302): the chain's bit says which set moves first, and the lanes of a warp hold
                 // different chains.  Three phases: the odd monomers of the chains that start with their odd set,
                 // the even monomers of every chain, the odd monomers of the chains that start with their even
-                // set.  A chain takes part in the two phases that are its own order; every slot is evaluated
-                // where it can move (six evaluations per lane instead of four).
-                const bool odd_first = order_bit != 0u;
+                // set.  A chain takes part in the two phases that are its own order.  A phase no chain of the warp
+                // takes part in is skipped: the block has grouped its chains by their bit, so all but one of its
+                // tiles run two phases -- four evaluations per lane, as in the fixed order.
+                const bool odd_first = (E & 1u) != 0u;
+                const uint32_t vote = __ballot_sync(kFull, odd_first);
                 a1 = a3 = false;
-                float sx, sy, sz;
-#pragma unroll
-                for (int phase = 0; phase < 3; ++phase) {
-                    if (phase == 1) {          // even monomers (slots 0, 2) of every chain
-                        float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
-                        xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
-                        bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
-                        a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
-                        bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
-                        a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
-                        X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
-                        X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
-                    } else {                   // odd monomers (slots 1, 3): phase 0 if odd_first, phase 2 if not
-                        // a chain whose turn it is not compares with u = +inf, which accepts nothing
-                        const bool due = (phase == 0) == odd_first;
-                        const float inf = __int_as_float(0x7F800000);
-                        const float u1 = due ? q1.u : inf, u3 = due ? q3.u : inf;
-                        float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
-                        xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
-                        bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
-                        const bool b1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, u1);
-                        bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
-                        const bool b3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, u3);
-                        X.y = b1 ? x1n : X.y; Y.y = b1 ? y1n : Y.y; Z.y = b1 ? z1n : Z.y;
-                        X.w = b3 ? x3n : X.w; Y.w = b3 ? y3n : Y.w; Z.w = b3 ? z3n : Z.w;
-                        a1 = a1 || b1; a3 = a3 || b3;
-                    }
+                auto even_set = [&]() {        // slots 0, 2 of every chain
+                    float sx, sy, sz;
+                    float xl = __shfl_up_sync(kFull, X.w, 1), yl = __shfl_up_sync(kFull, Y.w, 1), zl = __shfl_up_sync(kFull, Z.w, 1);
+                    xl = has_l0 ? xl : X.x; yl = has_l0 ? yl : Y.x; zl = has_l0 ? zl : Z.x;
+                    bond_sum(X.x, Y.x, Z.x, xl, yl, zl, X.y, Y.y, Z.y, sx, sy, sz);
+                    a0 = metropolis(bonded_delta(half_k0, mf0, q0.a, q0.b, q0.c, sx, sy, sz) + e0, q0.u);
+                    bond_sum(X.z, Y.z, Z.z, X.y, Y.y, Z.y, X.w, Y.w, Z.w, sx, sy, sz);
+                    a2 = metropolis(bonded_delta(half_k0, 2.0f, q2.a, q2.b, q2.c, sx, sy, sz) + e2, q2.u);
+                    X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
+                    X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
+                };
+                auto odd_set = [&](float u1, float u3) {   // slots 1, 3; a chain whose turn it is not is given u = +inf
+                    float sx, sy, sz;
+                    float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
+                    xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
+                    bond_sum(X.y, Y.y, Z.y, X.x, Y.x, Z.x, X.z, Y.z, Z.z, sx, sy, sz);
+                    const bool b1 = metropolis(bonded_delta(half_k0, 2.0f, q1.a, q1.b, q1.c, sx, sy, sz) + e1, u1);
+                    bond_sum(X.w, Y.w, Z.w, X.z, Y.z, Z.z, xr, yr, zr, sx, sy, sz);
+                    const bool b3 = metropolis(bonded_delta(half_k0, mf3, q3.a, q3.b, q3.c, sx, sy, sz) + e3, u3);
+                    X.y = b1 ? x1n : X.y; Y.y = b1 ? y1n : Y.y; Z.y = b1 ? z1n : Z.y;
+                    X.w = b3 ? x3n : X.w; Y.w = b3 ? y3n : Y.w; Z.w = b3 ? z3n : Z.w;
+                    a1 = a1 || b1; a3 = a3 || b3;
+                };
+                if (vote == 0u) {              // every chain of the warp: even set, then odd set
+                    even_set();
+                    odd_set(q1.u, q3.u);
+                } else if (vote == kFull) {    // every chain: odd set, then even set
+                    odd_set(q1.u, q3.u);
+                    even_set();
+                } else {                       // mixed (one tile in 16)
+                    const float inf = __int_as_float(0x7F800000);
+                    odd_set(odd_first ? q1.u : inf, odd_first ? q3.u : inf);
+                    even_set();
+                    odd_set(odd_first ? inf : q1.u, odd_first ? inf : q3.u);
                 }
             }
 
@@ -666,6 +701,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             if ((uint32_t)(bits >> 32)) atomicOr(dec_words + (gid >> 5) + 1u, (uint32_t)(bits >> 32));
         }
         X = Xn; Y = Yn; Z = Zn; C = Cn;
+        if (kOrder) E = En;
         tile = tile_n;
         tile_n = __shfl_sync(kFull, tile_nn, 0);
     }
