@@ -242,13 +242,24 @@ def aggregate_moves_per_s(n_beads: int, steps: int, world: int, ms_total_max: fl
 def all_configs(P, torch):
     """Step time of every config (profiles/*_all_configs.txt)."""
     peak, _ = peaks()
-    cases = [("C1", workloads.c1(), {}), ("C2 kappaN=50", workloads.c2(kappaN=50.0), {}), ("C3", workloads.c3(), {}),
-             ("C3 random set order", workloads.c3(), {"order": 1}), ("C5 a_s=0.05 (literal)", workloads.c5(), {}),
+    from dataclasses import replace
+    c3 = workloads.c3()
+    # the C3 melt with every chain handed in as a bond list (general-architecture kernel, one launch per
+    # independent set), and a melt of the same size of 3-arm stars (31 monomers: centre + 3 arms of 10)
+    c3_bonds = replace(c3, name="C3bonds", bonds=(tuple((j, j + 1) for j in range(31)),))
+    star = tuple((0 if k == 0 else 1 + a * 10 + k - 1, 1 + a * 10 + k) for a in range(3) for k in range(10))
+    stars = replace(c3, name="stars", specs=((528516, (0,) + (0,) * 15 + (1,) * 15),), bonds=(star,))
+    cases = [("C1", workloads.c1(), {}), ("C2 kappaN=50", workloads.c2(kappaN=50.0), {}), ("C3", c3, {}),
+             ("C3 random set order", c3, {"order": 1}), ("C3 molecule-parallel scheme (Code 1)", c3, {"scheme": 1}),
+             ("C3 chains as bond lists", c3_bonds, {}), ("3-arm star melt, 16.4M beads", stars, {}),
+             ("C5 a_s=0.05 (literal)", workloads.c5(), {}),
              ("C5 a_s=0.05 b0^2", workloads.c5(smc_step=0.05 / 63), {}), ("C4", workloads.c4(), {})]
     for name, w, kw in cases:
         sim = P.from_workload(w)
         if "order" in kw:
             sim.set_option(P.OPT_SET_ORDER, 1)
+        if "scheme" in kw:
+            sim.set_option(P.OPT_SCHEME, kw["scheme"])
         n = 200 if w.n_beads < 2e6 else (50 if w.n_beads < 1e8 else 10)
         sim.step(5)
         sim.sync()
@@ -261,7 +272,7 @@ def all_configs(P, torch):
             sim.sync()
             best = min(best, e0.elapsed_time(e1) / n)
         att, acc, _ = sim.stats()
-        print(f"{name:24s} beads {w.n_beads:>10d}  {best * 1e3:9.1f} us/step  {w.n_beads / best / 1e6:8.2f} G moves/s  "
+        print(f"{name:38s} beads {w.n_beads:>10d}  {best * 1e3:9.1f} us/step  {w.n_beads / best / 1e6:8.2f} G moves/s  "
               f"24 B/move of measured HBM peak {MOVE_BYTES_PER_BEAD * w.n_beads / (best * 1e-3) / 1e9 / peak:.3f}  "
               f"acceptance {acc / max(1, att):.3f}", flush=True)
         sim.destroy()

@@ -791,6 +791,87 @@ arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, fl
         atomicAdd(acc_slots + ((t >> 5) % kAccSlots), (unsigned long long)n_acc);
 }
 
+// The same with the molecules staged in shared memory, all independent sets in one launch: a warp copies a
+// group of consecutive molecules (group * N consecutive beads per coordinate array) with coalesced loads,
+// works through the sets one after the other -- the members of a set of all molecules of the group spread over
+// its lanes, neighbours read from shared memory, __syncwarp between sets -- and writes the group back: every
+// position crosses HBM once per sweep, and the architecture (offsets, neighbour lists, set members: the
+// compressed-architecture array of PAPER.md:344-354 in plain 32-bit words) sits in shared memory too.
+//   arch        nbr_off[N + 1] | nbr[2 n_bonds] | members[N] | set_off[n_sets + 1] | set_magic[n_sets]
+//               (set_magic = floor(2^32 / set size) + 1: item / set size by one multiply, exact below 2^16)
+//   group       molecules per warp and pass (group * N <= 65535)
+// Dynamic shared memory: arch words + toff[N], then warps * 3 * group * N floats.
+template <int kMove, bool kIncr, bool kRecord, bool kPack>
+__global__ void __launch_bounds__(256)
+arch_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
+                   const float* __restrict__ omega, uint32_t* __restrict__ counts,
+                   const uint32_t* __restrict__ toff_tab, const uint32_t* __restrict__ arch, uint32_t n_arch_words,
+                   uint32_t N, uint32_t n_bonds, uint32_t n_sets, uint32_t group, uint64_t n_mol, uint32_t gid0,
+                   const uint32_t* __restrict__ orig, uint32_t* __restrict__ dec_words,
+                   unsigned long long* __restrict__ acc_slots)
+{
+    extern __shared__ __align__(16) uint32_t s_words[];
+    const uint32_t lane = threadIdx.x & 31u, wib = threadIdx.x >> 5, warps = blockDim.x >> 5;
+    for (uint32_t k = threadIdx.x; k < n_arch_words; k += blockDim.x) s_words[k] = arch[k];
+    for (uint32_t k = threadIdx.x; k < N; k += blockDim.x) s_words[n_arch_words + k] = toff_tab[k];
+    __syncthreads();
+    const uint32_t* nbr_off = s_words;
+    const uint32_t* nbr = nbr_off + (N + 1u);
+    const uint32_t* members = nbr + 2u * n_bonds;
+    const uint32_t* set_off = members + N;
+    const uint32_t* set_magic = set_off + (n_sets + 1u);
+    const uint32_t* toff = s_words + n_arch_words;
+    const uint32_t head = (n_arch_words + N + 3u) & ~3u;
+    float* sx = reinterpret_cast<float*>(s_words + head) + (size_t)wib * 3u * group * N;
+    float* sy = sx + group * N;
+    float* sz = sy + group * N;
+    const uint64_t n_groups = (n_mol + group - 1u) / group;
+    uint32_t n_acc = 0;
+    for (uint64_t grp = (uint64_t)blockIdx.x * warps + wib; grp < n_groups; grp += (uint64_t)gridDim.x * warps) {
+        const uint64_t m0 = grp * group, base = m0 * N;
+        const uint32_t n_here = (uint32_t)min((uint64_t)group, n_mol - m0), n_floats = n_here * N;
+        for (uint32_t e = lane; e < n_floats; e += 32u) {
+            sx[e] = x[base + e];
+            sy[e] = y[base + e];
+            sz[e] = z[base + e];
+        }
+        __syncwarp();
+        for (uint32_t i_set = 0; i_set < n_sets; ++i_set) {
+            const uint32_t first = set_off[i_set], set_size = set_off[i_set + 1u] - first, magic = set_magic[i_set];
+            const uint32_t items = n_here * set_size;
+            for (uint32_t it = lane; it < items; it += 32u) {
+                const uint32_t m = set_size == 1u ? it : __umulhi(it, magic);   // it / set_size (2^32 / 1 has no 32-bit magic)
+                const uint32_t j = members[first + (it - m * set_size)];
+                const uint32_t i = m * N + j;
+                float px = sx[i], py = sy[i], pz = sz[i];
+                float bsx = 0.0f, bsy = 0.0f, bsz = 0.0f;
+                const uint32_t a0 = nbr_off[j], a1 = nbr_off[j + 1u];
+                for (uint32_t a = a0; a < a1; ++a) {                          // other sets: not written during this set
+                    const uint32_t k = m * N + nbr[a];
+                    const float bx = px - sx[k], by = py - sy[k], bz = pz - sz[k];
+                    if (a == a0) { bsx = bx; bsy = by; bsz = bz; } else { bsx = bsx + bx; bsy = bsy + by; bsz = bsz + bz; }
+                }
+                const uint32_t gid = gid0 + orig[m0 + m] * N + j;
+                const bool acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, bsx, bsy, bsz, (float)(a1 - a0),
+                                                                toff[j], gid);
+                if (acc) { sx[i] = px; sy[i] = py; sz[i] = pz; }
+                if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
+                n_acc += acc ? 1u : 0u;
+            }
+            __syncwarp();
+        }
+        for (uint32_t e = lane; e < n_floats; e += 32u) {
+            x[base + e] = sx[e];
+            y[base + e] = sy[e];
+            z[base + e] = sz[e];
+        }
+        __syncwarp();
+    }
+    n_acc = __reduce_add_sync(0xFFFFFFFFu, n_acc);
+    if (lane == 0 && n_acc)
+        atomicAdd(acc_slots + ((blockIdx.x * warps + wib) % kAccSlots), (unsigned long long)n_acc);
+}
+
 // ------------------------------------------------------------------------------------------------
 // Molecule-parallel scheme (Code 1): one thread per molecule, which N times picks
 // one of its particles at random and attempts to move it; attempts of one molecule are sequential

@@ -369,10 +369,13 @@ def _branched_melt(move="local", smc_step=0.0):
                               bonds=(star, ring, comb, None))
 
 
+@pytest.mark.parametrize("kernel", [P.KERNEL_AUTO, P.KERNEL_GENERIC], ids=["staged", "per-set"])
 @pytest.mark.parametrize("move,step", [("local", 0.0), ("smc", 0.05 / 15)])
-def test_stars_rings_and_combs(move, step):
+def test_stars_rings_and_combs(move, step, kernel):
+    """Default: the molecules staged in shared memory, all sets in one launch; KERNEL_GENERIC: one launch per set
+    on global memory."""
     w = _branched_melt(move, step)
-    lockstep(w, 5, xyz0=_tree_walk(w))
+    lockstep(w, 5, xyz0=_tree_walk(w), kernel=kernel)
 
 
 def test_linear_chain_given_as_bonds_equals_the_fused_kernel():
