@@ -440,7 +440,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 // tiles are processed here; the host sends a ragged tail (< 128 beads, whole chains) to the generic
 // kernel.  Block b owns the contiguous tile range [b T / B, (b+1) T / B); its warps take those tiles
 // round-robin.  Per tile and lane (4 consecutive monomers in registers):
-//   1. the next tile's positions are requested (register prefetch, hides the HBM latency);
+//   1. the tile's positions are requested (they are first needed after step 2, which hides the latency);
 //   2. all four Philox draws (they depend on nothing loaded);
 //   3. local move: all four trial positions, all eight cell indices, all eight omega gathers in
 //      flight at once -- dE_nb (Eq. 15) does not depend on the neighbours, only dE_b does;
@@ -531,9 +531,6 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     if (tile < t_end) {
         if (kOrder) E = s_perm[((tile - t_begin) << cpt_shift) + ci];
         const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * kTile + 4u * lane;
-        X = ld_stream(x + i0);
-        Y = ld_stream(y + i0);
-        Z = ld_stream(z + i0);
         C = orig[i0 >> log2N];
     }
     while (tile < t_end) {
@@ -545,13 +542,16 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         uint32_t tile_nn = 0u;
         if (lane == 0) tile_nn = atomicAdd(s_next + (wib & zero), 1u);
 
-        // 1. prefetch the next tile of this warp (clamped to the last tile: a harmless re-read)
+        // 1. the chain index of the next tile of this warp (clamped to the last tile: a harmless re-read)
         uint32_t En = 0u;
         if (kOrder) En = s_perm[((min(tile_n, t_end - 1u) - t_begin) << cpt_shift) + ci];
         const uint32_t i0n = kOrder ? (En & ~1u) + j0 : min(tile_n, t_end - 1u) * kTile + 4u * lane;
-        const float4 Xn = ld_stream(x + i0n);
-        const float4 Yn = ld_stream(y + i0n);
-        const float4 Zn = ld_stream(z + i0n);
+        // this tile's positions: asked for now, first needed after the four Philox draws below (~150
+        // instructions of this warp and as many of each of its four neighbours on the scheduler), which covers
+        // the latency without holding a second tile in registers
+        X = ld_stream(x + i0);
+        Y = ld_stream(y + i0);
+        Z = ld_stream(z + i0);
         const uint32_t Cn = orig[i0n >> log2N];
 
         // 2. random numbers of the four moves
@@ -700,7 +700,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             if ((uint32_t)bits) atomicOr(dec_words + (gid >> 5), (uint32_t)bits);
             if ((uint32_t)(bits >> 32)) atomicOr(dec_words + (gid >> 5) + 1u, (uint32_t)(bits >> 32));
         }
-        X = Xn; Y = Yn; Z = Zn; C = Cn;
+        C = Cn;
         if (kOrder) E = En;
         tile = tile_n;
         tile_n = __shfl_sync(kFull, tile_nn, 0);
