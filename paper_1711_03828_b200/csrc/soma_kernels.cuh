@@ -380,12 +380,15 @@ __device__ __forceinline__ float smc_exponent(float half_as_k0, float mf, float 
 // i_old, i_new: cell_at() of the old and the new position (same type).  kPack: the cell's word is index >> 1,
 // the type's half index & 1; the sums are exact modulo 2^32 whatever the order of the updates, so the word
 // always holds n_A + 65536 n_B (the field kernel checks that no half has outgrown its 16 bits).
+//   tk: the bead's type + k_rec as handed to cell_at() (k_rec is even for records, so bit 0 is the type: the
+//   increment does not depend on the cells and can be kept across tiles)
 template <bool kPack>
-__device__ __forceinline__ void count_follow(uint32_t* __restrict__ counts, bool acc, uint32_t i_old, uint32_t i_new)
+__device__ __forceinline__ void count_follow(uint32_t* __restrict__ counts, bool acc, uint32_t i_old, uint32_t i_new,
+                                             uint32_t tk)
 {
     if (acc && i_new != i_old) {
         if (kPack) {
-            const uint32_t one = 1u << ((i_new & 1u) << 4);
+            const uint32_t one = 1u << ((tk & 1u) << 4);
             atomicAdd(counts + (i_new >> 1), one);
             atomicAdd(counts + (i_old >> 1), 0u - one);
         } else {
@@ -418,7 +421,7 @@ __device__ __forceinline__ bool mc_move_s(const MoveP& P, const float* __restric
     x = acc ? x2 : x;
     y = acc ? y2 : y;
     z = acc ? z2 : z;
-    if (kIncr) count_follow<kPack>(counts, acc, i_old, i_new);
+    if (kIncr) count_follow<kPack>(counts, acc, i_old, i_new, toff + P.g.k_rec);
     return acc;
 }
 
@@ -643,10 +646,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
             // 5. occupation numbers follow the accepted moves
             if (kIncr) {
-                count_follow<kPack>(counts, a0, o0, n0);
-                count_follow<kPack>(counts, a1, o1, n1);
-                count_follow<kPack>(counts, a2, o2, n2);
-                count_follow<kPack>(counts, a3, o3, n3);
+                count_follow<kPack>(counts, a0, o0, n0, tk.x);
+                count_follow<kPack>(counts, a1, o1, n1, tk.y);
+                count_follow<kPack>(counts, a2, o2, n2, tk.z);
+                count_follow<kPack>(counts, a3, o3, n3, tk.w);
             }
         } else {
             // Smart-MC: the proposal needs the bonded force, i.e. the neighbours as they are now
@@ -667,7 +670,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             a2 = metropolis(smc_exponent(hak, 2.0f, bonded_delta(half_k0, 2.0f, dx2, dy2, dz2, sx2, sy2, sz2), e2), q2.u);
             X.x = a0 ? x0n : X.x; Y.x = a0 ? y0n : Y.x; Z.x = a0 ? z0n : Z.x;
             X.z = a2 ? x2n : X.z; Y.z = a2 ? y2n : Y.z; Z.z = a2 ? z2n : Z.z;
-            if (kIncr) { count_follow<kPack>(counts, a0, o0, n0); count_follow<kPack>(counts, a2, o2, n2); }
+            if (kIncr) { count_follow<kPack>(counts, a0, o0, n0, tk.x); count_follow<kPack>(counts, a2, o2, n2, tk.z); }
 
             float xr = __shfl_down_sync(kFull, X.x, 1), yr = __shfl_down_sync(kFull, Y.x, 1), zr = __shfl_down_sync(kFull, Z.x, 1);
             xr = has_r3 ? xr : X.w; yr = has_r3 ? yr : Y.w; zr = has_r3 ? zr : Z.w;
@@ -685,7 +688,7 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             a3 = metropolis(smc_exponent(hak, mf3, bonded_delta(half_k0, mf3, dx3, dy3, dz3, sx3, sy3, sz3), e3), q3.u);
             X.y = a1 ? x1n : X.y; Y.y = a1 ? y1n : Y.y; Z.y = a1 ? z1n : Z.y;
             X.w = a3 ? x3n : X.w; Y.w = a3 ? y3n : Y.w; Z.w = a3 ? z3n : Z.w;
-            if (kIncr) { count_follow<kPack>(counts, a1, o1, n1); count_follow<kPack>(counts, a3, o3, n3); }
+            if (kIncr) { count_follow<kPack>(counts, a1, o1, n1, tk.y); count_follow<kPack>(counts, a3, o3, n3, tk.w); }
         }
 
         st_stream(x + i0, X);

@@ -97,3 +97,21 @@ def test_stale_profile_entries_are_ignored(tmp_path, monkeypatch):
     assert bench.profile_entry("C3")["dram_bytes"] == 5 and bench.profile_entry("C1") is None
     (tmp_path / "paper_1711_03828_b200" / "csrc" / "k.cuh").write_text("v2")      # the kernels changed
     assert bench.profile_entry("C3") is None
+
+
+def test_ingest_ncu_csv_sums_the_launches_of_one_sweep(tmp_path, monkeypatch):
+    import bench
+    monkeypatch.setattr(bench, "ROOT", tmp_path)
+    (tmp_path / "profiles").mkdir()
+    (tmp_path / "paper_1711_03828_b200" / "csrc").mkdir(parents=True)
+    (tmp_path / "paper_1711_03828_b200" / "csrc" / "k.cuh").write_text("kernels")
+    csv = tmp_path / "t.csv"
+    head = '"ID","Process ID","Process Name","Host Name","Kernel Name","Context","Stream","Block Size","Grid Size","Device","CC","Section Name","Metric Name","Metric Unit","Metric Value"'
+    row = lambda i, m, u, v: f'"{i}","1","python","h","k","1","7","(640, 1, 1)","(148, 1, 1)","0","10.0","Command line profiler metrics","{m}","{u}","{v}"'
+    csv.write_text("==PROF== Connected\n" + head + "\n" + "\n".join([
+        row(0, "dram__bytes_read.sum", "Mbyte", "200.5"), row(0, "dram__bytes_write.sum", "byte", "1,000"),
+        row(0, "smsp__inst_executed.sum", "inst", "70"), row(1, "dram__bytes_read.sum", "byte", "24"),
+        row(1, "dram__bytes_write.sum", "byte", "6"), row(1, "smsp__inst_executed.sum", "inst", "5")]) + "\n")
+    bench.ingest_ncu_csv(str(csv), "C5")
+    e = bench.profile_entry("C5")
+    assert e["dram_bytes"] == 200500000 + 1000 + 30 and e["inst_executed"] == 75 and e["launches"] == 2
