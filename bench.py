@@ -298,6 +298,9 @@ def main():
                     help="N > 1: ONE system of N x the config's chains in a box N x as long (same density), molecules "
                          "distributed over the ranks, one all-reduce of the occupation numbers per sweep (SURVEY 8(e)); "
                          "default: N independent replicas")
+    ap.add_argument("--peers", action="store_true",
+                    help="with --sharded: no all-reduce -- every rank's field kernel reduces all ranks' exchange arrays "
+                         "itself over peer memory (CUDA IPC / NVLink), behind a one-element all-reduce as the barrier")
     ap.add_argument("--ingest-ncu", metavar="CSV",
                     help="no run: write the profiles/traffic.json entry of --config from an ncu --csv metrics file")
     args = ap.parse_args()
@@ -376,7 +379,9 @@ def main():
         from paper_1711_03828_b200.sharded import ShardedSoma
         w = replace(w, specs=tuple((n * world, t) for n, t in w.specs), box=(w.box[0] * world, w.box[1], w.box[2]),
                     grid=(w.grid[0] * world, w.grid[1], w.grid[2]))
-        config.update({"parallelism": f"one system over {world} GPU(s): molecules distributed, counts all-reduced every sweep",
+        config.update({"parallelism": f"one system over {world} GPU(s): molecules distributed, " +
+                                      ("exchange arrays reduced by the field kernel over peer memory" if args.peers and world > 1
+                                       else "exchange array all-reduced every sweep"),
                        "chains": w.n_chains, "beads": w.n_beads, "grid": list(w.grid), "box": list(w.box)})
 
         class _Sharded:                       # the calls bench makes, on this rank's part of the system
@@ -393,7 +398,7 @@ def main():
             def __getattr__(self, name):
                 return getattr(self.sim, name)
 
-        sim = _Sharded(ShardedSoma(w, dist=dist))
+        sim = _Sharded(ShardedSoma(w, dist=dist, peers=args.peers))
     else:
         wr = w if rank == 0 else replace(w, seed=w.seed + rank)   # independent replicas
         sim = P.from_workload(wr, xyz0=None)       # Gaussian-walk start drawn on the device from the seed

@@ -186,6 +186,25 @@ int soma_shard_exchange(soma_ctx *ctx, void **dev_words, uint64_t *n_words);
  * to_host = 0 copies host_words in.  Synchronises. */
 int soma_shard_exchange_copy(soma_ctx *ctx, uint32_t *host_words, int to_host);
 
+/* Peer mode: the field kernel does the reduction itself.  Instead of the caller's all-reduce, the kernel launched by
+ * soma_shard_fields reads the exchange arrays of ALL ranks word by word through peer memory -- the other GPUs'
+ * memory over NVLink / NVSwitch, mapped with CUDA IPC (or plain device addresses when the ranks are contexts of one
+ * process) -- adds them up, folds the sum into the whole system's occupation numbers and computes omega: one kernel
+ * for the exchange step and a4.  What remains for the caller is a BARRIER between soma_shard_moves and
+ * soma_shard_fields (every rank's move kernel must have finished before any rank's field kernel reads its array;
+ * in stream order, e.g. a one-element all-reduce enqueued behind the moves).  The exchange allocation holds two
+ * buffers used alternately: the arrays a field kernel has read are left untouched (other ranks read them too) and
+ * this rank's other buffer -- which every rank finished reading a sweep ago, by the same barrier -- is cleared for
+ * the next sweep.  soma_shard_exchange then returns the buffer the NEXT soma_shard_moves counts into.
+ *   soma_shard_peer_handle   64 bytes: the CUDA IPC handle of this rank's exchange allocation, to be sent to the peers
+ *   soma_shard_set_peers     n_ranks, my_rank, and for every other rank either peer_dev[r] (device address of its
+ *                            allocation = what soma_shard_exchange returned right after soma_init_shard; same
+ *                            process) or, where that is NULL, handles[64 r .. 64 r + 63] (opened here).  Call it on
+ *                            every rank after soma_init_shard and before the first soma_shard_fields.
+ * Needs SOMA_OPT_FIELD_INTERVAL = 1 and the same SOMA_OPT_COUNT_BITS on every rank. */
+int soma_shard_peer_handle(soma_ctx *ctx, void *handle64);
+int soma_shard_set_peers(soma_ctx *ctx, int n_ranks, int my_rank, void *const *peer_dev, const void *handles);
+
 /* a4: folds the (summed) exchange array into the whole system's occupation numbers, clears it, and computes
  * omega.  advance != 0 closes the sweep begun by soma_shard_moves (sweep counter + 1; omega is only
  * recomputed when SOMA_OPT_FIELD_INTERVAL says so, the numbers are folded in any case); advance = 0: stage 1

@@ -30,7 +30,7 @@ SYMBOLS = (
     "soma_set_external", "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
     "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields", "soma_shard_exchange",
-    "soma_shard_exchange_copy",
+    "soma_shard_exchange_copy", "soma_shard_peer_handle", "soma_shard_set_peers",
 )
 
 
@@ -63,6 +63,8 @@ def load() -> C.CDLL:
     L.soma_shard_fields.argtypes = [vp, i32]
     L.soma_shard_exchange.argtypes = [vp, C.POINTER(vp), C.POINTER(u64)]
     L.soma_shard_exchange_copy.argtypes = [vp, vp, i32]
+    L.soma_shard_peer_handle.argtypes = [vp, vp]
+    L.soma_shard_set_peers.argtypes = [vp, i32, i32, C.POINTER(vp), vp]
     L.soma_step.argtypes = [vp, i32]
     L.soma_fields.argtypes = [vp, vp, vp, i32]
     L.soma_positions.argtypes = [vp, vp, i32]
@@ -164,6 +166,20 @@ class Soma:
         p, n = C.c_void_p(), C.c_uint64()
         _check(self._L.soma_shard_exchange(self._h, C.byref(p), C.byref(n)))
         return int(p.value), int(n.value)
+
+    def shard_peer_handle(self) -> bytes:
+        """CUDA IPC handle (64 bytes) of this rank's exchange allocation."""
+        buf = C.create_string_buffer(64)
+        _check(self._L.soma_shard_peer_handle(self._h, buf))
+        return buf.raw
+
+    def shard_set_peers(self, n_ranks: int, my_rank: int, peer_addresses=None, handles=None) -> None:
+        """peer_addresses: per rank a device address (same process) or None; handles: per rank 64 bytes or None."""
+        addr = (C.c_void_p * n_ranks)(*[C.c_void_p(a) if a else C.c_void_p(None) for a in (peer_addresses or [None] * n_ranks)])
+        blob = None
+        if handles is not None:
+            blob = C.create_string_buffer(b"".join(h if h is not None else bytes(64) for h in handles), 64 * n_ranks)
+        _check(self._L.soma_shard_set_peers(self._h, n_ranks, my_rank, addr, blob))
 
     def shard_exchange_tensor(self):
         """The exchange array as a torch int32 tensor on the device (no copy): what the all-reduce runs on."""

@@ -105,6 +105,12 @@ struct soma_ctx {
     uint64_t n_beads = 0, n_pad = 0, cells = 0;
     uint64_t n_beads_global = 0;     // beads of the whole system (= n_beads unless this context is a shard)
     int sharded = 0;                 // created by soma_init_shard: soma_shard_moves / soma_shard_fields instead of soma_step
+    // peer mode (soma_shard_set_peers): the field kernel reduces the ranks' exchange arrays itself over peer memory.
+    // The allocation holds two buffers of n_types * cells words used alternately (exchange = the current one).
+    uint32_t* exchange_base = nullptr;
+    int n_peers = 0, my_rank = 0, peer_parity = 0;
+    std::vector<void*> peer_opened;          // CUDA IPC mappings to close
+    const uint32_t** peer_table = nullptr;   // device: [n_peers] base addresses of the ranks' allocations
     uint32_t* exchange = nullptr;    // shard: what this rank's move kernels count into; summed over the ranks by the caller,
                                      // folded into counts (the whole system's numbers) by the field kernel, which clears it
 
@@ -520,7 +526,8 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
 
 // a4.  A shard folds the exchange array (summed over the ranks by now) into its copy of the whole system's
 // occupation numbers on the way.
-int launch_fields(soma_ctx* c, bool fold_exchange = false)
+//   fold: 0 no exchange array, 1 fold this rank's (already summed) exchange array, 2 reduce the peers' arrays
+int launch_fields(soma_ctx* c, int fold = 0)
 {
     const soma::FieldP F = c->fieldp();
 #ifndef SOMA_FIELD_THREADS
@@ -533,15 +540,19 @@ int launch_fields(soma_ctx* c, bool fold_exchange = false)
     // One cell per thread: with programmatic dependent launch the many small blocks slip in behind the
     // draining move blocks.
     const unsigned long long n = c->n_beads_global;        // the beads counts holds (the packed format's overflow check)
-    uint32_t* ex = fold_exchange ? c->exchange : nullptr;
+    const size_t stride = (size_t)c->cells * c->n_types;   // words per exchange buffer
+    uint32_t* ex = fold == 1 ? c->exchange : fold == 2 ? c->exchange_base + (size_t)(1 - c->peer_parity) * stride : nullptr;
+    const uint32_t* const* peers = fold == 2 ? c->peer_table : nullptr;
+    const uint32_t n_peers = (uint32_t)c->n_peers;
+    const size_t peer_off = (size_t)c->peer_parity * stride;
     if (c->pack) {
-        CU(launch_pdl(pdl, soma::field_kernel<2, true>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex));
+        CU(launch_pdl(pdl, soma::field_kernel<2, true>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex, peers, n_peers, peer_off));
         return SOMA_OK;
     }
     switch (c->n_types) {
-        case 1: CU(launch_pdl(pdl, soma::field_kernel<1, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
-        case 2: CU(launch_pdl(pdl, soma::field_kernel<2, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
-        default: CU(launch_pdl(pdl, soma::field_kernel<0, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex)); break;
+        case 1: CU(launch_pdl(pdl, soma::field_kernel<1, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex, peers, n_peers, peer_off)); break;
+        case 2: CU(launch_pdl(pdl, soma::field_kernel<2, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex, peers, n_peers, peer_off)); break;
+        default: CU(launch_pdl(pdl, soma::field_kernel<0, false>, blocks, threads, 0, c->stream, F, c->counts, c->omega, c->ext, c->forbidden, c->ticket_sum, c->overflow_dev, n, ex, peers, n_peers, peer_off)); break;
     }
     return SOMA_OK;
 }
@@ -698,7 +709,9 @@ void soma_destroy(soma_ctx* c)
     cudaStreamSynchronize(c->stream);
     for (auto& e : c->ev) cudaEventDestroy(e);
     cudaFree(c->x); cudaFree(c->y); cudaFree(c->z);
-    cudaFree(c->exchange);
+    for (void* m : c->peer_opened) cudaIpcCloseMemHandle(m);
+    cudaFree(c->peer_table);
+    cudaFree(c->exchange_base);
     cudaFree(c->n_outside);
     cudaFree(c->ticket_sum);
     cudaFree(c->grid_stage);
@@ -907,7 +920,11 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
     CUI(cudaMalloc(&c->y, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->z, sizeof(float) * c->n_pad));
     CUI(cudaMalloc(&c->counts, sizeof(uint32_t) * cells * n_types));
-    if (c->sharded) CUI(cudaMalloc(&c->exchange, sizeof(uint32_t) * cells * n_types));
+    if (c->sharded) {
+        CUI(cudaMalloc(&c->exchange_base, 2 * sizeof(uint32_t) * cells * n_types));
+        CUI(cudaMemsetAsync(c->exchange_base, 0, 2 * sizeof(uint32_t) * cells * n_types, c->stream));
+        c->exchange = c->exchange_base;
+    }
     CUI(cudaMalloc(&c->omega, sizeof(float) * cells * n_types));
     CUI(cudaMalloc(&c->toff, sizeof(uint32_t) * toff_host.size()));
     if (!arch_host.empty()) {
@@ -1079,13 +1096,66 @@ int soma_shard_exchange_copy(soma_ctx* c, uint32_t* host_words, int to_host)
     return SOMA_OK;
 }
 
+int soma_shard_peer_handle(soma_ctx* c, void* handle64)
+{
+    if (!c || !handle64) return fail(SOMA_EINVAL, "soma_shard_peer_handle: NULL argument");
+    DeviceGuard on_device(c->device);
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_peer_handle: the context was not created by soma_init_shard");
+    static_assert(sizeof(cudaIpcMemHandle_t) == 64, "CUDA IPC handles are 64 bytes");
+    cudaIpcMemHandle_t h;
+    CU(cudaIpcGetMemHandle(&h, c->exchange_base));
+    std::memcpy(handle64, &h, sizeof h);
+    return SOMA_OK;
+}
+
+int soma_shard_set_peers(soma_ctx* c, int n_ranks, int my_rank, void* const* peer_dev, const void* handles)
+{
+    if (!c) return fail(SOMA_EINVAL, "soma_shard_set_peers: ctx is NULL");
+    DeviceGuard on_device(c->device);
+    if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_set_peers: the context was not created by soma_init_shard");
+    if (n_ranks < 1 || my_rank < 0 || my_rank >= n_ranks || (!peer_dev && !handles))
+        return fail(SOMA_EINVAL, "soma_shard_set_peers: need 0 <= my_rank < n_ranks and the peers' addresses or handles");
+    if (c->n_peers) return fail(SOMA_ESTATE, "soma_shard_set_peers: the peers of this context are already set");
+    if (c->sweep != 0) return fail(SOMA_ESTATE, "soma_shard_set_peers: call it before the first sweep");
+    std::vector<const uint32_t*> table(n_ranks);
+    for (int r = 0; r < n_ranks; ++r) {
+        if (r == my_rank) { table[r] = c->exchange_base; continue; }
+        if (peer_dev && peer_dev[r]) { table[r] = (const uint32_t*)peer_dev[r]; continue; }
+        if (!handles) return fail(SOMA_EINVAL, "soma_shard_set_peers: no address and no handle for rank %d", r);
+        cudaIpcMemHandle_t h;
+        std::memcpy(&h, (const char*)handles + 64 * (size_t)r, sizeof h);
+        void* mapped = nullptr;
+        CU(cudaIpcOpenMemHandle(&mapped, h, cudaIpcMemLazyEnablePeerAccess));
+        c->peer_opened.push_back(mapped);
+        table[r] = (const uint32_t*)mapped;
+    }
+    CU(cudaMalloc(&c->peer_table, sizeof(uint32_t*) * n_ranks));
+    CU(cudaMemcpyAsync(c->peer_table, table.data(), sizeof(uint32_t*) * n_ranks, cudaMemcpyHostToDevice, c->stream));
+    CU(cudaStreamSynchronize(c->stream));
+    c->n_peers = n_ranks;
+    c->my_rank = my_rank;
+    return SOMA_OK;
+}
+
 int soma_shard_fields(soma_ctx* c, int advance)
 {
     if (!c) return fail(SOMA_EINVAL, "soma_shard_fields: ctx is NULL");
     DeviceGuard on_device(c->device);
     if (!c->sharded) return fail(SOMA_ESTATE, "soma_shard_fields: the context was not created by soma_init_shard");
+    if (c->n_peers) {
+        // the field kernel reduces the ranks' exchange arrays itself (peer memory), folds the sum into the whole
+        // system's numbers and clears this rank's other buffer, into which the next sweep counts
+        if (c->field_interval > 1)
+            return fail(SOMA_ESTATE, "soma_shard_fields: with peers set, SOMA_OPT_FIELD_INTERVAL must be 1");
+        int rc = launch_fields(c, 2);
+        if (rc) return rc;
+        c->peer_parity ^= 1;
+        c->exchange = c->exchange_base + (size_t)c->peer_parity * c->cells * c->n_types;
+        if (advance) c->sweep += 1;
+        return SOMA_OK;
+    }
     if (!advance || c->field_interval <= 1 || (c->sweep + 1) % (uint64_t)c->field_interval == 0) {
-        int rc = launch_fields(c, true);                   // a4 from the occupation numbers of the whole system
+        int rc = launch_fields(c, 1);                      // a4 from the occupation numbers of the whole system
         if (rc) return rc;
     } else {                                               // the counts stay current; omega is not due
         const uint64_t n = counts_bytes(c) / sizeof(uint32_t);

@@ -1066,12 +1066,19 @@ __device__ __forceinline__ void field_of_cell(const FieldP& F, const uint32_t (&
 //              kernels of this rank counted into, summed over all ranks by the caller: the change of the whole
 //              system's occupation numbers since the last call, in the format of counts.  It is added to counts
 //              and cleared for the next sweep.  Sums of words are exact modulo 2^32, packed or not.
+//   peers      NULL, or the exchange arrays of ALL ranks (this one included) in peer memory -- other GPUs over
+//              NVLink / NVSwitch, or CUDA IPC mappings: the kernel does the reduction itself, word by word, instead
+//              of a collective before it (n_peers pointers, each read at word offset peer_off).  Nobody may
+//              still be writing them (the caller's barrier).  The arrays read are left as they are -- other
+//              ranks read them too -- and `exchange` is then this rank's OTHER buffer, which every rank has
+//              finished reading a sweep ago: it is cleared for the next sweep (double buffering, soma_b200.cu).
 template <int kTypes, bool kPack>
 __global__ void __launch_bounds__(256)
 field_kernel(const FieldP F, uint32_t* __restrict__ counts, float* __restrict__ omega,
              const float* __restrict__ ext, const uint8_t* __restrict__ forbidden,
              unsigned long long* __restrict__ ticket_sum, uint32_t* __restrict__ overflow,
-             unsigned long long n_counted, uint32_t* __restrict__ exchange)
+             unsigned long long n_counted, uint32_t* __restrict__ exchange,
+             const uint32_t* const* __restrict__ peers, uint32_t n_peers, size_t peer_off)
 {
     static_assert(!kPack || kTypes == 2, "packed occupation numbers: two types");
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
@@ -1084,7 +1091,11 @@ field_kernel(const FieldP F, uint32_t* __restrict__ counts, float* __restrict__ 
         float w[kMaxTypes];
         if (kPack) {
             uint32_t v = counts[c];
-            if (exchange) {
+            if (peers) {
+                for (uint32_t r = 0; r < n_peers; ++r) v += __ldcg(peers[r] + peer_off + c);
+                counts[c] = v;
+                exchange[c] = 0u;
+            } else if (exchange) {
                 v += exchange[c];
                 counts[c] = v;
                 exchange[c] = 0u;
@@ -1098,7 +1109,11 @@ field_kernel(const FieldP F, uint32_t* __restrict__ counts, float* __restrict__ 
                 if (i >= nt) continue;
                 const size_t at = (size_t)i * F.cells + c;
                 n[i] = counts[at];
-                if (exchange) {
+                if (peers) {
+                    for (uint32_t r = 0; r < n_peers; ++r) n[i] += __ldcg(peers[r] + peer_off + at);
+                    counts[at] = n[i];
+                    exchange[at] = 0u;
+                } else if (exchange) {
                     n[i] += exchange[at];
                     counts[at] = n[i];
                     exchange[at] = 0u;

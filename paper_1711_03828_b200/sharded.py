@@ -9,6 +9,12 @@ kernel reads the sum from (no copy, no conversion in between) -- the only exchan
 Everything else is the single-GPU library: ``soma_init_shard``, ``soma_shard_moves``,
 ``soma_shard_exchange``, ``soma_shard_fields`` (include/soma_b200.h).
 
+``peers=True`` replaces the all-reduce by the library's peer mode: the ranks exchange the CUDA IPC handles of
+their exchange allocations once, and from then on every rank's field kernel reads all ranks' arrays over
+NVLink / NVSwitch peer memory and reduces them itself -- the exchange step and a4 in one kernel.  What is left of
+the collective is a barrier (a one-element all-reduce in stream order with NCCL; a stream synchronisation and a
+host barrier with any other backend).
+
 Because the Philox counter of a bead is its index in the whole system and integer sums commute, the
 trajectory does not depend on the number of ranks: positions, occupation numbers and fields equal
 those of the undivided system bit for bit.
@@ -57,7 +63,8 @@ def local_positions(xyz_global: np.ndarray, slices: Sequence[Tuple[int, int]]) -
 class ShardedSoma:
     """This rank's part of a system described by a ``workloads.Workload`` (rank / world from ``dist``)."""
 
-    def __init__(self, w, dist=None, xyz0_global: Optional[np.ndarray] = None, stream: Optional[int] = None):
+    def __init__(self, w, dist=None, xyz0_global: Optional[np.ndarray] = None, stream: Optional[int] = None,
+                 peers: bool = False):
         import torch
         self.dist = dist
         self.rank = dist.get_rank() if dist is not None else 0
@@ -75,10 +82,26 @@ class ShardedSoma:
         self.n_types = w.n_types
         # the library's exchange array as a tensor (uint32 bits in int32: sums are exact modulo 2^32)
         self.exchange = self.sim.shard_exchange_tensor()
+        self.peers = bool(peers) and self.world > 1
+        if self.peers:
+            handles = [None] * self.world
+            dist.all_gather_object(handles, self.sim.shard_peer_handle())
+            self.sim.shard_set_peers(self.world, self.rank,
+                                     handles=[None if r == self.rank else h for r, h in enumerate(handles)])
+            self._in_stream = dist.get_backend() == "nccl"
+            self._token = torch.zeros(1, dtype=torch.int32, device="cuda") if self._in_stream else None
         self._exchange(advance=False)
 
     def _exchange(self, advance: bool) -> None:
-        if self.dist is not None and self.world > 1:
+        if self.peers:
+            # every rank's kernels have counted before any rank's field kernel reads: a barrier is all that is
+            # left of the collective (in stream order with NCCL: no host synchronisation)
+            if self._in_stream:
+                self.dist.all_reduce(self._token)
+            else:
+                self.sim.sync()
+                self.dist.barrier()
+        elif self.dist is not None and self.world > 1:
             self.dist.all_reduce(self.exchange)                   # the only collective of the path (sum), in place
         self.sim.shard_fields(advance=advance)                    # a4 from the whole system's n_i(c)
 

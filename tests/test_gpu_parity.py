@@ -696,6 +696,99 @@ def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move,
         sim.destroy()
 
 
+@pytest.mark.parametrize("count_bits", [0, 16])
+def test_three_shards_reduce_their_exchange_arrays_in_the_field_kernel(count_bits):
+    """Peer mode: no all-reduce -- every shard's field kernel reads the exchange arrays of all three (here three
+    contexts of one process on one device, so the peers' addresses are plain device pointers), adds them, folds
+    the sum and computes omega.  Stepped one after the other (all moves, then all field kernels: the barrier the
+    caller owes), the shards equal the undivided context bit for bit, sweep after sweep (double-buffered arrays)."""
+    from paper_1711_03828_b200.sharded import local_positions, shard_layout
+    w = workloads.Workload("shard_peers", ((1301, workloads.diblock(32, 16)), (77, workloads.homopolymer(8, 1))), 32, 2,
+                           (4.0, 4.0, 3.0), (8, 8, 6), 20.0, 50.0, 0.1, 11)
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    whole = P.from_workload(w, xyz0=xyz0)
+    specs = [(n, np.asarray(t, np.uint8)) for n, t in w.specs]
+    shards = []
+    for rank in range(3):
+        local, first, n_global, slices = shard_layout(specs, rank, 3)
+        sim = P.Soma(local, w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A, w.seed,
+                     xyz0=local_positions(xyz0, slices), spec_first_bead=first, global_n_beads=n_global)
+        sim.set_option(P.OPT_COUNT_BITS, count_bits)
+        shards.append((sim, slices))
+    addresses = [sim.shard_exchange()[0] for sim, _ in shards]
+    for rank, (sim, _) in enumerate(shards):
+        sim.shard_set_peers(3, rank, peer_addresses=addresses)
+    for sim, _ in shards:
+        sim.shard_fields(advance=False)                   # stage 1: the three histograms, summed by each kernel
+    for sweep in range(7):
+        om_w, cnt_w = whole.fields()
+        for sim, slices in shards:
+            om_s, cnt_s = sim.fields()
+            assert np.array_equal(cnt_s, cnt_w) and np.array_equal(om_s, om_w), sweep
+            assert np.array_equal(sim.positions(), local_positions(whole.positions(), slices))
+        whole.step(1)
+        for sim, _ in shards:
+            sim.shard_moves()
+        for sim, _ in shards:                             # every rank has moved: the barrier
+            sim.sync()
+        for sim, _ in shards:
+            sim.shard_fields(advance=True)
+    assert sum(sim.stats()[1] for sim, _ in shards) == whole.stats()[1]
+    with pytest.raises(P.SomaError):
+        shards[0][0].shard_set_peers(3, 0, peer_addresses=addresses)     # only once
+    whole.destroy()
+    for sim, _ in shards:
+        sim.destroy()
+
+
+def _peer_rank(rank, world, port, out):
+    import os
+    import torch.distributed as dist
+    from paper_1711_03828_b200.sharded import ShardedSoma
+    os.environ.update(MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    dist.init_process_group("gloo", rank=rank, world_size=world)
+    w = workloads.c1()
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    sh = ShardedSoma(w, dist=dist, xyz0_global=xyz0, peers=True)
+    sh.step(6)
+    om, cnt = sh.fields()
+    out[rank] = (sh.positions(), om, cnt, sh.slices)
+    dist.barrier()                                        # nobody unmaps memory a peer's kernel may still read
+    sh.destroy()
+    dist.destroy_process_group()
+
+
+def test_two_processes_share_their_exchange_arrays_through_cuda_ipc():
+    """The peer mode across processes: two ranks (processes) on this one GPU, their exchange allocations mapped
+    into each other with CUDA IPC handles, a host barrier (gloo) in place of the collective -- no kernel of one
+    rank waits for another.  Both equal the undivided context bit for bit."""
+    import socket
+    import torch.multiprocessing as mp
+    from paper_1711_03828_b200.sharded import local_positions
+    with socket.socket() as s_:
+        s_.bind(("127.0.0.1", 0))
+        port = s_.getsockname()[1]
+    ctx = mp.get_context("spawn")
+    with ctx.Manager() as m:
+        out = m.dict()
+        procs = [ctx.Process(target=_peer_rank, args=(r, 2, port, out)) for r in range(2)]
+        for p_ in procs:
+            p_.start()
+        for p_ in procs:
+            p_.join(timeout=300)
+        assert all(p_.exitcode == 0 for p_ in procs), [p_.exitcode for p_ in procs]
+        res = dict(out)
+    w = workloads.c1()
+    whole = P.from_workload(w, xyz0=np.stack(workloads.gaussian_walks(w)))
+    whole.step(6)
+    om_w, cnt_w = whole.fields()
+    for rank in range(2):
+        pos, om, cnt, slices = res[rank]
+        assert np.array_equal(cnt, cnt_w) and np.array_equal(om, om_w)
+        assert np.array_equal(pos, local_positions(whole.positions(), slices))
+    whole.destroy()
+
+
 def test_sharded_driver_with_one_rank_equals_the_plain_context():
     from paper_1711_03828_b200.sharded import ShardedSoma
     w = workloads.c1()
