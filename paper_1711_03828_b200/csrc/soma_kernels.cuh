@@ -502,26 +502,30 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         // needs nothing of the predecessor kernel (orig[] only changes in a re-sort), so it runs before the wait.
         // The lanes of a warp hold different chains, and a warp whose chains all start with the same set does
         // four evaluations per lane like the fixed order, a mixed one six (three phases); so the chains are
-        // regrouped by their bit within groups of 32 consecutive chains -- tiles are made of 128 / N consecutive
-        // entries of the list -- and (N = 32) at most one tile in eight is mixed, while a tile's chains stay
-        // neighbours in the storage order.  A stable partition per group: a warp per group, a lane per chain.
-        for (uint32_t lo0 = wib * 32u; lo0 < n_slots; lo0 += 8u * kWarps * 32u) {
-            uint32_t first[8];                                // eight groups' loads in flight
+        // regrouped by their bit within groups of 64 consecutive chains -- tiles are made of 128 / N consecutive
+        // entries of the list -- and (N = 32) at most one tile in sixteen is mixed, while a tile's chains stay
+        // neighbours in the storage order.  A stable partition per group: a warp per group, two chains per lane.
+        for (uint32_t lo0 = wib * 64u; lo0 < n_slots; lo0 += 4u * kWarps * 64u) {
+            uint32_t first[8];                                // four groups' loads in flight
 #pragma unroll
             for (uint32_t k = 0; k < 8u; ++k) {
-                const uint32_t s = lo0 + k * kWarps * 32u + lane;
+                const uint32_t s = lo0 + (k >> 1) * kWarps * 64u + (k & 1u) * 32u + lane;
                 first[k] = s < n_slots ? orig[slot_begin + s] : 0u;
             }
 #pragma unroll
-            for (uint32_t k = 0; k < 8u; ++k) {
-                const uint32_t lo = lo0 + k * kWarps * 32u, s = lo + lane;
+            for (uint32_t k = 0; k < 4u; ++k) {
+                const uint32_t lo = lo0 + k * kWarps * 64u, sa = lo + lane, sb = sa + 32u;
                 if (lo >= n_slots) break;
-                const uint32_t b = s < n_slots ? first_set_bit(gid0 + (first[k] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
-                const uint32_t in = __ballot_sync(kFull, s < n_slots), ones = __ballot_sync(kFull, b != 0u);
+                const uint32_t ba = sa < n_slots ? first_set_bit(gid0 + (first[2 * k] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
+                const uint32_t bb = sb < n_slots ? first_set_bit(gid0 + (first[2 * k + 1] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
+                const uint32_t ones_a = __ballot_sync(kFull, ba != 0u), ones_b = __ballot_sync(kFull, bb != 0u);
+                const uint32_t zeros_a = __ballot_sync(kFull, sa < n_slots) & ~ones_a, zeros_b = __ballot_sync(kFull, sb < n_slots) & ~ones_b;
                 const uint32_t below = (1u << lane) - 1u;
-                const uint32_t n_zero = __popc(in & ~ones);
-                const uint32_t pos = b ? n_zero + __popc(ones & below) : __popc(in & ~ones & below);
-                if (s < n_slots) s_perm[lo + pos] = ((slot_begin + s) << log2N) | b;   // N >= 4: the low bits are free
+                const uint32_t n_zero = __popc(zeros_a) + __popc(zeros_b);
+                const uint32_t pos_a = ba ? n_zero + __popc(ones_a & below) : __popc(zeros_a & below);
+                const uint32_t pos_b = bb ? n_zero + __popc(ones_a) + __popc(ones_b & below) : __popc(zeros_a) + __popc(zeros_b & below);
+                if (sa < n_slots) s_perm[lo + pos_a] = ((slot_begin + sa) << log2N) | ba;   // N >= 4: the low bits are free
+                if (sb < n_slots) s_perm[lo + pos_b] = ((slot_begin + sb) << log2N) | bb;
             }
         }
     }
