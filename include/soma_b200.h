@@ -63,7 +63,9 @@ enum {
     SOMA_OPT_MOVE = 2,             /* 1: local displacement (default), 2: Smart-MC                            */
     SOMA_OPT_SMC_STEP = 3,         /* Smart-MC step a_s in R_e0^2 (> 0)                                       */
     SOMA_OPT_RECORD_DECISIONS = 4, /* 1: keep the accept/reject bit of every move of the last sweep           */
-    SOMA_OPT_KERNEL = 5,           /* 0: auto (default), 1: force the generic two-launch kernels,             */
+    SOMA_OPT_KERNEL = 5,           /* 0: auto (default); 1: force the one-thread-per-monomer kernels on global */
+                                   /* memory (two launches per sweep for linear chains, one per independent   */
+                                   /* set for bond-list architectures, no shared-memory staging);              */
                                    /* 2: chain-resident fused kernel (error if an architecture cannot use it) */
     SOMA_OPT_DENSITY = 6,          /* 0: incremental count update fused into the move kernel (default),       */
                                    /* 1: clear + full histogram kernel after every sweep                      */
