@@ -169,7 +169,10 @@ int soma_init(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_
  * and once after soma_init_shard (or after every rank's soma_set_positions): all-reduce; soma_shard_fields(ctx, 0).
  * No copy and no conversion lies between the move kernel, the collective and the field kernel.  The
  * positions, occupation numbers and fields equal those of the undivided system bit for bit.  soma_step
- * returns SOMA_ESTATE on such a context. */
+ * returns SOMA_ESTATE on such a context.  Every rank must use the same grid format: a shard does not fall
+ * back from the packed records on its own (an overflow shows as SOMA_EOVERFLOW after the next
+ * soma_shard_fields), and after SOMA_OPT_COUNT_BITS was changed -- on every rank -- the exchange array holds
+ * the rank's histogram again and wants the all-reduce and soma_shard_fields(ctx, 0) like after soma_init_shard. */
 int soma_init_shard(soma_ctx **out, const soma_chain_spec *chains, int n_specs, int N_ref, int n_types,
                     const float *box, const int *grid, float chiN, float kappaN, float A, uint64_t seed,
                     const float *host_xyz0, void *cuda_stream, const uint64_t *spec_first_bead,
