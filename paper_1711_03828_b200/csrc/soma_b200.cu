@@ -81,12 +81,12 @@ struct Spec {
     uint32_t log2N = 0;     // fused_ok only
     uint64_t chain_off = 0; // offset into orig[]
     uint32_t n_tiles = 0;   // full 128-bead tiles (fused_ok only)
-    // general architecture (bond list): device words nbr_off[N+1] | nbr[2 n_bonds] | members[N] at arch_off
+    // general architecture (bond list): the device words of Fig. 2 and the set members behind them at arch_off
     bool general = false;
     uint32_t n_bonds = 0;
     uint64_t arch_off = 0;
     std::vector<uint32_t> set_off;   // [n_sets + 1] offsets into members[]
-    uint32_t n_arch_words = 0;       // nbr_off | nbr | members | set_off | set_magic
+    uint32_t n_arch_words = 0;       // Fig. 2 words | members | set_off | set_magic
 };
 
 constexpr int kEventPool = 2048;
@@ -352,7 +352,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         if (s.n_beads == 0) continue;
         if (s.general) {        // bond-list architecture: the independent sets one after the other
             const uint32_t* arch = c->arch + s.arch_off;
-            const uint32_t *nbr_off = arch, *nbr = arch + (s.N + 1), *members = nbr + 2 * (size_t)s.n_bonds;
+            const uint32_t* members = arch + 1 + s.N + 2 * (size_t)s.n_bonds;
             // molecules staged in shared memory, every set in one launch (positions cross HBM once per sweep)
             const uint32_t group = std::max<uint32_t>(1u, 256u / s.N);   // ~256 beads per warp and pass (measured: 219 us at C3 against 232 with 512, 292 with 1024)
             const int warps = 8;
@@ -385,7 +385,7 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
                 const int threads = 256;
                 Timed t(c, SOMA_K_MOVE, 1);
                 soma::arch_move_kernel<kMove, kIncr, kRecord, kPack><<<(unsigned)((n_items + threads - 1) / threads), threads, 0, c->stream>>>(
-                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, nbr_off, nbr,
+                    P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, arch,
                     members + s.set_off[i_set], s.N, set_size, n_items, (uint32_t)s.gid0, c->orig + s.chain_off,
                     c->decisions, c->acc_slots);
             }
@@ -819,15 +819,26 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
                 set_of[j] = col;
                 n_sets = std::max(n_sets, col + 1);
             }
+            // the architecture as the 32-bit words of Fig. 2 (soma_kernels.cuh): N | per monomer
+            // (first bond word << 8 | type) | per bond (signed partner offset << 5 | bond type << 1 | last)
+            if (1 + (uint64_t)s.N + 2 * (uint64_t)s.n_bonds >= (1u << 24) || s.N >= (1u << 26)) {
+                delete c;
+                return fail(SOMA_EINVAL, "soma_init: spec %d: architecture too large for the 24-bit bond-list offsets of Fig. 2", a);
+            }
             s.arch_off = arch_host.size();
-            uint32_t run = 0;
-            for (uint32_t j = 0; j < s.N; ++j) { arch_host.push_back(run); run += (uint32_t)nb[j].size(); }
-            arch_host.push_back(run);
-            for (uint32_t j = 0; j < s.N; ++j) for (uint32_t k : nb[j]) arch_host.push_back(k);
+            arch_host.push_back(s.N);
+            uint32_t run = 1 + s.N;
+            for (uint32_t j = 0; j < s.N; ++j) {
+                arch_host.push_back(((nb[j].empty() ? 0u : run) << 8) | (s.n_chains ? chains[a].types[j] : 0u));
+                run += (uint32_t)nb[j].size();
+            }
+            for (uint32_t j = 0; j < s.N; ++j)
+                for (size_t q = 0; q < nb[j].size(); ++q)
+                    arch_host.push_back(((uint32_t)((int32_t)nb[j][q] - (int32_t)j) << 5) | (q + 1 == nb[j].size() ? 1u : 0u));
             s.set_off.assign(1, 0);
             for (uint32_t col = 0; col < n_sets; ++col) {
                 for (uint32_t j = 0; j < s.N; ++j) if (set_of[j] == col) arch_host.push_back(j);
-                s.set_off.push_back((uint32_t)(arch_host.size() - s.arch_off - (s.N + 1) - 2 * (size_t)s.n_bonds));
+                s.set_off.push_back((uint32_t)(arch_host.size() - s.arch_off - (1 + s.N) - 2 * (size_t)s.n_bonds));
             }
             // for the staged kernel: set_off[n_sets + 1] | set_magic[n_sets] (division by the set size as a multiply)
             for (uint32_t v : s.set_off) arch_host.push_back(v);

@@ -759,18 +759,50 @@ generic_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y,
 }
 
 // ------------------------------------------------------------------------------------------------
+// Molecular architecture, stored once per molecule type as the array of 32-bit words of Fig. 2:
+//   word 0                 N, the number of monomers
+//   words 1 .. N           per monomer: upper 3 bytes = index (in this array) of its first bond word, 0 if it has
+//                          no bond; lowest byte = its type
+//   then the bond words    upper 27 bits = signed offset from the monomer to its bonded partner, next 4 bits =
+//                          bond type (0: the harmonic spring of Eq. 2, the only one), lowest bit = 1 on the
+//                          monomer's last bond.  A monomer's partners come in ascending order (R25).
+// Behind it, what the set scheme needs (not part of Fig. 2):
+//   members[N] (set by set) | set_off[n_sets + 1] | set_magic[n_sets] (floor(2^32 / set size) + 1)
+// arch_bond_sum() walks the bond words of monomer j: s = sum over its partners of (r_j - r_partner) in list order
+// (the first term assigned, the others added, so that a linear chain given as bonds reproduces the chain kernels
+// bit for bit); returns the number of partners.  pos(k) gives the position of monomer k of the same molecule.
+// ------------------------------------------------------------------------------------------------
+template <typename PosOf>
+__device__ __forceinline__ uint32_t arch_bond_sum(const uint32_t* __restrict__ arch, uint32_t j, float px, float py, float pz,
+                                                  PosOf pos, float& sx, float& sy, float& sz)
+{
+    sx = sy = sz = 0.0f;
+    uint32_t at = arch[1u + j] >> 8, n = 0u;
+    if (at == 0u) return 0u;
+    uint32_t w;
+    do {
+        w = arch[at++];
+        const uint32_t k = j + (uint32_t)((int32_t)w >> 5);              // signed 27-bit offset
+        float qx, qy, qz;
+        pos(k, qx, qy, qz);
+        const float bx = px - qx, by = py - qy, bz = pz - qz;
+        if (n == 0u) { sx = bx; sy = by; sz = bz; } else { sx = sx + bx; sy = sy + by; sz = sz + bz; }
+        ++n;
+    } while (!(w & 1u));
+    return n;
+}
+
+// ------------------------------------------------------------------------------------------------
 // One independent set of a general molecular architecture (DESIGN.md
 // R25): one thread per member of set `i_set` of every molecule; the host launches the sets one after the
-// other.  The architecture is stored once per molecule type (the idea of Fig. 2) as
-// 32-bit words:  nbr_off[N + 1] | nbr[2 n_bonds] (ascending per monomer) | members[N] (set by set).
-// The bond sum s of Eq. 2 runs over the neighbour list in that order.
+// other.  arch: the architecture words above (global memory); members: the members of this set.
 // ------------------------------------------------------------------------------------------------
 template <int kMove, bool kIncr, bool kRecord, bool kPack>
 __global__ void __launch_bounds__(256)
 arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                  const float* __restrict__ omega, uint32_t* __restrict__ counts,
-                 const uint32_t* __restrict__ toff_tab, const uint32_t* __restrict__ nbr_off,
-                 const uint32_t* __restrict__ nbr, const uint32_t* __restrict__ members, uint32_t N,
+                 const uint32_t* __restrict__ toff_tab, const uint32_t* __restrict__ arch,
+                 const uint32_t* __restrict__ members, uint32_t N,
                  uint32_t set_size, uint64_t n_items, uint32_t gid0, const uint32_t* __restrict__ orig,
                  uint32_t* __restrict__ dec_words, unsigned long long* __restrict__ acc_slots)
 {
@@ -781,15 +813,12 @@ arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, fl
         const uint32_t j = members[(uint32_t)(t - mol * set_size)];      // monomer of this set member
         const uint64_t base = mol * N, i = base + j;
         float px = x[i], py = y[i], pz = z[i];
-        float sx = 0.0f, sy = 0.0f, sz = 0.0f;
-        const uint32_t a0 = nbr_off[j], a1 = nbr_off[j + 1u];
-        for (uint32_t a = a0; a < a1; ++a) {                              // other sets: not written in this launch
-            const uint64_t k = base + nbr[a];
-            const float bx = px - x[k], by = py - y[k], bz = pz - z[k];
-            if (a == a0) { sx = bx; sy = by; sz = bz; } else { sx = sx + bx; sy = sy + by; sz = sz + bz; }
-        }
+        float sx, sy, sz;
+        const uint32_t n_nb = arch_bond_sum(arch, j, px, py, pz,        // other sets: not written in this launch
+            [&](uint32_t k, float& qx, float& qy, float& qz) { qx = x[base + k]; qy = y[base + k]; qz = z[base + k]; },
+            sx, sy, sz);
         const uint32_t gid = gid0 + orig[mol] * N + j;
-        acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, sx, sy, sz, (float)(a1 - a0), toff_tab[j], gid);
+        acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, sx, sy, sz, (float)n_nb, toff_tab[j], gid);
         if (acc) { x[i] = px; y[i] = py; z[i] = pz; }
         if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
     }
@@ -804,8 +833,8 @@ arch_move_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, fl
 // its lanes, neighbours read from shared memory, __syncwarp between sets -- and writes the group back: every
 // position crosses HBM once per sweep, and the architecture (offsets, neighbour lists, set members: the
 // compressed-architecture array of PAPER.md:344-354 in plain 32-bit words) sits in shared memory too.
-//   arch        nbr_off[N + 1] | nbr[2 n_bonds] | members[N] | set_off[n_sets + 1] | set_magic[n_sets]
-//               (set_magic = floor(2^32 / set size) + 1: item / set size by one multiply, exact below 2^16)
+//   arch        the architecture words above with members | set_off | set_magic behind them
+//               (set_magic: item / set size by one multiply, exact below 2^16)
 //   group       molecules per warp and pass (group * N <= 65535)
 // Dynamic shared memory: arch words + toff[N], then warps * 3 * group * N floats.
 template <int kMove, bool kIncr, bool kRecord, bool kPack>
@@ -822,9 +851,7 @@ arch_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     for (uint32_t k = threadIdx.x; k < n_arch_words; k += blockDim.x) s_words[k] = arch[k];
     for (uint32_t k = threadIdx.x; k < N; k += blockDim.x) s_words[n_arch_words + k] = toff_tab[k];
     __syncthreads();
-    const uint32_t* nbr_off = s_words;
-    const uint32_t* nbr = nbr_off + (N + 1u);
-    const uint32_t* members = nbr + 2u * n_bonds;
+    const uint32_t* members = s_words + 1u + N + 2u * n_bonds;
     const uint32_t* set_off = members + N;
     const uint32_t* set_magic = set_off + (n_sets + 1u);
     const uint32_t* toff = s_words + n_arch_words;
@@ -851,15 +878,13 @@ arch_staged_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
                 const uint32_t j = members[first + (it - m * set_size)];
                 const uint32_t i = m * N + j;
                 float px = sx[i], py = sy[i], pz = sz[i];
-                float bsx = 0.0f, bsy = 0.0f, bsz = 0.0f;
-                const uint32_t a0 = nbr_off[j], a1 = nbr_off[j + 1u];
-                for (uint32_t a = a0; a < a1; ++a) {                          // other sets: not written during this set
-                    const uint32_t k = m * N + nbr[a];
-                    const float bx = px - sx[k], by = py - sy[k], bz = pz - sz[k];
-                    if (a == a0) { bsx = bx; bsy = by; bsz = bz; } else { bsx = bsx + bx; bsy = bsy + by; bsz = bsz + bz; }
-                }
+                float bsx, bsy, bsz;
+                const uint32_t mol0 = m * N;
+                const uint32_t n_nb = arch_bond_sum(s_words, j, px, py, pz,   // other sets: not written during this set
+                    [&](uint32_t k, float& qx, float& qy, float& qz) { qx = sx[mol0 + k]; qy = sy[mol0 + k]; qz = sz[mol0 + k]; },
+                    bsx, bsy, bsz);
                 const uint32_t gid = gid0 + orig[m0 + m] * N + j;
-                const bool acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, bsx, bsy, bsz, (float)(a1 - a0),
+                const bool acc = mc_move_s<kMove, kIncr, kPack>(P, omega, counts, px, py, pz, bsx, bsy, bsz, (float)n_nb,
                                                                 toff[j], gid);
                 if (acc) { sx[i] = px; sy[i] = py; sz[i] = pz; }
                 if (kRecord && acc) atomicOr(dec_words + (gid >> 5), 1u << (gid & 31u));
