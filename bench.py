@@ -68,11 +68,19 @@ class ClockSampler:
         try:
             import pynvml
             pynvml.nvmlInit()
-            # NVML enumerates the physical devices; honour CUDA_VISIBLE_DEVICES for a plain integer list
-            vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
-            ids = [int(v) for v in vis.split(",")] if vis and all(v.strip().isdigit() for v in vis.split(",")) else None
-            phys = ids[index] if ids and index < len(ids) else index
-            self.handle = pynvml.nvmlDeviceGetHandleByIndex(phys)
+            # NVML enumerates the physical devices, CUDA the visible ones: find this CUDA device by its UUID,
+            # else by its place in a plain integer CUDA_VISIBLE_DEVICES list
+            self.handle = None
+            try:
+                import torch
+                uuid = str(torch.cuda.get_device_properties(index).uuid)
+                self.handle = pynvml.nvmlDeviceGetHandleByUUID(uuid if uuid.startswith("GPU-") else "GPU-" + uuid)
+            except Exception:
+                self.handle = None
+            if self.handle is None:
+                vis = os.environ.get("CUDA_VISIBLE_DEVICES", "")
+                ids = [int(v) for v in vis.split(",")] if vis and all(v.strip().isdigit() for v in vis.split(",")) else None
+                self.handle = pynvml.nvmlDeviceGetHandleByIndex(ids[index] if ids and index < len(ids) else index)
             self.max_mhz = float(pynvml.nvmlDeviceGetMaxClockInfo(self.handle, pynvml.NVML_CLOCK_SM))
             self.nvml, self.source = pynvml, "nvml"
         except Exception:
