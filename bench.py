@@ -64,7 +64,7 @@ class ClockSampler:
 
     def __init__(self, index: int, period_s: float = 0.001):
         self.index, self.period, self.samples, self.stop, self.t = index, period_s, [], threading.Event(), None
-        self.nvml, self.handle, self.max_mhz, self.source = None, None, None, "nvidia-smi"
+        self.nvml, self.handle, self.max_mhz, self.source, self.t_from = None, None, None, "nvidia-smi", None
         try:
             import pynvml
             pynvml.nvmlInit()
@@ -102,7 +102,7 @@ class ClockSampler:
     def _run(self):
         while not self.stop.is_set():
             try:
-                self.samples.append(self._once())
+                self.samples.append(self._once() + [time.perf_counter()])
             except Exception:
                 if self.nvml is not None:      # NVML failed mid-run: fall back
                     self.nvml, self.source = None, "nvidia-smi"
@@ -116,11 +116,18 @@ class ClockSampler:
     def __exit__(self, *a):
         self.stop.set()
         self.t.join(timeout=6)
+        if self.t_from is not None:            # keep what was sampled while the timed region ran
+            inside = [s for s in self.samples if s[-1] >= self.t_from]
+            self.samples = inside or self.samples[-1:]
         if not self.samples:                   # a region shorter than one sample: take one now
             try:
-                self.samples.append(self._once())
+                self.samples.append(self._once() + [time.perf_counter()])
             except Exception:
                 pass
+
+    def mark(self):
+        """The timed region starts now: samples taken earlier (warm-up) are dropped at the end."""
+        self.t_from = time.perf_counter()
 
     def summary(self):
         if not self.samples:
@@ -339,7 +346,7 @@ def main():
     config = {"workload": f"{w.name}: {w.note}", "chains": w.n_chains, "beads": w.n_beads, "grid": list(w.grid),
               "box": list(w.box), "chiN": w.chiN, "kappaN": w.kappaN, "A": w.A, "seed": w.seed, "move": w.move,
               "parallelism": "replicas only" if world > 1 else "single GPU",
-              "timing": "W warm-up steps (the last five at most enqueued after the synchronisation, directly before the start "
+              "timing": "W warm-up steps (the last five at most enqueued after the synchronisation and ~10 ms of unrelated device work, directly before the start "
                         "event), K steps in one soma_step(K) call between two CUDA events, barrier + synchronize on both sides",
               "l2_policy": (f"inputs larger than L2 (positions {12 * w.n_beads / 1e6:.0f} MB > 126 MB L2); no explicit flush"
                             if 12 * w.n_beads > 126e6 else
@@ -421,14 +428,20 @@ def main():
     # all, which a 20-step region of 2 ms would carry as +3 %); the events are in stream order, so exactly the K
     # steps lie between them.
     pre_roll = min(5, args.warmup)
-    sim.step(args.warmup - pre_roll)
-    barrier()
-    l0 = sim.launch_count()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    with ClockSampler(local_rank) as clk:
-        time.sleep(0.003)                      # the sampling thread is running before the region starts
+    with ClockSampler(local_rank) as clk:      # the sampling thread is up before the GPU is left idle for the last time
+        sim.step(args.warmup - pre_roll)
+        barrier()
+        # ~10 ms of unrelated device work (a 256 MB buffer incremented 120 times) between the synchronisation and
+        # the pre-roll: the board is back at its working clocks and power state when the pre-roll starts (measured
+        # on a 20-step region: 101.9 -> 101.2 us per step); no step of the workload is added or skipped
+        spin = torch.empty(64 << 20, dtype=torch.float32, device="cuda")
+        for _ in range(120):
+            spin.add_(1.0)
+        del spin
         sim.step(pre_roll)
         l0 = sim.launch_count()
+        clk.mark()
         e0.record()
         sim.step(args.steps)                   # one soma_step(K) call: K x (move launch, field launch), no Python in between
         e1.record()
