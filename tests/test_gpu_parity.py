@@ -37,13 +37,16 @@ def field_close(w, got, want):
 
 
 def smc_positions_close(got, want):
-    """north_star: accepted positions within 1e-6 R_e.  The Smart-MC displacement d goes through logf / sincosf,
-    which are not bit-reproducible between glibc and the GPU, and what both sides store is fl32(r + d): with
-    |d_gpu - d_cpu| <= 1e-6 the two roundings of the sum (half an ulp each) can add up to one ulp of the stored
-    coordinate on top -- 1.9e-6 at |r| = 24 R_e (C5's box), 6e-8 at |r| < 1.  The bound below is therefore the
-    tightest statement about d that can be checked on stored fp32 positions (R17); comparing
-    displacements (after - before) instead of positions is the same comparison, the common start cancels."""
-    tol = POS_TOL_SMC + np.spacing(np.maximum(np.abs(got), np.abs(want)))
+    """north_star: accepted positions within 1e-6 R_e.  The Smart-MC displacement d goes through log / sin / cos,
+    which are not bit-reproducible between glibc and the GPU, and what both sides store is fl32(r + d).  With
+    |d_gpu - d_cpu| <= 1e-6 the two exact sums differ by at most 1e-6, each is rounded to a multiple of the ulp of
+    the stored coordinate, so the stored values differ by a whole number of ulps not above 1e-6 + 1 ulp: at most
+    ulp * floor(1e-6 / ulp + 1) -- exactly one ulp (the neighbouring float) wherever the ulp exceeds 1e-6 (|r| >= 8:
+    1.9e-6 at |r| = 24 R_e, C5's box), 1e-6 rounded up to the grid of floats below that.  This is the tightest
+    statement about d that stored fp32 positions allow (R17); comparing displacements (after - before)
+    instead of positions is the same comparison, the common start cancels."""
+    ulp = np.spacing(np.maximum(np.abs(got), np.abs(want))).astype(np.float64)
+    tol = ulp * np.floor(POS_TOL_SMC / ulp + 1.0)
     return bool(np.all(np.abs(got.astype(np.float64) - want.astype(np.float64)) <= tol))
 
 
