@@ -66,7 +66,8 @@ enum {
     SOMA_OPT_KERNEL = 5,           /* 0: auto (default); 1: force the one-thread-per-monomer kernels on global */
                                    /* memory (two launches per sweep for linear chains, one per independent   */
                                    /* set for bond-list architectures, no shared-memory staging);              */
-                                   /* 2: chain-resident fused kernel (error if an architecture cannot use it) */
+                                   /* 2: chain-resident fused kernel (error if an architecture cannot use it:  */
+                                   /* it takes linear chains whose length is a multiple of 4 and at most 128)  */
     SOMA_OPT_DENSITY = 6,          /* 0: incremental count update fused into the move kernel (default),       */
                                    /* 1: clear + full histogram kernel after every sweep                      */
     SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */

@@ -77,8 +77,9 @@ struct Spec {
     uint64_t gid0 = 0;      // global index of the first bead (unpadded, the API's bead index)
     uint64_t off = 0;       // offset of the segment in the padded device arrays
     uint32_t toff_off = 0;  // offset into the toff table
-    bool fused_ok = false;  // N in {4, ..., 128}, N | 128
-    uint32_t log2N = 0;     // fused_ok only
+    bool fused_ok = false;  // 4 | N, N <= 128
+    bool any_n = false;     // fused_ok and N does not divide 128: floor(128 / N) chains per tile, idle lanes (kAnyN)
+    uint32_t log2N = 0;     // fused_ok: log2 N, or (any_n) the chains per tile
     uint64_t chain_off = 0; // offset into orig[]
     uint32_t n_tiles = 0;   // full 128-bead tiles (fused_ok only)
     // general architecture (bond list): the device words of Fig. 2 and the set members behind them at arch_off
@@ -310,10 +311,10 @@ cudaError_t launch_pdl(bool pdl, void (*kernel)(KArgs...), unsigned blocks, unsi
     return cudaLaunchKernelEx(&cfg, kernel, KArgs(args)...);
 }
 
-template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack>
+template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack, bool kAnyN>
 int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
-    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder, kPack>;
+    auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder, kPack, kAnyN>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
     constexpr size_t kOrderSmemMax = 160 * 1024;       // shared memory for the order bits of a block's chains
     static int resident[kMaxDevices] = {};             // blocks per SM of this instantiation, asked once per device
@@ -331,7 +332,7 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     // their order bit); more (not all resident) blocks if that does not fit into shared memory
     size_t order_smem = 0;
     if (kOrder) {
-        const size_t chains_per_tile = soma::kTile / s.N;
+        const size_t chains_per_tile = soma::kTile / s.N;      // floor: also for kAnyN
         for (int waves = 1;; ++waves) {
             order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile * 4 + 16;
             if (order_smem <= kOrderSmemMax) break;
@@ -340,8 +341,9 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
     }
     Timed t(c, SOMA_K_MOVE, 1);
     CU(launch_pdl(c->pdl != 0, kernel, (unsigned)blocks, (unsigned)threads, order_smem, c->stream,
-                  P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off, s.N - 1u,
-                  s.n_tiles, (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions, c->acc_slots));
+                  P, c->x + s.off, c->y + s.off, c->z + s.off, c->omega, count_target(c), c->toff + s.toff_off,
+                  kAnyN ? s.N : s.N - 1u, s.n_tiles, (uint32_t)s.gid0, c->orig + s.chain_off, s.log2N, c->decisions,
+                  c->acc_slots));
     return SOMA_OK;
 }
 
@@ -431,10 +433,13 @@ int launch_moves_t(soma_ctx* c, const soma::MoveP& P)
         const uint32_t* toff = c->toff + s.toff_off;
         uint64_t done = 0;   // beads of this architecture handled by the fused kernel
         if (spec_uses_fused(c, s) && s.n_tiles > 0) {
-            int rc = (kMove == 1 && c->set_order == 1) ? launch_fused<kMove, kIncr, kRecord, kMove == 1, kPack>(c, P, s)
-                                                       : launch_fused<kMove, kIncr, kRecord, false, kPack>(c, P, s);
+            const bool order = kMove == 1 && c->set_order == 1;
+            int rc = s.any_n ? (order ? launch_fused<kMove, kIncr, kRecord, kMove == 1, kPack, true>(c, P, s)
+                                      : launch_fused<kMove, kIncr, kRecord, false, kPack, true>(c, P, s))
+                             : (order ? launch_fused<kMove, kIncr, kRecord, kMove == 1, kPack, false>(c, P, s)
+                                      : launch_fused<kMove, kIncr, kRecord, false, kPack, false>(c, P, s));
             if (rc) return rc;
-            done = (uint64_t)s.n_tiles * soma::kTile;
+            done = s.any_n ? (uint64_t)s.n_tiles * s.log2N * s.N : (uint64_t)s.n_tiles * soma::kTile;
         }
         if (done < s.n_beads) {   // whole chains the fused kernel does not cover (all of them, or a ragged tail)
             const uint64_t n_chains = (s.n_beads - done) / s.N;
@@ -846,8 +851,12 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
                 arch_host.push_back((uint32_t)((1ull << 32) / (s.set_off[col + 1] - s.set_off[col])) + 1u);
             s.n_arch_words = (uint32_t)(arch_host.size() - s.arch_off);
         }
-        s.fused_ok = !s.general && s.N >= 4 && s.N <= 128 && (128 % s.N) == 0;
-        if (s.fused_ok) {
+        s.fused_ok = !s.general && s.N >= 4 && s.N <= 128 && (s.N % 4) == 0;
+        s.any_n = s.fused_ok && (128 % s.N) != 0;
+        if (s.any_n) {
+            s.log2N = 128 / s.N;                                   // chains per tile
+            s.n_tiles = (uint32_t)(s.n_chains / s.log2N);
+        } else if (s.fused_ok) {
             while ((1u << s.log2N) < s.N) ++s.log2N;
             s.n_tiles = (uint32_t)(s.n_chains * s.N / soma::kTile);
         }

@@ -460,7 +460,10 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 // kOrder: dynamic shared memory = four bytes per chain of the block's tile range (the host keeps the ranges
 // short enough); the block draws the order bit of all its chains before it waits for its predecessor.
 // ------------------------------------------------------------------------------------------------
-template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack>
+// kAnyN: chain lengths that are a multiple of 4 up to 128 but do not divide 128 (12, 20, 24, 48, 100, ...): a tile
+// holds floor(128 / N) whole chains, the lanes beyond them idle (they load harmlessly, decide nothing and
+// store nothing); n_mask then carries N and log2N the chains per tile.
+template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack, bool kAnyN = false>
 __global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
@@ -473,9 +476,14 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     const uint32_t wib = threadIdx.x >> 5;
     constexpr uint32_t kWarps = kFusedThreads / 32;
     pdl_trigger();
-    const uint32_t j0 = (4u * lane) & n_mask;                 // monomer index of slot 0
+    const uint32_t len = n_mask, cpt = log2N;                 // kAnyN: chain length, chains per tile
+    const uint32_t cit_raw = kAnyN ? lane / (len >> 2) : 0u;  // kAnyN: this lane's chain in its tile
+    const bool active = !kAnyN || cit_raw < cpt;
+    const uint32_t cit = kAnyN ? min(cit_raw, cpt - 1u) : 0u;
+    const uint32_t tile_beads = kAnyN ? cpt * len : kTile;
+    const uint32_t j0 = kAnyN ? 4u * lane - cit_raw * len : (4u * lane) & n_mask;   // monomer index of slot 0
     const bool has_l0 = j0 != 0u;                             // slot 0 has a left neighbour
-    const bool has_r3 = ((j0 + 4u) & n_mask) != 0u;           // slot 3 has a right neighbour
+    const bool has_r3 = kAnyN ? j0 + 4u != len : ((j0 + 4u) & n_mask) != 0u;   // slot 3 has a right neighbour
     const uint4 toff = *reinterpret_cast<const uint4*>(toff_tab + j0);
     const uint4 tk = make_uint4(toff.x + P.g.k_rec, toff.y + P.g.k_rec, toff.z + P.g.k_rec, toff.w + P.g.k_rec);
     const float mf0 = has_l0 ? 2.0f : 1.0f, mf3 = has_r3 ? 2.0f : 1.0f;
@@ -494,9 +502,12 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     // kOrder: the chains of this block's tile range, regrouped (entry = index of the chain's first bead in this
     // architecture's arrays, bit 0 = odd set first)
     extern __shared__ __align__(16) uint32_t s_perm[];
-    const uint32_t slot_begin = (t_begin * kTile) >> log2N;
-    const uint32_t n_slots = ((t_end - t_begin) * kTile) >> log2N;
-    const uint32_t cpt_shift = 7u - log2N, ci = (4u * lane) >> log2N;   // chains per tile = 128 / N; this lane's chain in its tile
+    const uint32_t slot_begin = kAnyN ? t_begin * cpt : (t_begin * kTile) >> log2N;
+    const uint32_t n_slots = kAnyN ? (t_end - t_begin) * cpt : ((t_end - t_begin) * kTile) >> log2N;
+    const uint32_t cpt_shift = 7u - log2N, ci = kAnyN ? cit : (4u * lane) >> log2N;   // chains per tile = 128 / N; this lane's chain in its tile
+    // list entry of the tile `t` for this lane; bead offset of a chain slot; chain slot of a bead offset
+    auto entry_at = [&](uint32_t t) { return kAnyN ? (t - t_begin) * cpt + ci : ((t - t_begin) << cpt_shift) + ci; };
+    auto beads_of = [&](uint32_t slot) { return kAnyN ? slot * len : slot << log2N; };
     if (kOrder) {
         // "Generate random permutation of the sets" (Code 2) for every chain this block will move:
         // needs nothing of the predecessor kernel (orig[] only changes in a re-sort), so it runs before the wait.
@@ -516,16 +527,16 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             for (uint32_t k = 0; k < 4u; ++k) {
                 const uint32_t lo = lo0 + k * kWarps * 64u, sa = lo + lane, sb = sa + 32u;
                 if (lo >= n_slots) break;
-                const uint32_t ba = sa < n_slots ? first_set_bit(gid0 + (first[2 * k] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
-                const uint32_t bb = sb < n_slots ? first_set_bit(gid0 + (first[2 * k + 1] << log2N), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
+                const uint32_t ba = sa < n_slots ? first_set_bit(gid0 + beads_of(first[2 * k]), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
+                const uint32_t bb = sb < n_slots ? first_set_bit(gid0 + beads_of(first[2 * k + 1]), P.sweep_lo, P.sweep_hi, P.rk[0][0], P.rk[0][1]) : 0u;
                 const uint32_t ones_a = __ballot_sync(kFull, ba != 0u), ones_b = __ballot_sync(kFull, bb != 0u);
                 const uint32_t zeros_a = __ballot_sync(kFull, sa < n_slots) & ~ones_a, zeros_b = __ballot_sync(kFull, sb < n_slots) & ~ones_b;
                 const uint32_t below = (1u << lane) - 1u;
                 const uint32_t n_zero = __popc(zeros_a) + __popc(zeros_b);
                 const uint32_t pos_a = ba ? n_zero + __popc(ones_a & below) : __popc(zeros_a & below);
                 const uint32_t pos_b = bb ? n_zero + __popc(ones_a) + __popc(ones_b & below) : __popc(zeros_a) + __popc(zeros_b & below);
-                if (sa < n_slots) s_perm[lo + pos_a] = ((slot_begin + sa) << log2N) | ba;   // N >= 4: the low bits are free
-                if (sb < n_slots) s_perm[lo + pos_b] = ((slot_begin + sb) << log2N) | bb;
+                if (sa < n_slots) s_perm[lo + pos_a] = beads_of(slot_begin + sa) | ba;   // 4 | N: the low bits are free
+                if (sb < n_slots) s_perm[lo + pos_b] = beads_of(slot_begin + sb) | bb;
             }
         }
     }
@@ -536,13 +547,13 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
     uint32_t C = 0u;                                          // the caller's index of this lane's chain
     uint32_t E = 0u;                                          // kOrder: this lane's entry of the list
     if (tile < t_end) {
-        if (kOrder) E = s_perm[((tile - t_begin) << cpt_shift) + ci];
-        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * kTile + 4u * lane;
-        C = orig[i0 >> log2N];
+        if (kOrder) E = s_perm[entry_at(tile)];
+        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * tile_beads + 4u * lane;
+        C = orig[kAnyN ? (kOrder ? (E >> 2) / (len >> 2) : tile * cpt + cit) : i0 >> log2N];
     }
     while (tile < t_end) {
-        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * kTile + 4u * lane;
-        const uint32_t gid = gid0 + (C << log2N) + j0;
+        const uint32_t i0 = kOrder ? (E & ~1u) + j0 : tile * tile_beads + 4u * lane;
+        const uint32_t gid = gid0 + beads_of(C) + j0;
         // the tile after the next one.  The counter is addressed through `warp & zero` (zero: a kernel argument
         // bit that is never set): with a provably uniform address ptxas wraps the atomic of this single lane
         // into its warp-aggregation sequence (vote, popc, leader election: a dozen instructions per tile)
@@ -551,19 +562,21 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
 
         // 1. the chain index of the next tile of this warp (clamped to the last tile: a harmless re-read)
         uint32_t En = 0u;
-        if (kOrder) En = s_perm[((min(tile_n, t_end - 1u) - t_begin) << cpt_shift) + ci];
-        const uint32_t i0n = kOrder ? (En & ~1u) + j0 : min(tile_n, t_end - 1u) * kTile + 4u * lane;
+        if (kOrder) En = s_perm[entry_at(min(tile_n, t_end - 1u))];
+        const uint32_t i0n = kOrder ? (En & ~1u) + j0 : min(tile_n, t_end - 1u) * tile_beads + 4u * lane;
         // this tile's positions: asked for now, first needed after the four Philox draws below (~150
         // instructions of this warp and as many of each of its four neighbours on the scheduler), which covers
         // the latency without holding a second tile in registers
         X = ld_stream(x + i0);
         Y = ld_stream(y + i0);
         Z = ld_stream(z + i0);
-        const uint32_t Cn = orig[i0n >> log2N];
+        const uint32_t Cn = orig[kAnyN ? (kOrder ? (En >> 2) / (len >> 2) : min(tile_n, t_end - 1u) * cpt + cit) : i0n >> log2N];
 
         // 2. random numbers of the four moves
-        const Draw q0 = draw_move<kMove>(P, gid), q1 = draw_move<kMove>(P, gid + 1u),
-                   q2 = draw_move<kMove>(P, gid + 2u), q3 = draw_move<kMove>(P, gid + 3u);
+        Draw q0 = draw_move<kMove>(P, gid), q1 = draw_move<kMove>(P, gid + 1u),
+             q2 = draw_move<kMove>(P, gid + 2u), q3 = draw_move<kMove>(P, gid + 3u);
+        if (kAnyN && !active)                                 // an idle lane compares with u = +inf, which accepts nothing
+            q0.u = q1.u = q2.u = q3.u = __int_as_float(0x7F800000);
 
         bool a0, a1, a2, a3;
         if (kMove == 1) {
@@ -695,9 +708,11 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
             if (kIncr) { count_follow<kPack>(counts, a1, o1, n1, tk.y); count_follow<kPack>(counts, a3, o3, n3, tk.w); }
         }
 
-        st_stream(x + i0, X);
-        st_stream(y + i0, Y);
-        st_stream(z + i0, Z);
+        if (active) {
+            st_stream(x + i0, X);
+            st_stream(y + i0, Y);
+            st_stream(z + i0, Z);
+        }
 
         const uint32_t nib = (a0 ? 1u : 0u) | (a1 ? 2u : 0u) | (a2 ? 4u : 0u) | (a3 ? 8u : 0u);
         n_acc += __popc(nib);

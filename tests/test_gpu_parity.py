@@ -158,6 +158,30 @@ def test_ragged_last_tile_of_the_fused_kernel():
     lockstep(w, 5, kernel=P.KERNEL_FUSED)
 
 
+@pytest.mark.parametrize("variant", ["local", "random-order", "smart-mc", "packed", "generic"])
+def test_chain_lengths_that_do_not_divide_the_tile(variant):
+    """Chain lengths that are a multiple of 4 but do not divide 128 run in the fused kernel with floor(128 / N)
+    chains per tile and idle lanes: 100 (one chain, 25 lanes), 48 (two chains), 20 (six chains, 30 lanes), 12 (ten),
+    with ragged remainders (chains that do not fill a tile go to the generic kernel)."""
+    w = workloads.Workload("anyN", ((37, workloads.diblock(100, 40)), (131, workloads.diblock(20, 7)),
+                                    (50, workloads.homopolymer(48, 1)), (63, workloads.diblock(12, 6)),
+                                    (40, workloads.diblock(32, 16))),
+                           32, 2, (4.0, 4.0, 4.0), (16, 16, 16), 20.0, 50.0, 0.1, 19,
+                           move="smc" if variant == "smart-mc" else "local", smc_step=0.05 / 31)
+    lockstep(w, 4, set_order=1 if variant == "random-order" else 0, count_bits=16 if variant == "packed" else 0,
+             kernel=P.KERNEL_GENERIC if variant == "generic" else P.KERNEL_AUTO)
+    if variant == "local":                               # and the fused kernel really took them
+        xyz0 = np.stack(workloads.gaussian_walks(w))
+        a, b_ = P.from_workload(w, xyz0=xyz0), P.from_workload(w, xyz0=xyz0)
+        b_.set_option(P.OPT_KERNEL, P.KERNEL_GENERIC)
+        n0, m0 = a.launch_count(), b_.launch_count()
+        a.step(3); b_.step(3)
+        assert np.array_equal(a.positions(), b_.positions()) and a.stats() == b_.stats()
+        assert a.launch_count() - n0 < b_.launch_count() - m0
+        a.set_option(P.OPT_KERNEL, P.KERNEL_FUSED)       # every architecture can use it
+        a.destroy(); b_.destroy()
+
+
 def test_unwrapped_coordinates_far_from_the_origin():
     w = workloads.c1()
     x, y, z = workloads.gaussian_walks(w)
