@@ -264,8 +264,11 @@ def all_configs(P, torch):
     c3_bonds = replace(c3, name="C3bonds", bonds=(tuple((j, j + 1) for j in range(31)),))
     star = tuple((0 if k == 0 else 1 + a * 10 + k - 1, 1 + a * 10 + k) for a in range(3) for k in range(10))
     stars = replace(c3, name="stars", specs=((528516, (0,) + (0,) * 15 + (1,) * 15),), bonds=(star,))
+    n100 = replace(c3, name="N100", specs=((163840, workloads.diblock(100, 50)),), N_ref=100)
+    n48 = replace(c3, name="N48", specs=((341333, workloads.diblock(48, 24)),), N_ref=48)
     cases = [("C1", workloads.c1(), {}), ("C2 kappaN=50", workloads.c2(kappaN=50.0), {}), ("C3", c3, {}),
              ("C3 random set order", c3, {"order": 1}), ("C3 molecule-parallel scheme (Code 1)", c3, {"scheme": 1}),
+             ("diblock melt N = 100 (25 of 32 lanes)", n100, {}), ("diblock melt N = 48 (24 of 32 lanes)", n48, {}),
              ("C3 chains as bond lists", c3_bonds, {}), ("3-arm star melt, 16.4M beads", stars, {}),
              ("C5 a_s=0.05 (literal)", workloads.c5(), {}),
              ("C5 a_s=0.05 b0^2", workloads.c5(smc_step=0.05 / 63), {}), ("C4", workloads.c4(), {})]
