@@ -128,6 +128,15 @@ typedef struct {
     const uint32_t *bonds;   /* host, [2 * n_bonds] monomer pairs (i, j), i != j, each pair once; or NULL */
 } soma_chain_spec;
 
+/* The architecture array the library keeps for a molecule type given by a bond list: the 32-bit words of Fig. 2
+ * -- word 0: N; words 1..N, per monomer: (index of its first bond word << 8) | type, index 0 if it
+ * has no bond; then per bond, in ascending order of the partner: (signed offset to the partner << 5) | (bond type
+ * << 1) | 1 on the monomer's last bond -- followed by the independent sets (greedy first fit):
+ * members[N] set by set | set_off[n_sets + 1] | floor(2^32 / set size) + 1 per set.  Host only (no device needed):
+ * for inspection and tests.  words_out may be NULL to ask for the length; *n_sets (nullable) gets the number of sets. */
+int soma_architecture_words(const soma_chain_spec *spec, uint32_t *words_out, uint64_t capacity, uint64_t *n_words,
+                            uint32_t *n_sets);
+
 /* Create a system and run stage 1 (densities, fields) on its initial configuration.
  *   chains/n_specs  architectures, stored one after the other in the bead arrays (n_specs >= 1)
  *   N_ref           reference chain length N of PAPER.md:157: k_0 = 3 (N_ref-1)/R_e0^2 (Eq. 2 with

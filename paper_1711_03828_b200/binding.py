@@ -30,7 +30,7 @@ SYMBOLS = (
     "soma_set_external", "soma_set_option", "soma_stats", "soma_decisions", "soma_kernel_times", "soma_launch_count",
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
     "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields", "soma_shard_exchange",
-    "soma_shard_exchange_copy", "soma_shard_peer_handle", "soma_shard_set_peers",
+    "soma_shard_exchange_copy", "soma_shard_peer_handle", "soma_shard_set_peers", "soma_architecture_words",
 )
 
 
@@ -63,6 +63,7 @@ def load() -> C.CDLL:
     L.soma_shard_fields.argtypes = [vp, i32]
     L.soma_shard_exchange.argtypes = [vp, C.POINTER(vp), C.POINTER(u64)]
     L.soma_shard_exchange_copy.argtypes = [vp, vp, i32]
+    L.soma_architecture_words.argtypes = [C.POINTER(_ChainSpec), vp, u64, C.POINTER(u64), C.POINTER(C.c_uint32)]
     L.soma_shard_peer_handle.argtypes = [vp, vp]
     L.soma_shard_set_peers.argtypes = [vp, i32, i32, C.POINTER(vp), vp]
     L.soma_step.argtypes = [vp, i32]
@@ -104,6 +105,19 @@ def _ptr(buf) -> Tuple[int, bool]:
     import torch  # torch is plumbing here: device memory and streams
     assert isinstance(buf, torch.Tensor) and buf.is_contiguous()
     return buf.data_ptr(), buf.is_cuda
+
+
+def architecture_words(types: Sequence[int], bonds: Sequence[Tuple[int, int]]) -> Tuple[np.ndarray, int]:
+    """(the Fig. 2 architecture array of a molecule type given by its bond list, number of independent sets): host only."""
+    L = load()
+    t = np.ascontiguousarray(types, np.uint8)
+    b = np.ascontiguousarray(bonds, np.uint32).reshape(-1, 2)
+    spec = _ChainSpec(1, len(t), t.ctypes.data_as(C.POINTER(C.c_uint8)), len(b), b.ctypes.data_as(C.POINTER(C.c_uint32)))
+    n, n_sets = C.c_uint64(), C.c_uint32()
+    _check(L.soma_architecture_words(C.byref(spec), None, 0, C.byref(n), C.byref(n_sets)))
+    out = np.empty(n.value, np.uint32)
+    _check(L.soma_architecture_words(C.byref(spec), C.c_void_p(out.ctypes.data), n.value, C.byref(n), C.byref(n_sets)))
+    return out, int(n_sets.value)
 
 
 class Soma:

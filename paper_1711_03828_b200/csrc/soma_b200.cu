@@ -279,6 +279,63 @@ struct Timed {
     }
 };
 
+// ---- architecture of a molecule type given by its bond list ----------------------------------------
+// Appends to `words` the array of Fig. 2 (layout in soma_kernels.cuh): N | per monomer (index of
+// its first bond word << 8 | type) | per bond (signed partner offset << 5 | bond type << 1 | last-bond flag), and
+// behind it the independent sets (greedy first fit in monomer order, R25): members[N] (set by set) |
+// set_off[n_sets + 1] | set_magic[n_sets].  Indices are relative to the first word appended.  Host only.
+int build_architecture(const soma_chain_spec& spec, int a, std::vector<uint32_t>& words, std::vector<uint32_t>& set_off)
+{
+    const uint32_t N = spec.n_beads, n_bonds = spec.n_bonds;
+    if (!spec.bonds) return fail(SOMA_EINVAL, "soma_init: spec %d: n_bonds > 0 but bonds is NULL", a);
+    // neighbour lists in ascending order
+    std::vector<std::vector<uint32_t>> nb(N);
+    for (uint32_t b = 0; b < n_bonds; ++b) {
+        const uint32_t i = spec.bonds[2 * b], j = spec.bonds[2 * b + 1];
+        if (i >= N || j >= N || i == j)
+            return fail(SOMA_EINVAL, "soma_init: spec %d bond %u (%u, %u): need i != j, both < n_beads", a, b, i, j);
+        nb[i].push_back(j);
+        nb[j].push_back(i);
+    }
+    std::vector<uint32_t> set_of(N, 0);
+    uint32_t n_sets = 0;
+    for (uint32_t j = 0; j < N; ++j) {
+        std::sort(nb[j].begin(), nb[j].end());
+        if (std::adjacent_find(nb[j].begin(), nb[j].end()) != nb[j].end())
+            return fail(SOMA_EINVAL, "soma_init: spec %d: a bond of monomer %u is listed twice", a, j);
+        uint32_t col = 0;
+        for (bool clash = true; clash; ) {
+            clash = false;
+            for (uint32_t k : nb[j]) if (k < j && set_of[k] == col) clash = true;
+            if (clash) ++col;
+        }
+        set_of[j] = col;
+        n_sets = std::max(n_sets, col + 1);
+    }
+    if (1 + (uint64_t)N + 2 * (uint64_t)n_bonds >= (1u << 24) || N >= (1u << 26))
+        return fail(SOMA_EINVAL, "soma_init: spec %d: architecture too large for the 24-bit bond-list offsets of Fig. 2", a);
+    const size_t first = words.size();
+    words.push_back(N);
+    uint32_t run = 1 + N;
+    for (uint32_t j = 0; j < N; ++j) {
+        words.push_back(((nb[j].empty() ? 0u : run) << 8) | (spec.types ? spec.types[j] : 0u));
+        run += (uint32_t)nb[j].size();
+    }
+    for (uint32_t j = 0; j < N; ++j)
+        for (size_t q = 0; q < nb[j].size(); ++q)
+            words.push_back(((uint32_t)((int32_t)nb[j][q] - (int32_t)j) << 5) | (q + 1 == nb[j].size() ? 1u : 0u));
+    set_off.assign(1, 0);
+    for (uint32_t col = 0; col < n_sets; ++col) {
+        for (uint32_t j = 0; j < N; ++j) if (set_of[j] == col) words.push_back(j);
+        set_off.push_back((uint32_t)(words.size() - first - (1 + N) - 2 * (size_t)n_bonds));
+    }
+    // for the staged kernel: division by the set size as a multiply
+    for (uint32_t v : set_off) words.push_back(v);
+    for (uint32_t col = 0; col < n_sets; ++col)
+        words.push_back((uint32_t)((1ull << 32) / (set_off[col + 1] - set_off[col])) + 1u);
+    return SOMA_OK;
+}
+
 // ---- launches -----------------------------------------------------------------------------------
 // where the move and histogram kernels count: a shard counts its contribution into the exchange array
 inline uint32_t* count_target(const soma_ctx* c) { return c->sharded ? c->exchange : c->counts; }
@@ -705,7 +762,25 @@ int copy_soa(soma_ctx* c, float* dst_user, const float* src_user, bool to_user, 
 extern "C" {
 
 const char* soma_last_error(void) { return g_err.c_str(); }
-const char* soma_version(void) { return "soma-b200 0.1 (sm_100a)"; }
+const char* soma_version(void) { return "soma-b200 0.2 (sm_100a)"; }
+
+int soma_architecture_words(const soma_chain_spec* spec, uint32_t* words_out, uint64_t capacity, uint64_t* n_words,
+                            uint32_t* n_sets)
+{
+    if (!spec || !n_words) return fail(SOMA_EINVAL, "soma_architecture_words: NULL argument");
+    if (spec->n_beads < 1 || spec->n_bonds < 1)
+        return fail(SOMA_EINVAL, "soma_architecture_words: need n_beads >= 1 and a bond list (a linear chain keeps no array)");
+    std::vector<uint32_t> words, set_off;
+    int rc = build_architecture(*spec, 0, words, set_off);
+    if (rc) return rc;
+    *n_words = words.size();
+    if (n_sets) *n_sets = (uint32_t)(set_off.size() - 1);
+    if (words_out) {
+        if (capacity < words.size()) return fail(SOMA_EINVAL, "soma_architecture_words: %zu words needed, room for %llu", words.size(), (unsigned long long)capacity);
+        std::memcpy(words_out, words.data(), sizeof(uint32_t) * words.size());
+    }
+    return SOMA_OK;
+}
 
 void soma_destroy(soma_ctx* c)
 {
@@ -795,60 +870,9 @@ static int init_impl(soma_ctx** out, const soma_chain_spec* chains, int n_specs,
         s.n_bonds = chains[a].n_bonds;
         s.general = s.n_bonds > 0;
         if (s.general) {
-            if (!chains[a].bonds) { delete c; return fail(SOMA_EINVAL, "soma_init: spec %d: n_bonds > 0 but bonds is NULL", a); }
-            // neighbour lists in ascending order, greedy first-fit independent sets (R25)
-            std::vector<std::vector<uint32_t>> nb(s.N);
-            for (uint32_t b = 0; b < s.n_bonds; ++b) {
-                const uint32_t i = chains[a].bonds[2 * b], j = chains[a].bonds[2 * b + 1];
-                if (i >= s.N || j >= s.N || i == j) {
-                    delete c;
-                    return fail(SOMA_EINVAL, "soma_init: spec %d bond %u (%u, %u): need i != j, both < n_beads", a, b, i, j);
-                }
-                nb[i].push_back(j);
-                nb[j].push_back(i);
-            }
-            std::vector<uint32_t> set_of(s.N, 0);
-            uint32_t n_sets = 0;
-            for (uint32_t j = 0; j < s.N; ++j) {
-                std::sort(nb[j].begin(), nb[j].end());
-                if (std::adjacent_find(nb[j].begin(), nb[j].end()) != nb[j].end()) {
-                    delete c;
-                    return fail(SOMA_EINVAL, "soma_init: spec %d: a bond of monomer %u is listed twice", a, j);
-                }
-                uint32_t col = 0;
-                for (bool clash = true; clash; ) {
-                    clash = false;
-                    for (uint32_t k : nb[j]) if (k < j && set_of[k] == col) clash = true;
-                    if (clash) ++col;
-                }
-                set_of[j] = col;
-                n_sets = std::max(n_sets, col + 1);
-            }
-            // the architecture as the 32-bit words of Fig. 2 (soma_kernels.cuh): N | per monomer
-            // (first bond word << 8 | type) | per bond (signed partner offset << 5 | bond type << 1 | last)
-            if (1 + (uint64_t)s.N + 2 * (uint64_t)s.n_bonds >= (1u << 24) || s.N >= (1u << 26)) {
-                delete c;
-                return fail(SOMA_EINVAL, "soma_init: spec %d: architecture too large for the 24-bit bond-list offsets of Fig. 2", a);
-            }
             s.arch_off = arch_host.size();
-            arch_host.push_back(s.N);
-            uint32_t run = 1 + s.N;
-            for (uint32_t j = 0; j < s.N; ++j) {
-                arch_host.push_back(((nb[j].empty() ? 0u : run) << 8) | (s.n_chains ? chains[a].types[j] : 0u));
-                run += (uint32_t)nb[j].size();
-            }
-            for (uint32_t j = 0; j < s.N; ++j)
-                for (size_t q = 0; q < nb[j].size(); ++q)
-                    arch_host.push_back(((uint32_t)((int32_t)nb[j][q] - (int32_t)j) << 5) | (q + 1 == nb[j].size() ? 1u : 0u));
-            s.set_off.assign(1, 0);
-            for (uint32_t col = 0; col < n_sets; ++col) {
-                for (uint32_t j = 0; j < s.N; ++j) if (set_of[j] == col) arch_host.push_back(j);
-                s.set_off.push_back((uint32_t)(arch_host.size() - s.arch_off - (1 + s.N) - 2 * (size_t)s.n_bonds));
-            }
-            // for the staged kernel: set_off[n_sets + 1] | set_magic[n_sets] (division by the set size as a multiply)
-            for (uint32_t v : s.set_off) arch_host.push_back(v);
-            for (uint32_t col = 0; col < n_sets; ++col)
-                arch_host.push_back((uint32_t)((1ull << 32) / (s.set_off[col + 1] - s.set_off[col])) + 1u);
+            int rc_arch = build_architecture(chains[a], a, arch_host, s.set_off);
+            if (rc_arch) { delete c; return rc_arch; }
             s.n_arch_words = (uint32_t)(arch_host.size() - s.arch_off);
         }
         s.fused_ok = !s.general && s.N >= 4 && s.N <= 128 && (s.N % 4) == 0;
