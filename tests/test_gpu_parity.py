@@ -299,6 +299,34 @@ def test_packed_occupation_numbers_overflow_is_detected():
     sim.destroy(); big.destroy()
 
 
+def test_auto_grid_format_falls_back_to_planes_when_a_cell_is_too_dense():
+    """A grid whose planes would take more than 48 MB gets the packed records by default; if the configuration
+    handed in puts more than 65535 beads of one type into a cell, soma_init / soma_set_positions recount with
+    32-bit planes on their own, and the results are the oracle's either way."""
+    n = 70000
+    w = workloads.Workload("big-grid", ((n, (0,)), (1000, (1, 1, 0, 1))), 4, 2, (16.0, 16.0, 8.0), (200, 200, 100), 5.0, 10.0, 0.05, 3)
+    assert 16 * w.n_cells > 48 << 20
+    rng = np.random.default_rng(4)
+    spread = (np.asarray(w.box)[:, None] * rng.random((3, w.n_beads))).astype(np.float32)
+    dense = spread.copy()
+    dense[:, :n] = (0.01 + 0.05 * rng.random((3, n))).astype(np.float32)          # all A singles in cell (0, 0, 0)
+    orc = oracle_system(w)
+    for xyz in (spread, dense):
+        sim = P.from_workload(w, xyz0=xyz)
+        want = orc.histogram(*[xyz[a].copy() for a in range(3)])
+        om, cnt = sim.fields()
+        assert np.array_equal(cnt, want) and field_close(w, om, orc.fields(want)) <= FIELD_RTOL
+        sim.step(2)
+        pos = sim.positions()
+        assert np.array_equal(sim.fields()[1], orc.histogram(*[pos[a].copy() for a in range(3)]))
+        sim.set_positions(dense if xyz is spread else spread)            # and the other way round on a live context
+        other = dense if xyz is spread else spread
+        assert np.array_equal(sim.fields()[1], orc.histogram(*[other[a].copy() for a in range(3)]))
+        sim.step(1)
+        sim.sync()
+        sim.destroy()
+
+
 # ---------------------------------------------------------------------------------------------
 # Smart-MC
 # ---------------------------------------------------------------------------------------------
