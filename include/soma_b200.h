@@ -282,6 +282,53 @@ int soma_sync(soma_ctx *ctx);
 
 void soma_destroy(soma_ctx *ctx);
 
+/* Stage 1 (a3 + a4: occupation numbers of Eq. 4, then omega of Eq. 12) of a
+ * configuration the CALLER holds in device memory, without a context and without a single allocation.
+ *
+ * Who this is for.  Every other entry point works on a soma_ctx, and soma_init pays for that context with
+ * cudaMalloc.  Some programs that want the fields of a configuration cannot afford that call at the point where
+ * they need them:
+ *   - an analysis or steering tool that runs next to simulations which already fill the GPU (C4 alone is sized
+ *     for the 180 GB): a cudaMalloc there fails, or succeeds only by making a caching allocator give memory back;
+ *   - a host program (PyTorch is the usual case) whose allocator owns the device memory and hands out pieces of
+ *     it: memory taken behind its back is invisible to its accounting, and it can lend this call buffers but not
+ *     the right to allocate;
+ *   - a loop that other streams run beside: cudaMalloc and cudaFree may wait for the whole device, so that one
+ *     allocation in the wrong place stalls kernels that have nothing to do with this call.
+ * For them the occupation numbers -- the only memory stage 1 needs besides its input and output -- live in an
+ * array that is part of the library image: SOMA_STATIC_MAX_WORDS 32-bit words (4 MiB, plus a few counters) of
+ * device memory on every GPU on which this library has been used, from the first use until the process exits,
+ * whether or not this function is ever called again.  That is the price, and the limit: a grid with
+ * n_types * cells > SOMA_STATIC_MAX_WORDS (C1, C2, C3 fit; C4 and C5 do not), or architectures with more than
+ * SOMA_STATIC_MAX_MONOMERS monomers in all, are refused with SOMA_EINVAL before anything is launched.
+ *
+ *   chains/n_specs   as for soma_init (bond lists are ignored: bonds do not enter the densities); types are host
+ *                    memory, read during the call
+ *   N_ref, n_types, box, grid, chiN, kappaN   as for soma_init; hamiltonian as SOMA_OPT_HAMILTONIAN (0 | 1)
+ *   dev_xyz          DEVICE, input: x[n] | y[n] | z[n] float32 of all n = sum n_chains * n_beads beads, the layout
+ *                    of soma_positions
+ *   dev_omega        DEVICE, output: float32 [n_types][cells]
+ *   dev_counts       DEVICE, output, or NULL: uint32 [n_types][cells] occupation numbers
+ *   cuda_stream      the stream the work is enqueued on (NULL: the legacy default stream)
+ * Works on the calling thread's current device, which must own all three buffers.  The results equal, bit for bit,
+ * what soma_fields returns from a context created by soma_init on the same positions with SOMA_OPT_COUNT_BITS = 32
+ * (the same kernels' arithmetic; no external field, every type pair at chiN).
+ *
+ * No cudaMalloc, cudaFree or other allocating routine is called.  The first call on a device looks up where that
+ * device keeps the array (cudaGetSymbolAddress, which makes the CUDA runtime load this library's kernels onto the
+ * device if nothing has yet); later calls on that device reuse the address.  Make that first call before any
+ * stream capture is begun.  The call synchronises cuda_stream before it returns (it reads back the counter of
+ * out-of-domain coordinates): SOMA_EDOMAIN as for soma_set_positions, with omega and counts written all the same.
+ *
+ * One array per device serves every call, from every thread, on every stream, and keeps what the last call left
+ * in it; each call clears the part it uses first.  Two calls that run on the same GPU at the same time therefore
+ * corrupt each other's occupation numbers: callers serialise them (one stream, or their own ordering). */
+#define SOMA_STATIC_MAX_WORDS    1048576u  /* n_types * cells                         */
+#define SOMA_STATIC_MAX_MONOMERS 256u      /* monomers of all architectures together  */
+int soma_fields_static(const soma_chain_spec *chains, int n_specs, int N_ref, int n_types, const float *box,
+                       const int *grid, float chiN, float kappaN, int hamiltonian, const float *dev_xyz,
+                       float *dev_omega, uint32_t *dev_counts, void *cuda_stream);
+
 const char *soma_last_error(void);
 const char *soma_version(void);
 

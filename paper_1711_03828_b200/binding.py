@@ -31,7 +31,9 @@ SYMBOLS = (
     "soma_n_beads", "soma_n_cells", "soma_n_types", "soma_sync", "soma_destroy", "soma_last_error",
     "soma_version", "soma_init_shard", "soma_shard_moves", "soma_shard_fields", "soma_shard_exchange",
     "soma_shard_exchange_copy", "soma_shard_peer_handle", "soma_shard_set_peers", "soma_architecture_words",
+    "soma_fields_static",
 )
+STATIC_MAX_WORDS, STATIC_MAX_MONOMERS = 1 << 20, 256
 
 
 class SomaError(RuntimeError):
@@ -88,6 +90,8 @@ def load() -> C.CDLL:
     L.soma_destroy.restype = None
     L.soma_last_error.restype = C.c_char_p
     L.soma_version.restype = C.c_char_p
+    L.soma_fields_static.argtypes = [C.POINTER(_ChainSpec), i32, i32, i32, C.POINTER(C.c_float), C.POINTER(C.c_int),
+                                     C.c_float, C.c_float, i32, vp, vp, vp, vp]
     _lib = L
     return L
 
@@ -118,6 +122,39 @@ def architecture_words(types: Sequence[int], bonds: Sequence[Tuple[int, int]]) -
     out = np.empty(n.value, np.uint32)
     _check(L.soma_architecture_words(C.byref(spec), C.c_void_p(out.ctypes.data), n.value, C.byref(n), C.byref(n_sets)))
     return out, int(n_sets.value)
+
+
+def fields_static(specs: Sequence[Tuple[int, Sequence[int]]], N_ref: int, n_types: int, box: Sequence[float],
+                  grid: Sequence[int], chiN: float, kappaN: float, xyz, omega, counts=None, hamiltonian: int = 0,
+                  stream: Optional[int] = None) -> None:
+    """soma_fields_static: omega (and counts) of the positions in the CUDA tensor `xyz`, written into the CUDA
+    tensors `omega` / `counts` the caller brings.  For callers that must not allocate device memory (a host
+    program whose allocator owns the GPU, a tool beside simulations that fill it): nothing is allocated, the
+    occupation numbers live in the library's static array (n_types * cells <= STATIC_MAX_WORDS).  Calls that
+    overlap on one GPU race on that array.  Synchronises `stream`."""
+    L = load()
+    keep = [np.ascontiguousarray(sp[1], dtype=np.uint8) for sp in specs]
+    arr = (_ChainSpec * len(specs))()
+    for i, (sp, t) in enumerate(zip(specs, keep)):
+        arr[i].n_chains = int(sp[0])
+        arr[i].n_beads = len(t)
+        arr[i].types = t.ctypes.data_as(C.POINTER(C.c_uint8))
+        arr[i].n_bonds = 0
+        arr[i].bonds = C.POINTER(C.c_uint32)()
+    cbox = (C.c_float * 3)(*[float(v) for v in box])
+    cgrid = (C.c_int * 3)(*[int(v) for v in grid])
+    if stream is None:
+        try:
+            import torch
+            stream = torch.cuda.current_stream().cuda_stream if torch.cuda.is_available() else 0
+        except Exception:
+            stream = 0
+    px = _ptr(xyz)[0] if xyz is not None else None
+    po = _ptr(omega)[0] if omega is not None else None
+    pc = _ptr(counts)[0] if counts is not None else None
+    _check(L.soma_fields_static(arr, len(specs), int(N_ref), int(n_types), cbox, cgrid, C.c_float(chiN),
+                                C.c_float(kappaN), int(hamiltonian), C.c_void_p(px), C.c_void_p(po), C.c_void_p(pc),
+                                C.c_void_p(stream or None)))
 
 
 class Soma:

@@ -25,6 +25,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <string>
 #include <vector>
@@ -1482,3 +1483,196 @@ int soma_sync(soma_ctx* c)
 }
 
 }  // extern "C"
+
+// ================================================================================================
+// soma_fields_static: stage 1 of a configuration the caller holds, for callers that cannot allocate
+// (include/soma_b200.h says who they are).  The occupation numbers -- the only memory stage 1 needs
+// besides its input and output -- are a file-scope device array: part of the library image, 4 MiB on
+// every GPU that has loaded this library, shared by every call.  Nothing above this line uses it, and
+// nothing below calls cudaMalloc, cudaFree or a library routine that allocates.
+// ================================================================================================
+namespace {
+
+constexpr uint32_t kStaticTail = 64;   // words behind the occupation numbers; word 0: beads outside the coordinate domain
+
+// In HOST code this name is only a handle for cudaGetSymbolAddress (it is not a device address: a kernel
+// handed `g_static_words` itself would read and write the wrong memory); device code may name it directly.
+static __device__ __align__(256) uint32_t g_static_words[SOMA_STATIC_MAX_WORDS + kStaticTail];
+
+struct StaticTypes {
+    uint8_t t[SOMA_STATIC_MAX_MONOMERS];   // bead type per monomer, the architectures one after the other
+};
+
+// histogram_kernel<false> with the type table in the kernel's parameters instead of in device memory
+// (a table in device memory would be one more buffer to allocate): Eq. 4, one count per bead.
+__global__ void __launch_bounds__(256)
+static_histogram_kernel(const soma::GridP g, const float* __restrict__ x, const float* __restrict__ y,
+                        const float* __restrict__ z, const __grid_constant__ StaticTypes types, uint32_t first,
+                        uint32_t N, uint32_t n_beads, uint32_t* __restrict__ counts, uint32_t* __restrict__ n_outside)
+{
+    const uint64_t stride = (uint64_t)gridDim.x * blockDim.x;
+    uint32_t bad = 0;
+    for (uint64_t i = (uint64_t)blockIdx.x * blockDim.x + threadIdx.x; i < n_beads; i += stride) {
+        const uint32_t j = (uint32_t)(i % N);
+        const float xi = x[i], yi = y[i], zi = z[i];
+        const uint32_t idx = soma::cell_at<false>(g, xi, yi, zi, (uint32_t)types.t[first + j] * g.cells + g.k_rec);
+        atomicAdd(counts + idx, 1u);
+        // the supported coordinates of cell_raw(): |t n| < 2^22 per axis (a NaN fails the comparison too)
+        const bool ok = fabsf(xi * g.inv_L[0] * g.nf[0]) < 4194304.0f && fabsf(yi * g.inv_L[1] * g.nf[1]) < 4194304.0f &&
+                        fabsf(zi * g.inv_L[2] * g.nf[2]) < 4194304.0f;
+        bad += ok ? 0u : 1u;
+    }
+    if (bad) atomicAdd(n_outside, bad);
+}
+
+// Where the current device keeps g_static_words.  Looked up once per device, with that device current.
+std::mutex g_static_mutex;
+uint32_t* g_static_addr[kMaxDevices] = {};
+
+int static_words_of(int dev, uint32_t** out)
+{
+    std::lock_guard<std::mutex> lock(g_static_mutex);
+    if (!g_static_addr[dev]) {
+        void* p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_static_words));
+        if (!p) return fail(SOMA_ECUDA, "soma_fields_static: cudaGetSymbolAddress returned no address on device %d", dev);
+        g_static_addr[dev] = static_cast<uint32_t*>(p);
+    }
+    *out = g_static_addr[dev];
+    return SOMA_OK;
+}
+
+// Is p device memory of device dev?  (A host pointer here would fault in the kernel, or on a system where
+// the GPU reaches host memory be used silently.)
+int static_check_pointer(const void* p, int dev, const char* name)
+{
+    cudaPointerAttributes at;
+    if (cudaPointerGetAttributes(&at, p) != cudaSuccess) {
+        cudaGetLastError();
+        return fail(SOMA_EINVAL, "soma_fields_static: %s is not a CUDA pointer", name);
+    }
+    if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged)
+        return fail(SOMA_EINVAL, "soma_fields_static: %s must be device memory", name);
+    if (at.type == cudaMemoryTypeDevice && at.device != dev)
+        return fail(SOMA_EINVAL, "soma_fields_static: %s lives on device %d, the current device is %d", name, at.device, dev);
+    return SOMA_OK;
+}
+
+}  // namespace
+
+extern "C" int soma_fields_static(const soma_chain_spec* chains, int n_specs, int N_ref, int n_types, const float* box,
+                                  const int* grid, float chiN, float kappaN, int hamiltonian, const float* dev_xyz,
+                                  float* dev_omega, uint32_t* dev_counts, void* cuda_stream)
+{
+    // ---- arguments: everything that can be refused is refused before the device is touched
+    if (!chains || n_specs < 1) return fail(SOMA_EINVAL, "soma_fields_static: need at least one chain spec");
+    if (N_ref < 1) return fail(SOMA_EINVAL, "soma_fields_static: N_ref must be >= 1");
+    if (n_types < 1 || n_types > SOMA_MAX_TYPES)
+        return fail(SOMA_EINVAL, "soma_fields_static: n_types must be in 1..%d", SOMA_MAX_TYPES);
+    if (!box || !grid) return fail(SOMA_EINVAL, "soma_fields_static: box/grid is NULL");
+    if (hamiltonian != 0 && hamiltonian != 1) return fail(SOMA_EINVAL, "soma_fields_static: hamiltonian must be 0 or 1");
+    if (!std::isfinite(chiN) || !std::isfinite(kappaN)) return fail(SOMA_EINVAL, "soma_fields_static: chiN/kappaN not finite");
+    soma_ctx p;                       // host-side parameter block only: gridp() / fieldp() as the contexts compute them
+    p.n_types = n_types;
+    p.N_ref = N_ref;
+    p.kappaN = kappaN;
+    p.hamiltonian = hamiltonian;
+    p.cells = 1;
+    for (int a = 0; a < 3; ++a) {
+        if (!(box[a] > 0.0f) || !std::isfinite(box[a])) return fail(SOMA_EINVAL, "soma_fields_static: box[%d] must be > 0", a);
+        if (grid[a] < 1 || grid[a] > (1 << 22)) return fail(SOMA_EINVAL, "soma_fields_static: grid[%d] must be in 1..2^22", a);
+        p.box[a] = box[a];
+        p.grid[a] = grid[a];
+        p.cells *= (uint64_t)grid[a];
+        if (p.cells > SOMA_STATIC_MAX_WORDS) break;
+    }
+    const uint64_t words = p.cells * (uint64_t)n_types;
+    if (p.cells > SOMA_STATIC_MAX_WORDS || words > SOMA_STATIC_MAX_WORDS)
+        return fail(SOMA_EINVAL, "soma_fields_static: the grid needs more than the %u words (n_types * cells) of the "
+                    "library's static array; larger grids need a context (soma_init), which allocates",
+                    (unsigned)SOMA_STATIC_MAX_WORDS);
+    for (int i = 0; i < n_types; ++i)
+        for (int k = 0; k < n_types; ++k) p.chiN[i][k] = i == k ? 0.0f : chiN;
+    StaticTypes types = {};
+    uint64_t n_monomers = 0, n_beads = 0;
+    for (int a = 0; a < n_specs; ++a) {
+        const uint32_t N = chains[a].n_beads;
+        if (N < 1 || (chains[a].n_chains > 0 && !chains[a].types))
+            return fail(SOMA_EINVAL, "soma_fields_static: spec %d: n_beads must be >= 1 and types non-NULL", a);
+        if (n_monomers + N > SOMA_STATIC_MAX_MONOMERS)
+            return fail(SOMA_EINVAL, "soma_fields_static: the architectures have more than %u monomers in all; such "
+                        "systems need a context (soma_init), which allocates", (unsigned)SOMA_STATIC_MAX_MONOMERS);
+        for (uint32_t j = 0; j < N; ++j) {
+            const uint8_t t = chains[a].n_chains ? chains[a].types[j] : 0;
+            if (t >= n_types)
+                return fail(SOMA_EINVAL, "soma_fields_static: spec %d monomer %u has type %u >= n_types", a, j, (unsigned)t);
+            types.t[n_monomers + j] = t;
+        }
+        n_monomers += N;
+        if (chains[a].n_chains >= (1ull << 32) || (n_beads += chains[a].n_chains * N) >= (1ull << 32))
+            return fail(SOMA_EINVAL, "soma_fields_static: total beads must be < 2^32");
+    }
+    if (n_beads == 0) return fail(SOMA_EINVAL, "soma_fields_static: the system has no beads");
+    if (!dev_xyz || !dev_omega) return fail(SOMA_EINVAL, "soma_fields_static: dev_xyz / dev_omega is NULL");
+    p.n_beads = p.n_beads_global = n_beads;
+
+    // ---- device
+    int n_dev = 0, dev = 0, major = 0, n_sm = 0;
+    if (cudaGetDeviceCount(&n_dev) != cudaSuccess || n_dev < 1) {
+        cudaGetLastError();
+        return fail(SOMA_ENODEVICE, "soma_fields_static: no CUDA device (this library has no CPU path)");
+    }
+    CU(cudaGetDevice(&dev));
+    if (dev < 0 || dev >= kMaxDevices) return fail(SOMA_EINVAL, "soma_fields_static: device %d is beyond the %d this library tracks", dev, kMaxDevices);
+    CU(cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, dev));
+    CU(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    if (major != 10) return fail(SOMA_ENODEVICE, "soma_fields_static: kernels are built for sm_100a only, device is sm_%dx", major);
+    int rc = static_check_pointer(dev_xyz, dev, "dev_xyz");
+    if (!rc) rc = static_check_pointer(dev_omega, dev, "dev_omega");
+    if (!rc && dev_counts) rc = static_check_pointer(dev_counts, dev, "dev_counts");
+    if (rc) return rc;
+    uint32_t* words_dev = nullptr;    // the DEVICE address of g_static_words on this device
+    rc = static_words_of(dev, &words_dev);
+    if (rc) return rc;
+    uint32_t* n_outside = words_dev + SOMA_STATIC_MAX_WORDS;
+    cudaStream_t stream = (cudaStream_t)cuda_stream;
+
+    // ---- a3: the array keeps the last call's numbers; clear what this call counts into
+    CU(cudaMemsetAsync(words_dev, 0, sizeof(uint32_t) * words, stream));
+    CU(cudaMemsetAsync(n_outside, 0, sizeof(uint32_t), stream));
+    const soma::GridP g = p.gridp();
+    uint64_t bead0 = 0;
+    uint32_t first = 0;
+    for (int a = 0; a < n_specs; ++a) {
+        const uint32_t N = chains[a].n_beads;
+        const uint64_t nb = chains[a].n_chains * N;
+        if (nb) {
+            const int threads = 256;
+            const uint64_t blocks = std::min<uint64_t>((nb + threads - 1) / threads, (uint64_t)n_sm * 16);
+            static_histogram_kernel<<<(unsigned)blocks, threads, 0, stream>>>(
+                g, dev_xyz + bead0, dev_xyz + n_beads + bead0, dev_xyz + 2 * n_beads + bead0, types, first, N, (uint32_t)nb,
+                words_dev, n_outside);
+            CU(cudaGetLastError());
+        }
+        bead0 += nb;
+        first += N;
+    }
+
+    // ---- a4: the contexts' field kernel, reading the static array, writing the caller's omega
+    const soma::FieldP F = p.fieldp();
+    const int threads = 256;
+    const unsigned blocks = (unsigned)((p.cells + threads - 1) / threads);
+    switch (n_types) {
+        case 1: CU(launch_pdl(false, soma::field_kernel<1, false>, blocks, threads, 0, stream, F, words_dev, dev_omega, nullptr, nullptr, nullptr, nullptr, 0ull, nullptr, nullptr, 0u, (size_t)0)); break;
+        case 2: CU(launch_pdl(false, soma::field_kernel<2, false>, blocks, threads, 0, stream, F, words_dev, dev_omega, nullptr, nullptr, nullptr, nullptr, 0ull, nullptr, nullptr, 0u, (size_t)0)); break;
+        default: CU(launch_pdl(false, soma::field_kernel<0, false>, blocks, threads, 0, stream, F, words_dev, dev_omega, nullptr, nullptr, nullptr, nullptr, 0ull, nullptr, nullptr, 0u, (size_t)0)); break;
+    }
+    if (dev_counts) CU(cudaMemcpyAsync(dev_counts, words_dev, sizeof(uint32_t) * words, cudaMemcpyDeviceToDevice, stream));
+    uint32_t bad = 0;
+    CU(cudaMemcpyAsync(&bad, n_outside, sizeof(uint32_t), cudaMemcpyDeviceToHost, stream));
+    CU(cudaStreamSynchronize(stream));
+    if (bad)
+        return fail(SOMA_EDOMAIN, "soma_fields_static: %u beads have a coordinate that is not finite or lies outside "
+                    "the supported domain |x n / L| < 2^22 per axis", bad);
+    return SOMA_OK;
+}
