@@ -129,13 +129,21 @@ class ClockSampler:
         """The timed region starts now: samples taken earlier (warm-up) are dropped at the end."""
         self.t_from = time.perf_counter()
 
-    def summary(self):
+    def summary(self, region=None):
+        """region: (t0, t1) on the perf_counter clock -- the host's estimate of when the timed region ran on the
+        device; the number of samples that fall inside it is reported beside the number the statistics are over."""
         if not self.samples:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["clock query unavailable"]}
         mhz = sorted(s[0] for s in self.samples)
         reasons = [n for i, n in enumerate(self.NAMES) if any(s[2 + i] for s in self.samples)]
-        return {"sm_mhz": mhz[len(mhz) // 2], "sm_min_mhz": mhz[0], "sm_max_mhz": self.samples[0][1],
-                "reasons": reasons, "samples": len(mhz), "source": self.source}
+        out = {"sm_mhz": mhz[len(mhz) // 2], "sm_min_mhz": mhz[0], "sm_max_mhz": self.samples[0][1],
+               "reasons": reasons, "samples": len(mhz), "source": self.source}
+        if region is not None:
+            out["samples_in_timed_region"] = sum(1 for s in self.samples if region[0] <= s[-1] <= region[1])
+            out["window"] = ("samples: from the host's mark() -- the device work queued in front of the start event (spin, "
+                             "pre-roll) and the timed region; samples_in_timed_region: those within the last ms_total "
+                             "before the closing synchronisation returned")
+        return out
 
 
 def kernel_source_hash() -> str:
@@ -431,6 +439,7 @@ def main():
     # all, which a 20-step region of 2 ms would carry as +3 %); the events are in stream order, so exactly the K
     # steps lie between them.
     pre_roll = min(5, args.warmup)
+    config["pre_roll"] = {"steps": pre_roll, "spin": {"buffer_bytes": 256 << 20, "passes": 120, "approx_ms": 10}}
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     with ClockSampler(local_rank) as clk:      # the sampling thread is up before the GPU is left idle for the last time
         sim.step(args.warmup - pre_roll)
@@ -449,7 +458,9 @@ def main():
         sim.step(args.steps)                   # one soma_step(K) call: K x (move launch, field launch), no Python in between
         e1.record()
         barrier()
+        t_end = time.perf_counter()            # the closing synchronisation has returned: the device finished just before
     ms_total = e0.elapsed_time(e1)
+    timed_region = (t_end - ms_total * 1e-3 - 2e-4, t_end)
     launches = sim.launch_count() - l0
     ms_total = max_over_ranks(ms_total, dist, "cuda")
     value = aggregate_moves_per_s(nb, args.steps, world, ms_total)
@@ -483,7 +494,7 @@ def main():
     prof = profile_entry(w.name)
     roofline["traffic"] = prof["dram_bytes"] if prof else None
     # second roof: warp-instruction issue, one instruction per cycle and scheduler
-    clocks_now = clk.summary()
+    clocks_now = clk.summary(timed_region)
     if clocks_now.get("sm_mhz") and prof:
         n_sm = torch.cuda.get_device_properties(local_rank).multi_processor_count
         peak_ips = n_sm * SCHEDULERS_PER_SM * clocks_now["sm_mhz"] * 1e6
@@ -518,7 +529,7 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": ms_total / args.steps, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic", "config": config,
-            "clocks": clk.summary(), "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
+            "clocks": clocks_now, "e2e": e2e, "gpu_launches": launches, "roofline": roofline,
             "acceptance": acc / max(1, att)}
     if world == 1 and args.aged > 0 and not args.sharded:
         # The same step over a long stretch (default 5000 sweeps, ~0.5 s): the melt orders on the way
