@@ -61,7 +61,9 @@ enum {
 enum {
     SOMA_OPT_HAMILTONIAN = 1,      /* 0: K^0_inter (Eq. 7, default), 1: K^1_inter (Eq. 8); refreshes omega   */
     SOMA_OPT_MOVE = 2,             /* 1: local displacement (default), 2: Smart-MC                            */
-    SOMA_OPT_SMC_STEP = 3,         /* Smart-MC step a_s in R_e0^2 (> 0)                                       */
+    SOMA_OPT_SMC_STEP = 3,         /* Smart-MC step a_s in R_e0^2, 0 < a_s <= 0.125 (SOMA_EINVAL beyond: the  */
+                                   /* proposal's fast Box-Muller is accurate to ~2e-6 per Gaussian, so that a  */
+                                   /* displacement stays within 1e-6 R_e0 of the exact one up to sqrt(2 a_s) = 0.5) */
     SOMA_OPT_RECORD_DECISIONS = 4, /* 1: keep the accept/reject bit of every move of the last sweep           */
     SOMA_OPT_KERNEL = 5,           /* 0: auto (default); 1: force the one-thread-per-monomer kernels on global */
                                    /* memory (two launches per sweep for linear chains, one per independent   */
@@ -72,8 +74,7 @@ enum {
                                    /* 1: clear + full histogram kernel after every sweep                      */
     SOMA_OPT_TIMING = 7,           /* 1: bracket every kernel with CUDA events (see soma_kernel_times)        */
     SOMA_OPT_SWEEP_COUNTER = 8,    /* set the sweep counter (the "time step" word of the Philox counter)      */
-                                   /* (key 9 is not used: see DESIGN.md 6.7 for the one-launch variants measured) */
-    SOMA_OPT_BLOCKS_PER_SM = 10,   /* tuning: grid of the fused kernel = SMs x this many blocks; 0 = resident max */
+                                   /* (keys 9 and 10 are not used)                                             */
     SOMA_OPT_LAYOUT = 11,          /* 0: chains stay in the caller's order in device memory; 1 (default): the  */
                                    /* library keeps them in Hilbert order of their centres of mass.  Storage   */
                                    /* only: every result is identical, every API array is in the caller's order */

@@ -4,7 +4,7 @@ The product is the C-ABI library ``libsoma_b200.so`` (``include/soma_b200.h``); 
 builds it (``_build``) and marshals arguments to it (``binding``).  No CPU fallback exists.
 """
 from .binding import (DENSITY_FULL, DENSITY_INCREMENTAL, KERNEL_AUTO, KERNEL_FUSED, KERNEL_GENERIC,  # noqa: F401
-                      K_COUNT, K_DENSITY, K_FIELD, K_LAYOUT, K_MOVE, OPT_LAYOUT, OPT_SORT_INTERVAL, OPT_SET_ORDER, OPT_FIELD_INTERVAL, OPT_SCHEME, OPT_PDL, MOVE_LOCAL, MOVE_SMC, OPT_BLOCKS_PER_SM, OPT_DENSITY,
+                      K_COUNT, K_DENSITY, K_FIELD, K_LAYOUT, K_MOVE, OPT_LAYOUT, OPT_SORT_INTERVAL, OPT_SET_ORDER, OPT_FIELD_INTERVAL, OPT_SCHEME, OPT_PDL, MOVE_LOCAL, MOVE_SMC, OPT_DENSITY,
                       OPT_HAMILTONIAN, OPT_KERNEL, OPT_MOVE, OPT_RECORD_DECISIONS, OPT_SMC_STEP,
                       OPT_SWEEP_COUNTER, OPT_TIMING, OPT_COUNT_BITS, EOVERFLOW, SYMBOLS, Soma, SomaError, load, unpack_decisions,
                       STATIC_MAX_WORDS, STATIC_MAX_MONOMERS, fields_static)

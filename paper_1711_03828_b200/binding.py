@@ -15,7 +15,7 @@ from . import _build
 
 OK = 0
 OPT_HAMILTONIAN, OPT_MOVE, OPT_SMC_STEP, OPT_RECORD_DECISIONS = 1, 2, 3, 4
-OPT_KERNEL, OPT_DENSITY, OPT_TIMING, OPT_SWEEP_COUNTER, OPT_BLOCKS_PER_SM = 5, 6, 7, 8, 10
+OPT_KERNEL, OPT_DENSITY, OPT_TIMING, OPT_SWEEP_COUNTER = 5, 6, 7, 8
 OPT_LAYOUT, OPT_SORT_INTERVAL, OPT_SET_ORDER, OPT_FIELD_INTERVAL, OPT_SCHEME, OPT_PDL = 11, 12, 13, 14, 15, 16
 OPT_COUNT_BITS = 17
 EOVERFLOW = -7

@@ -89,6 +89,10 @@ struct Spec {
     uint64_t arch_off = 0;
     std::vector<uint32_t> set_off;   // [n_sets + 1] offsets into members[]
     uint32_t n_arch_words = 0;       // Fig. 2 words | members | set_off | set_magic
+    // grid and shared memory of the fused kernel in random set order (launch_fused), kept per instantiation asked last
+    mutable const void* order_kernel = nullptr;
+    mutable int order_device = -1, order_blocks = 0;
+    mutable size_t order_smem = 0;
 };
 
 constexpr int kEventPool = 2048;
@@ -115,6 +119,8 @@ struct soma_ctx {
     const uint32_t** peer_table = nullptr;   // device: [n_peers] base addresses of the ranks' allocations
     uint32_t* exchange = nullptr;    // shard: what this rank's move kernels count into; summed over the ranks by the caller,
                                      // folded into counts (the whole system's numbers) by the field kernel, which clears it
+    bool counts_pending = false;     // shard: counts was cleared by a histogram (which went into the exchange array) and is
+                                     // not the whole system's numbers until the next soma_shard_fields folds the sum in
 
     float *x = nullptr, *y = nullptr, *z = nullptr;
     uint32_t* counts = nullptr;      // planes [n_types][cells], or packed [cells] (pack)
@@ -158,7 +164,6 @@ struct soma_ctx {
     int hamiltonian = 0, move = 1, record = 0, kernel_choice = 0, density_mode = 0, timing = 0;
     uint32_t* n_outside = nullptr;   // device counter: beads whose coordinates are outside the supported domain
     int pdl = 1;             // programmatic dependent launch of the fused and field kernels (SOMA_OPT_PDL)
-    int blocks_per_sm = 0;   // grid of the fused kernel = n_sm * blocks_per_sm; 0 = as many as are resident
     float smc_step = 0.0f;
 
     uint64_t sweep = 0, attempted = 0, launches = 0;
@@ -374,27 +379,67 @@ int launch_fused(soma_ctx* c, const soma::MoveP& P, const Spec& s)
 {
     auto kernel = soma::fused_sweep_kernel<kMove, kIncr, kRecord, kOrder, kPack, kAnyN>;
     constexpr int threads = soma::kFusedThreads, warps_per_block = threads / 32;
-    constexpr size_t kOrderSmemMax = 160 * 1024;       // shared memory for the order bits of a block's chains
-    static int resident[kMaxDevices] = {};             // blocks per SM of this instantiation, asked once per device
-    int& res = resident[c->device % kMaxDevices];
-    if (res == 0) {
-        if (kOrder) CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kOrderSmemMax));
-        CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&res, kernel, threads, 0));
-        if (res < 1) res = 1;
+    // blocks per SM of this instantiation (without dynamic shared memory) and the shared memory a block may ask for,
+    // asked once per device; the mutex makes the first launches of two threads safe
+    static std::mutex mu;
+    static int resident[kMaxDevices] = {};
+    static size_t smem_limit[kMaxDevices] = {};
+    const int dev_slot = c->device % kMaxDevices;
+    {
+        std::lock_guard<std::mutex> lock(mu);
+        if (resident[dev_slot] == 0) {
+            int r = 0;
+            if (kOrder) {
+                // shared memory for the order bits of a block's chains: 160 KB, or what the device grants a block if
+                // that is less (static shared memory of the kernel taken off)
+                int optin = 0;
+                cudaFuncAttributes fa;
+                CU(cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
+                CU(cudaFuncGetAttributes(&fa, kernel));
+                size_t lim = std::min<size_t>(160 * 1024, (size_t)optin > fa.sharedSizeBytes ? (size_t)optin - fa.sharedSizeBytes : 0);
+                if (lim < 1024) return fail(SOMA_ECUDA, "launch_fused: the device grants a block %d bytes of shared memory", optin);
+                CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)lim));
+                smem_limit[dev_slot] = lim;
+            }
+            CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&r, kernel, threads, 0));
+            resident[dev_slot] = r < 1 ? 1 : r;
+        }
     }
-    const int per_sm = c->blocks_per_sm > 0 ? c->blocks_per_sm : res;   // auto: every block resident, one wave
+    const int res = resident[dev_slot];
+    int per_sm = res;                                  // every block resident, one wave
     int blocks = c->n_sm * per_sm;
     const int max_useful = (int)((s.n_tiles + warps_per_block - 1) / warps_per_block);
     if (blocks > max_useful) blocks = max_useful;
     // random set order: four bytes per chain of the longest tile range a block can get (the chains grouped by
-    // their order bit); more (not all resident) blocks if that does not fit into shared memory
+    // their order bit); more (not all resident) blocks if that does not fit into shared memory.  The shared memory
+    // may lower the number of resident blocks, and fewer blocks need more of it each: iterate to the fixed point
+    // (per_sm only falls; on a B200 the kernel's registers allow one block per SM and the loop runs once).  The
+    // result depends on the spec and the instantiation only: kept with the spec.
     size_t order_smem = 0;
     if (kOrder) {
-        const size_t chains_per_tile = soma::kTile / s.N;      // floor: also for kAnyN
-        for (int waves = 1;; ++waves) {
-            order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile * 4 + 16;
-            if (order_smem <= kOrderSmemMax) break;
-            blocks = c->n_sm * per_sm * (waves + 1);
+        if (s.order_kernel == (const void*)kernel && s.order_device == c->device) {
+            blocks = s.order_blocks;
+            order_smem = s.order_smem;
+        } else {
+            const size_t limit = smem_limit[dev_slot];
+            const size_t chains_per_tile = soma::kTile / s.N;      // floor: also for kAnyN
+            for (;;) {
+                for (int waves = 1;; ++waves) {
+                    blocks = std::min(c->n_sm * per_sm * waves, max_useful);
+                    order_smem = ((size_t)s.n_tiles / blocks + 1) * chains_per_tile * 4 + 16;
+                    if (order_smem <= limit || blocks == max_useful) break;
+                }
+                if (order_smem > limit) return fail(SOMA_ECUDA, "launch_fused: order bits of one warp's tiles exceed shared memory");
+                int r = 0;
+                CU(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&r, kernel, threads, order_smem));
+                if (r < 1) r = 1;
+                if (r >= per_sm) break;
+                per_sm = r;
+            }
+            s.order_kernel = (const void*)kernel;
+            s.order_device = c->device;
+            s.order_blocks = blocks;
+            s.order_smem = order_smem;
         }
     }
     Timed t(c, SOMA_K_MOVE, 1);
@@ -570,6 +615,7 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
 {
     CU(cudaMemsetAsync(c->counts, 0, counts_bytes(c), c->stream));
     if (c->sharded) CU(cudaMemsetAsync(c->exchange, 0, counts_bytes(c), c->stream));   // counts = 0 + sum of the ranks' histograms
+    if (c->sharded) c->counts_pending = true;
     const soma::GridP g = c->gridp();
     for (const Spec& s : c->specs) {
         if (s.n_beads == 0) continue;
@@ -593,10 +639,7 @@ int launch_histogram(soma_ctx* c, bool check_domain_too)
 int launch_fields(soma_ctx* c, int fold = 0)
 {
     const soma::FieldP F = c->fieldp();
-#ifndef SOMA_FIELD_THREADS
-#define SOMA_FIELD_THREADS 256
-#endif
-    const int threads = SOMA_FIELD_THREADS;
+    const int threads = 256;
     const unsigned blocks = (unsigned)((c->cells + threads - 1) / threads);
     Timed t(c, SOMA_K_FIELD, 1);
     const bool pdl = c->pdl != 0;
@@ -620,9 +663,14 @@ int launch_fields(soma_ctx* c, int fold = 0)
     return SOMA_OK;
 }
 
-// omega after a parameter change (a shard holds the whole system's occupation numbers too)
+// omega after a parameter change (a shard holds the whole system's occupation numbers too).  Between a histogram
+// of a shard (soma_init_shard, soma_set_positions, a change of SOMA_OPT_COUNT_BITS) and the soma_shard_fields(ctx, 0)
+// that follows it, counts is all zero: omega of that would be meaningless, and the packed format's check (halves
+// against the number of beads) would raise the sticky overflow flag.  Nothing to do then: that soma_shard_fields
+// computes omega with the parameters as they are by then.
 int refresh_fields(soma_ctx* c)
 {
+    if (c->sharded && c->counts_pending) return SOMA_OK;
     return launch_fields(c);
 }
 
@@ -1163,20 +1211,36 @@ int soma_shard_set_peers(soma_ctx* c, int n_ranks, int my_rank, void* const* pee
     if (c->n_peers) return fail(SOMA_ESTATE, "soma_shard_set_peers: the peers of this context are already set");
     if (c->sweep != 0) return fail(SOMA_ESTATE, "soma_shard_set_peers: call it before the first sweep");
     std::vector<const uint32_t*> table(n_ranks);
+    // on any failure below the context is left as it was: mappings opened by this call are closed again and the
+    // table is freed, so that the call can be repeated
+    auto undo = [c](int code) {
+        for (void* m : c->peer_opened) cudaIpcCloseMemHandle(m);
+        c->peer_opened.clear();
+        if (c->peer_table) cudaFree(c->peer_table);
+        c->peer_table = nullptr;
+        cudaGetLastError();
+        return code;
+    };
     for (int r = 0; r < n_ranks; ++r) {
         if (r == my_rank) { table[r] = c->exchange_base; continue; }
         if (peer_dev && peer_dev[r]) { table[r] = (const uint32_t*)peer_dev[r]; continue; }
-        if (!handles) return fail(SOMA_EINVAL, "soma_shard_set_peers: no address and no handle for rank %d", r);
+        if (!handles) return undo(fail(SOMA_EINVAL, "soma_shard_set_peers: no address and no handle for rank %d", r));
         cudaIpcMemHandle_t h;
         std::memcpy(&h, (const char*)handles + 64 * (size_t)r, sizeof h);
         void* mapped = nullptr;
-        CU(cudaIpcOpenMemHandle(&mapped, h, cudaIpcMemLazyEnablePeerAccess));
+        cudaError_t e = cudaIpcOpenMemHandle(&mapped, h, cudaIpcMemLazyEnablePeerAccess);
+        if (e != cudaSuccess)
+            return undo(fail(SOMA_ECUDA, "soma_shard_set_peers: cudaIpcOpenMemHandle for rank %d: %s", r, cudaGetErrorString(e)));
         c->peer_opened.push_back(mapped);
         table[r] = (const uint32_t*)mapped;
     }
-    CU(cudaMalloc(&c->peer_table, sizeof(uint32_t*) * n_ranks));
-    CU(cudaMemcpyAsync(c->peer_table, table.data(), sizeof(uint32_t*) * n_ranks, cudaMemcpyHostToDevice, c->stream));
-    CU(cudaStreamSynchronize(c->stream));
+    cudaError_t e = cudaMalloc(&c->peer_table, sizeof(uint32_t*) * n_ranks);
+    if (e == cudaSuccess)
+        e = cudaMemcpyAsync(c->peer_table, table.data(), sizeof(uint32_t*) * n_ranks, cudaMemcpyHostToDevice, c->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(c->stream);
+    if (e != cudaSuccess)
+        return undo(fail(e == cudaErrorMemoryAllocation ? SOMA_ENOMEM : SOMA_ECUDA, "soma_shard_set_peers: table of the peers' "
+                         "addresses: %s", cudaGetErrorString(e)));
     c->n_peers = n_ranks;
     c->my_rank = my_rank;
     return SOMA_OK;
@@ -1194,6 +1258,7 @@ int soma_shard_fields(soma_ctx* c, int advance)
             return fail(SOMA_ESTATE, "soma_shard_fields: with peers set, SOMA_OPT_FIELD_INTERVAL must be 1");
         int rc = launch_fields(c, 2);
         if (rc) return rc;
+        c->counts_pending = false;
         c->peer_parity ^= 1;
         c->exchange = c->exchange_base + (size_t)c->peer_parity * c->cells * c->n_types;
         if (advance) c->sweep += 1;
@@ -1208,6 +1273,7 @@ int soma_shard_fields(soma_ctx* c, int advance)
         soma::fold_exchange_kernel<<<(unsigned)((n + 255) / 256), 256, 0, c->stream>>>(c->counts, c->exchange, n);
         CU(cudaGetLastError());
     }
+    c->counts_pending = false;
     if (advance) c->sweep += 1;
     return SOMA_OK;
 }
@@ -1338,6 +1404,11 @@ int soma_set_option(soma_ctx* c, int key, double value)
             return SOMA_OK;
         case SOMA_OPT_SMC_STEP:
             if (!(value > 0.0) || !std::isfinite(value)) return fail(SOMA_EINVAL, "SOMA_OPT_SMC_STEP: must be > 0");
+            // the proposal's Gaussians are off by up to ~2e-6 (draw_move), a displacement by sqrt(2 a_s) times
+            // that: within the 1e-6 R_e0 this library states for Smart-MC positions only while sqrt(2 a_s) <= 0.5
+            if (value > 0.125)
+                return fail(SOMA_EINVAL, "SOMA_OPT_SMC_STEP: a_s must be <= 0.125 R_e0^2 (beyond it the approximate "
+                            "Box-Muller of the proposal no longer keeps displacements within 1e-6 R_e0 of the exact ones)");
             c->smc_step = (float)value;
             return SOMA_OK;
         case SOMA_OPT_RECORD_DECISIONS:
@@ -1366,10 +1437,6 @@ int soma_set_option(soma_ctx* c, int key, double value)
         case SOMA_OPT_PDL:
             if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_PDL: 0 or 1");
             c->pdl = iv;
-            return SOMA_OK;
-        case SOMA_OPT_BLOCKS_PER_SM:
-            if (iv < 0 || iv > 32) return fail(SOMA_EINVAL, "SOMA_OPT_BLOCKS_PER_SM: 0 (auto) .. 32");
-            c->blocks_per_sm = iv;
             return SOMA_OK;
         case SOMA_OPT_LAYOUT: {
             if (iv != 0 && iv != 1) return fail(SOMA_EINVAL, "SOMA_OPT_LAYOUT: 0 or 1");

@@ -23,24 +23,9 @@ namespace soma {
 constexpr int kMaxTypes = 8;
 constexpr int kTile = 128;          // beads per warp tile in the fused kernel (4 per lane)
 constexpr int kAccSlots = 256;      // spread slots of the accepted-moves counter
-#ifndef SOMA_FUSED_THREADS
-#define SOMA_FUSED_THREADS 640       // threads per block of the fused kernel: one block of 20 warps per SM
-#endif
-constexpr int kFusedThreads = SOMA_FUSED_THREADS;
-#ifndef SOMA_MOL_UNROLL
-#define SOMA_MOL_UNROLL 4
-#endif
-constexpr int kMolUnroll = SOMA_MOL_UNROLL;   // attempts of the staged molecule kernel unrolled together
-
-#ifndef SOMA_SMC_FAST
-#define SOMA_SMC_FAST 1
-#endif
-#ifndef SOMA_OMEGA_NC
-#define SOMA_OMEGA_NC 0
-#endif
-#ifndef SOMA_FUSED_MIN_BLOCKS
-#define SOMA_FUSED_MIN_BLOCKS 1      // resident blocks per SM the fused kernel is compiled for (register cap: 96)
-#endif
+constexpr int kFusedThreads = 640;  // threads per block of the fused kernel: one block of 20 warps per SM
+constexpr int kFusedMinBlocks = 1;  // resident blocks per SM the fused kernel is compiled for (register cap: 96)
+constexpr int kMolUnroll = 4;       // attempts of the staged molecule kernel unrolled together
 
 struct GridP {
     float inv_L[3];   // fl32(1 / L_a)
@@ -152,28 +137,13 @@ __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;"
 
 // Positions cross the SM once per sweep: streaming (evict-first) loads and stores, so that they do not push
 // the omega lines the gathers reuse out of L1.
-#ifndef SOMA_STREAM_POS
-#define SOMA_STREAM_POS 1
-#endif
 __device__ __forceinline__ float4 ld_stream(const float* p)
 {
-#if SOMA_STREAM_POS == 1
     return __ldcs(reinterpret_cast<const float4*>(p));
-#elif SOMA_STREAM_POS == 2
-    float4 v;
-    asm volatile("ld.global.L1::no_allocate.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
-    return v;
-#else
-    return *reinterpret_cast<const float4*>(p);
-#endif
 }
 __device__ __forceinline__ void st_stream(float* p, const float4& v)
 {
-#if SOMA_STREAM_POS >= 1
     __stcs(reinterpret_cast<float4*>(p), v);
-#else
-    *reinterpret_cast<float4*>(p) = v;
-#endif
 }
 
 // top 23 bits -> float in [1, 2), exact
@@ -284,7 +254,6 @@ __device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
         uint32_t w[4], v[4];
         philox4x32_10_head(gid, P.head[0], P.rk, w);
         philox4x32_10_head(gid, P.head[1], P.rk, v);
-#if SOMA_SMC_FAST
         // Box-Muller with sin.approx / cos.approx (MUFU) for the angle, taken in [-pi, pi) where the
         // approximations are best (absolute error 2^-21.4): sin(t) = -sin(t - pi), cos(t) = -cos(t - pi), and
         // t - pi = 2 pi (U23 - 1.5) with an exact subtraction.  A Gaussian is then off by <= ~2e-6, a
@@ -295,14 +264,6 @@ __device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
         const float two_pi = 6.283185307179586f;
         const float ta = two_pi * (u23(w[1]) - 1.5f), tb = two_pi * (u23(w[3]) - 1.5f);
         const float sa = -__sinf(ta), ca = -__cosf(ta), cb = -__cosf(tb);
-#else
-        const float ra = sqrtf(-2.0f * logf(2.0f - u23(w[0])));
-        const float rb = sqrtf(-2.0f * logf(2.0f - u23(w[2])));
-        const float two_pi = 6.283185307179586f;
-        float sa, ca, sb, cb;
-        sincosf(two_pi * (u23(w[1]) - 1.0f), &sa, &ca);
-        sincosf(two_pi * (u23(w[3]) - 1.0f), &sb, &cb);
-#endif
         r.a = ra * ca; r.b = ra * sa; r.c = rb * cb;
         r.u = u23(v[0]) - 1.0f;
     }
@@ -315,15 +276,10 @@ __device__ __forceinline__ float field_delta(const float* __restrict__ omega, ui
 {
     float w_new = 0.0f, w_old = 0.0f;
     if (i_new != i_old) {
-#if SOMA_OMEGA_NC
-        w_new = __ldg(omega + i_new);
-        w_old = __ldg(omega + i_old);
-#else
         // ordinary loads: with programmatic dependent launch this kernel may be resident while the field
         // kernel still writes omega, which rules out the non-coherent path (ld.global.nc)
         asm("ld.global.f32 %0, [%1];" : "=f"(w_new) : "l"(omega + i_new));
         asm("ld.global.f32 %0, [%1];" : "=f"(w_old) : "l"(omega + i_old));
-#endif
     }
     return w_new - w_old;
 }
@@ -464,7 +420,7 @@ __device__ __forceinline__ bool mc_move(const MoveP& P, const float* __restrict_
 // holds floor(128 / N) whole chains, the lanes beyond them idle (they load harmlessly, decide nothing and
 // store nothing); n_mask then carries N and log2N the chains per tile.
 template <int kMove, bool kIncr, bool kRecord, bool kOrder, bool kPack, bool kAnyN = false>
-__global__ void __launch_bounds__(kFusedThreads, SOMA_FUSED_MIN_BLOCKS)
+__global__ void __launch_bounds__(kFusedThreads, kFusedMinBlocks)
 fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, float* __restrict__ z,
                    const float* __restrict__ omega, uint32_t* __restrict__ counts,
                    const uint32_t* __restrict__ toff_tab, uint32_t n_mask, uint32_t n_tiles,

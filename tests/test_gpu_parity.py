@@ -603,6 +603,109 @@ def test_c5_blend_full_size_smart_mc(smc_step):
 
 
 # ---------------------------------------------------------------------------------------------
+# the code paths that only large systems reach (What's weak 1): lock-step against the oracle at
+# sizes where the regrouping prologue of the random set order runs several passes and repeats, where its order
+# bits no longer fit into one wave's shared memory, where the fused kernel hands out tiles dynamically for chain
+# lengths that do not divide 128, and where the staged kernels go round their grid-stride loop more than once
+# ---------------------------------------------------------------------------------------------
+MAX_RESIDENT_WARPS = 148 * 64      # no more warps than this are resident on a B200 whatever the kernel
+
+
+def _short_chain_melt(name, n_chains, grid, seed):
+    # N = 4 diblocks at ~20 beads per cell; a box of 0.2 R_e0 cells
+    box = tuple(0.2 * g for g in grid)
+    return workloads.Workload(name, ((n_chains, workloads.diblock(4, 2)),), 4, 2, box, grid, 12.0, 30.0, 0.1, seed)
+
+
+def test_random_set_order_every_pass_of_the_regrouping_prologue():
+    """800,000 chains of N = 4 (3.2 M beads): a block of the fused kernel owns > 5120 chains, so the prologue that
+    regroups a block's chains by their order bit runs all of its passes (1280 chains each) and repeats its outer
+    loop (Code 2)."""
+    w = _short_chain_melt("order_800k", 800_000, (64, 50, 50), 31)
+    assert w.n_chains / 148 > 5120
+    flips = lockstep(w, 2, set_order=1)
+    assert flips <= 2 * FLIPS_PER_MOVE * w.n_beads
+
+
+def test_random_set_order_c3_full_size():
+    """The headline melt in random set order: the configuration behind 'C3 random set order' in bench.py --all-configs."""
+    w = workloads.c3()
+    log = []
+    lockstep(w, 2, set_order=1, flip_log=log)
+    assert max(log) <= FLIPS_PER_MOVE * w.n_beads, log
+
+
+def test_random_set_order_more_order_bits_than_one_wave_holds():
+    """6.2 M chains of N = 4 (24.8 M beads): with one resident block per SM a block would own ~41,900 chains, whose
+    order bits (4 bytes each) exceed the 160 KB of shared memory a block may take, so the launch falls back to
+    several waves of blocks."""
+    w = _short_chain_melt("order_6M", 6_200_000, (128, 100, 100), 33)
+    assert w.n_chains / 148 * 4 > 160 * 1024
+    flips = lockstep(w, 1, set_order=1)
+    assert flips <= FLIPS_PER_MOVE * w.n_beads
+
+
+@pytest.mark.parametrize("set_order", [0, 1], ids=["fixed-order", "random-order"])
+def test_chain_lengths_that_do_not_divide_the_tile_dynamic_tile_hand_out(set_order):
+    """9000 chains of N = 100 (one per tile) and 60,000 of N = 20 (six per tile): more than 40 tiles per block, so
+    the warps of a block draw further tiles from the block's counter after their two static rounds."""
+    w = workloads.Workload("anyN_large", ((9000, workloads.diblock(100, 40)), (60_000, workloads.diblock(20, 7))), 32, 2,
+                           (10.0, 10.0, 10.0), (50, 50, 50), 20.0, 50.0, 0.1, 37)
+    for n, t in w.specs:
+        assert n // (128 // len(t)) > 40 * 148
+    flips = lockstep(w, 2, set_order=set_order)
+    assert flips <= 2 * FLIPS_PER_MOVE * w.n_beads
+
+
+def test_star_melt_several_rounds_of_the_staged_architecture_kernel():
+    """400,000 three-arm stars (16 monomers, 6.4 M beads): 25,000 groups of 16 molecules for
+    at most 9472 resident warps, so every warp stages, sweeps and writes back several groups in its shared memory."""
+    w = workloads.Workload("stars_400k", ((400_000, (0,) + (0,) * 5 + (1,) * 10),), 16, 2, (12.0, 12.0, 10.0),
+                           (72, 72, 60), 18.0, 40.0, 0.1, 41, bonds=(_star_bonds(3, 5),))
+    assert w.n_chains / (256 // 16) > MAX_RESIDENT_WARPS
+    flips = lockstep(w, 2, xyz0=_tree_walk(w))
+    assert flips <= 2 * FLIPS_PER_MOVE * w.n_beads
+
+
+def test_molecule_parallel_scheme_several_rounds_of_the_staged_kernel():
+    """320,000 chains of N = 32 in the molecule-parallel scheme (Code 1): 10,000 groups of 32
+    chains for at most 9472 resident warps."""
+    w = workloads.Workload("code1_320k", ((320_000, workloads.diblock(32, 16)),), 32, 2, (16.0, 16.0, 10.0),
+                           (80, 80, 50), 30.0, 50.0, 0.1, 43)
+    assert w.n_chains / 32 > MAX_RESIDENT_WARPS
+    flips = lockstep(w, 1, scheme=1)
+    assert flips <= 5 * FLIPS_PER_MOVE * w.n_beads
+
+
+def test_smart_mc_step_where_the_position_budget_is_tight():
+    """Smart-MC with a_s = 0.025 R_e0^2 on short chains (N = N_ref = 4): the noise amplitude sqrt(2 a_s) = 0.22 is
+    where the approximate log / sin / cos of the GPU proposal use most of the 1e-6 R_e budget (their ~2e-6 relative
+    error of a Gaussian times 0.22), and -- unlike at C5's literal 0.05 on long chains -- a sizeable part of the moves
+    is accepted, so the position comparison is not vacuous."""
+    w = workloads.Workload("smc_tight", ((40_000, workloads.diblock(4, 2)),), 4, 2, (6.0, 6.0, 6.0), (20, 20, 20),
+                           12.0, 30.0, 0.1, 47, move="smc", smc_step=0.025)
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    sim = P.from_workload(w, xyz0=xyz0)
+    sim.step(1)
+    att, acc, _ = sim.stats()
+    sim.destroy()
+    assert acc / att > 0.02, acc / att
+    lockstep(w, 4, xyz0=xyz0)
+    lockstep(w, 2, xyz0=xyz0, kernel=P.KERNEL_GENERIC)
+
+
+def test_smart_mc_step_beyond_the_error_bound_is_refused():
+    """The proposal's approximations keep a displacement within 1e-6 R_e of the exact one up to a_s = 0.125
+    (sqrt(2 a_s) = 0.5); larger steps are refused rather than run outside the stated tolerance."""
+    sim = P.from_workload(workloads.c1())
+    sim.set_option(P.OPT_SMC_STEP, 0.125)
+    with pytest.raises(P.SomaError) as e:
+        sim.set_option(P.OPT_SMC_STEP, 0.1251)
+    assert e.value.code == -1 and "0.125" in str(e.value)
+    sim.destroy()
+
+
+# ---------------------------------------------------------------------------------------------
 # soma_init without positions: device-generated Gaussian walks vs the oracle's definition
 # ---------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("w", [workloads.c1(), workloads.small_cases()[7]], ids=lambda w: w.name)
@@ -751,6 +854,78 @@ def test_three_shards_on_one_gpu_equal_the_undivided_system_and_the_oracle(move,
         sim.destroy()
 
 
+@pytest.mark.parametrize("count_bits", [16, 32])
+def test_shard_parameters_set_before_the_first_exchange(count_bits):
+    """The natural order on a rank: soma_init_shard, then soma_set_external / soma_set_chi / the Hamiltonian, and only
+    then the first all-reduce and soma_shard_fields(ctx, 0).  In that window the shard's copy of the whole system's
+    occupation numbers is still empty; refreshing omega from it would be wrong and, with packed counts, would trip
+    the overflow check (halves against the number of beads) for good.  The calls must be accepted, raise no
+    SOMA_EOVERFLOW afterwards, and the fields must equal the undivided context's with the same parameters."""
+    from paper_1711_03828_b200.sharded import local_positions, shard_layout
+    w = workloads.Workload("shard_early", ((260, workloads.diblock(32, 16)), (40, workloads.homopolymer(8, 1))), 32, 2,
+                           (4.0, 4.0, 3.0), (8, 8, 6), 20.0, 50.0, 0.1, 13)
+    xyz0 = np.stack(workloads.gaussian_walks(w))
+    rng = np.random.default_rng(5)
+    ext = rng.normal(0.0, 0.3, (w.n_types, w.n_cells)).astype(np.float32)
+    forbidden = np.zeros(w.n_cells, np.uint8)
+    forbidden[:3] = 1
+
+    def configure(sim):
+        sim.set_option(P.OPT_COUNT_BITS, count_bits)
+        sim.set_external(ext, forbidden)
+        sim.set_chi(0, 1, 17.0)
+        sim.set_option(P.OPT_HAMILTONIAN, 1)
+
+    whole = P.from_workload(w, xyz0=xyz0)
+    configure(whole)
+    specs = [(n, np.asarray(t, np.uint8)) for n, t in w.specs]
+    shards = []
+    for rank in range(2):
+        local, first, n_global, slices = shard_layout(specs, rank, 2)
+        sim = P.Soma(local, w.N_ref, w.n_types, w.box, w.grid, w.chiN, w.kappaN, w.A, w.seed,
+                     xyz0=local_positions(xyz0, slices), spec_first_bead=first, global_n_beads=n_global)
+        configure(sim)                                     # before any soma_shard_fields
+        sim.sync()                                         # would report a sticky SOMA_EOVERFLOW
+        shards.append(sim)
+
+    def exchange(advance):
+        total = sum((sim.shard_exchange_get() for sim in shards), np.zeros(shards[0].shard_exchange()[1], np.uint32))
+        for sim in shards:
+            sim.shard_exchange_put(total)
+            sim.shard_fields(advance=advance)
+
+    exchange(False)
+    for sweep in range(3):
+        om_w, cnt_w = whole.fields()
+        for sim in shards:
+            sim.sync()
+            om_s, cnt_s = sim.fields()                     # soma_fields reports the overflow flag too
+            assert np.array_equal(cnt_s, cnt_w) and np.array_equal(om_s, om_w)
+        whole.step(1)
+        for sim in shards:
+            sim.shard_moves()
+        exchange(True)
+    # a parameter change while the numbers ARE current still refreshes omega at once
+    whole.set_chi(0, 1, 9.0)
+    for sim in shards:
+        sim.set_chi(0, 1, 9.0)
+        assert np.array_equal(sim.fields()[0], whole.fields()[0])
+    # ... and after new positions the window is open again
+    for sim, rank in zip(shards, range(2)):
+        _, _, _, slices = shard_layout(specs, rank, 2)
+        sim.set_positions(local_positions(xyz0, slices))
+        sim.set_option(P.OPT_HAMILTONIAN, 0)
+        sim.sync()
+    whole.set_positions(xyz0)
+    whole.set_option(P.OPT_HAMILTONIAN, 0)
+    exchange(False)
+    for sim in shards:
+        om_s, cnt_s = sim.fields()
+        assert np.array_equal(cnt_s, whole.fields()[1]) and np.array_equal(om_s, whole.fields()[0])
+        sim.destroy()
+    whole.destroy()
+
+
 @pytest.mark.parametrize("count_bits", [0, 16])
 def test_three_shards_reduce_their_exchange_arrays_in_the_field_kernel(count_bits):
     """Peer mode: no all-reduce -- every shard's field kernel reads the exchange arrays of all three (here three
@@ -771,6 +946,14 @@ def test_three_shards_reduce_their_exchange_arrays_in_the_field_kernel(count_bit
         sim.set_option(P.OPT_COUNT_BITS, count_bits)
         shards.append((sim, slices))
     addresses = [sim.shard_exchange()[0] for sim, _ in shards]
+    # a call that fails half-way (rank 1 by address, rank 2 by a handle that is none) leaves the context as it was:
+    # it can be repeated, and no peer is set meanwhile
+    with pytest.raises(P.SomaError) as e:
+        shards[0][0].shard_set_peers(3, 0, peer_addresses=[None, addresses[1], None], handles=[None, None, bytes(range(64))])
+    assert e.value.code == -2 and "rank 2" in str(e.value)
+    with pytest.raises(P.SomaError) as e:
+        shards[0][0].shard_set_peers(3, 0, peer_addresses=[None, addresses[1], None])
+    assert e.value.code == -1 and "rank 2" in str(e.value)
     for rank, (sim, _) in enumerate(shards):
         sim.shard_set_peers(3, rank, peer_addresses=addresses)
     for sim, _ in shards:
