@@ -95,10 +95,12 @@ __device__ __forceinline__ void philox4x32_10(uint32_t a, uint32_t b, uint32_t c
 //   h[3] = lo(a1 M0)                   d2 = h[3]
 // with a1 = hi(sweep_hi M1) ^ sweep_lo ^ rk[0][0].  Rounds 3-10 are the generic ones.  The output is
 // bit-identical to philox4x32_10; 18 instead of 20 wide multiplies per call.
-__device__ __forceinline__ void philox4x32_10_head(uint32_t gid, const uint32_t (&h)[4],
-                                                   const uint32_t (&rk)[10][2], uint32_t (&out)[4])
+// p1 = gid * M0, the one product of round 1 that differs between beads.  A lane of the fused kernel owns
+// consecutive beads, whose products differ by M0: it multiplies once and adds (exact in 64 bits).
+constexpr unsigned long long kPhiloxM0 = 0xD2511F53ull;
+__device__ __forceinline__ void philox4x32_10_head_p(unsigned long long p1, const uint32_t (&h)[4],
+                                                     const uint32_t (&rk)[10][2], uint32_t (&out)[4])
 {
-    const unsigned long long p1 = (unsigned long long)gid * 0xD2511F53ull;
     const uint32_t c1 = (uint32_t)(p1 >> 32) ^ h[0];
     const unsigned long long p2 = (unsigned long long)c1 * 0xCD9E8D57ull;
     uint32_t a = (uint32_t)(p2 >> 32) ^ h[1], b = (uint32_t)p2, c = (uint32_t)p1 ^ h[2], d = h[3];
@@ -114,6 +116,11 @@ __device__ __forceinline__ void philox4x32_10_head(uint32_t gid, const uint32_t 
         c = nc;
     }
     out[0] = a; out[1] = b; out[2] = c; out[3] = d;
+}
+__device__ __forceinline__ void philox4x32_10_head(uint32_t gid, const uint32_t (&h)[4],
+                                                   const uint32_t (&rk)[10][2], uint32_t (&out)[4])
+{
+    philox4x32_10_head_p((unsigned long long)gid * kPhiloxM0, h, rk, out);
 }
 
 // "Generate random permutation of the sets" (Code 2): a linear chain has two sets, so
@@ -240,20 +247,20 @@ __device__ __forceinline__ float neg2ln_u1(uint32_t w)
 // kMove 1: d uniform in (-A,A)^3, 2^23 equidistant values per axis.
 // kMove 2: g ~ N(0,1)^3 by Box-Muller on the words of call sub=0, u from call sub=1.
 template <int kMove>
-__device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
+__device__ __forceinline__ Draw draw_move_p(const MoveP& P, unsigned long long p1)   // p1 = gid * M0
 {
     Draw r;
     if (kMove == 1) {
         uint32_t w[4];
-        philox4x32_10_head(gid, P.head[0], P.rk, w);
+        philox4x32_10_head_p(p1, P.head[0], P.rk, w);
         r.a = fmaf(u23(w[0]), P.c1, P.c0);
         r.b = fmaf(u23(w[1]), P.c1, P.c0);
         r.c = fmaf(u23(w[2]), P.c1, P.c0);
         r.u = u23(w[3]) - 1.0f;
     } else {
         uint32_t w[4], v[4];
-        philox4x32_10_head(gid, P.head[0], P.rk, w);
-        philox4x32_10_head(gid, P.head[1], P.rk, v);
+        philox4x32_10_head_p(p1, P.head[0], P.rk, w);
+        philox4x32_10_head_p(p1, P.head[1], P.rk, v);
         // Box-Muller with sin.approx / cos.approx (MUFU) for the angle, taken in [-pi, pi) where the
         // approximations are best (absolute error 2^-21.4): sin(t) = -sin(t - pi), cos(t) = -cos(t - pi), and
         // t - pi = 2 pi (U23 - 1.5) with an exact subtraction.  A Gaussian is then off by <= ~2e-6, a
@@ -268,6 +275,12 @@ __device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
         r.u = u23(v[0]) - 1.0f;
     }
     return r;
+}
+
+template <int kMove>
+__device__ __forceinline__ Draw draw_move(const MoveP& P, uint32_t gid)
+{
+    return draw_move_p<kMove>(P, (unsigned long long)gid * kPhiloxM0);
 }
 
 // dE_nb = omega_k(c') - omega_k(c), Eq. 15; exactly 0 when the cell is kept.  The
@@ -529,8 +542,10 @@ fused_sweep_kernel(const MoveP P, float* __restrict__ x, float* __restrict__ y, 
         const uint32_t Cn = orig[kAnyN ? (kOrder ? (En >> 2) / (len >> 2) : min(tile_n, t_end - 1u) * cpt + cit) : i0n >> log2N];
 
         // 2. random numbers of the four moves
-        Draw q0 = draw_move<kMove>(P, gid), q1 = draw_move<kMove>(P, gid + 1u),
-             q2 = draw_move<kMove>(P, gid + 2u), q3 = draw_move<kMove>(P, gid + 3u);
+        // (round 1 of beads gid + 1 .. gid + 3 by addition: (gid + j) M0 = gid M0 + j M0, no carry out of 64 bits)
+        const unsigned long long p1 = (unsigned long long)gid * kPhiloxM0;
+        Draw q0 = draw_move_p<kMove>(P, p1), q1 = draw_move_p<kMove>(P, p1 + kPhiloxM0),
+             q2 = draw_move_p<kMove>(P, p1 + 2ull * kPhiloxM0), q3 = draw_move_p<kMove>(P, p1 + 3ull * kPhiloxM0);
         if (kAnyN && !active)                                 // an idle lane compares with u = +inf, which accepts nothing
             q0.u = q1.u = q2.u = q3.u = __int_as_float(0x7F800000);
 
